@@ -1,0 +1,289 @@
+"""CPU ORACLE for one EMC iteration (Expand -> Poisson log-likelihood -> normalise -> update ->
+Compress).  TEST INFRASTRUCTURE ONLY.
+
+This file is the plain, slow, obviously-correct restatement of what the CUDA path in
+`paper_1409_4256_b200/` must compute.  It is written from the paper and the readings in
+DESIGN.md §3, shares no code with the CUDA path, and may be imported only by `tests/`,
+`__graft_entry__.smoke()`, `bench.py`'s `cpu_baseline` leg and `bench.py --impl reference`.
+
+Every stage is a *direct formula*, so each function is that definition written out with numpy:
+fp32 inputs and outputs (the paper works in single precision), float64 arithmetic
+and accumulation inside.  Library primitives used as steps: numpy's float64 matmul, np.bincount
+(weighted scatter-add), np.exp/np.log.  No blocking, fusion or reordering beyond the formulas.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): every function below is pinned by closed forms,
+brute force on tiny inputs, invariants and independent library routines (scipy Rotation,
+scipy.ndimage.map_coordinates, scipy.stats.poisson, scipy.special.softmax/logsumexp); the table is
+in DESIGN.md §5.  The paper prints no worked numeric example of any stage, so no pin is a printed
+value (tests/golden/ holds only eq. (2.7)'s printed ladder).  No function is "parity unpinned".
+
+Notation (paper -> here): M_rot -> R (index r), M_data -> N (index d), M_pix -> P (index p),
+M_grid -> G = n^3 (index l); W_ij -> W[r,p]; blackboard W_l -> model[l]; P_jk -> P[r,d]; w_j -> w[r].
+"""
+from __future__ import annotations
+
+import numpy as np
+
+LOGW_FLOOR = np.float32(1e-30)      # DESIGN.md §3 G8: log(max(W, 1e-30))
+
+
+# ----------------------------------------------------------------------------------------------
+# Geometry: rotation, sample coordinates, base-corner index map   (eq. 2.9's argument R_j q_i)
+# ----------------------------------------------------------------------------------------------
+
+def rotation_matrix(quat):
+    """Active rotation matrix of a unit quaternion (w,x,y,z); PAPER.md:93 ("quaternions encode
+    rotations"), PAPER.md:66 (the sample position is R_j q_i).
+
+    Textbook formula, evaluated in float64 from the float32 components, every entry rounded once
+    to float32 (DESIGN.md §3 G4).  Returns [R,3,3] float32."""
+    qd = np.asarray(quat, dtype=np.float32).astype(np.float64)
+    w, x, y, z = qd[..., 0], qd[..., 1], qd[..., 2], qd[..., 3]
+    m = np.empty(qd.shape[:-1] + (3, 3), dtype=np.float64)
+    m[..., 0, 0] = 1.0 - 2.0 * (y * y + z * z)
+    m[..., 0, 1] = 2.0 * (x * y - w * z)
+    m[..., 0, 2] = 2.0 * (x * z + w * y)
+    m[..., 1, 0] = 2.0 * (x * y + w * z)
+    m[..., 1, 1] = 1.0 - 2.0 * (x * x + z * z)
+    m[..., 1, 2] = 2.0 * (y * z - w * x)
+    m[..., 2, 0] = 2.0 * (x * z - w * y)
+    m[..., 2, 1] = 2.0 * (y * z + w * x)
+    m[..., 2, 2] = 1.0 - 2.0 * (x * x + y * y)
+    return m.astype(np.float32)
+
+
+def sample_coords(quat, q, n):
+    """Grid coordinates x[r,p,:] = R_r q_p + c of every sample, c = n/2 (DESIGN.md §3 G5).
+
+    float32 arithmetic with every multiply and add rounded separately, in this order
+    (DESIGN.md §3 G4 -- this sequence is what makes the index map bit-exact on any machine):
+        x_a = ((R_a0*q_x + R_a1*q_y) + R_a2*q_z) + c
+    Returns [R,P,3] float32."""
+    rm = rotation_matrix(quat)                                  # [R,3,3] f32
+    q = np.asarray(q, dtype=np.float32)
+    c = np.float32(n / 2.0)
+    qx, qy, qz = q[None, :, 0], q[None, :, 1], q[None, :, 2]
+    out = np.empty((rm.shape[0], q.shape[0], 3), dtype=np.float32)
+    for a in range(3):
+        t0 = rm[:, a, 0, None] * qx                             # each op is one float32 rounding
+        t1 = rm[:, a, 1, None] * qy
+        t2 = rm[:, a, 2, None] * qz
+        out[:, :, a] = ((t0 + t1) + t2) + c
+    return out
+
+
+def base_corner(x, n):
+    """Base corner b = floor(x), fractional offsets t = x - b, validity and linear index.
+
+    Valid iff 0 <= b_a <= n-2 on all three axes (all 8 neighbours exist; DESIGN.md §3 G7).
+    idx = (b_x*n + b_y)*n + b_z (z fastest, G5) or -1.  Returns (b int32, t float32, valid, idx)."""
+    b = np.floor(x)
+    t = (x - b).astype(np.float32)                              # exact in float32
+    b = b.astype(np.int32)
+    valid = np.all((b >= 0) & (b <= n - 2), axis=-1)
+    idx = (b[..., 0].astype(np.int64) * n + b[..., 1]) * n + b[..., 2]
+    idx = np.where(valid, idx, -1).astype(np.int32)
+    return b, t, valid, idx
+
+
+def index_map(quat, q, n):
+    """The rotation -> voxel index map idx[r,p] (int32, -1 outside the grid).  Bit-exact target."""
+    return base_corner(sample_coords(quat, q, n), n)[3]
+
+
+def _corner_weights(t):
+    """Trilinear weights f for the 8 corners (i,j,k) in {0,1}^3, as float64 [..., 8] in the order
+    corner = 4i + 2j + k; per axis the weight is (1 - t) for offset 0 and t for offset 1.
+    This is the interpolation kernel f of eq. (2.8), PAPER.md:106-109 (f := trilinear, G-A9)."""
+    td = t.astype(np.float64)
+    w0 = 1.0 - td
+    w1 = td
+    ws = []
+    for i in (0, 1):
+        for j in (0, 1):
+            for k in (0, 1):
+                ws.append((w1 if i else w0)[..., 0] * (w1 if j else w0)[..., 1] * (w1 if k else w0)[..., 2])
+    return np.stack(ws, axis=-1)
+
+
+def _corner_offsets(n):
+    return np.array([(i * n + j) * n + k for i in (0, 1) for j in (0, 1) for k in (0, 1)], dtype=np.int64)
+
+
+# ----------------------------------------------------------------------------------------------
+# Stage 1: Expand (e-step), eq. (2.9)
+# ----------------------------------------------------------------------------------------------
+
+def expand(model, q, quat, chunk=64):
+    """W[r,p] = sum_l f(p_l - R_r q_p) model[l]  (eq. 2.9): trilinear read of the model at every
+    sample; samples outside the grid give W = 0 (G7).  Computed for every pixel, masked or not.
+    Returns (W [R,P] float32, idx [R,P] int32)."""
+    model = np.asarray(model, dtype=np.float32)
+    n = model.shape[0]
+    flat = model.reshape(-1).astype(np.float64)
+    quat = np.asarray(quat, dtype=np.float32)
+    n_rot, n_pix = quat.shape[0], np.asarray(q).shape[0]
+    w_out = np.zeros((n_rot, n_pix), dtype=np.float32)
+    idx_out = np.empty((n_rot, n_pix), dtype=np.int32)
+    off = _corner_offsets(n)
+    for r0 in range(0, n_rot, chunk):
+        r1 = min(n_rot, r0 + chunk)
+        _, t, valid, idx = base_corner(sample_coords(quat[r0:r1], q, n), n)
+        f = _corner_weights(t)                                  # [r,P,8]
+        base = np.where(valid, idx, 0).astype(np.int64)
+        vals = flat[base[..., None] + off]                      # [r,P,8]
+        w = (f * vals).sum(axis=-1)
+        w_out[r0:r1] = np.where(valid, w, 0.0).astype(np.float32)
+        idx_out[r0:r1] = idx
+    return w_out, idx_out
+
+
+# ----------------------------------------------------------------------------------------------
+# Stage 2: Poisson log-likelihood, north_star formula; Poisson model of PAPER.md:68
+# ----------------------------------------------------------------------------------------------
+
+def log_slices(w, idx):
+    """logW[r,p] = log(max(W, 1e-30)) for samples inside the grid, 0 outside (G7, G8)."""
+    w = np.asarray(w, dtype=np.float32)
+    lw = np.log(np.maximum(w, LOGW_FLOOR).astype(np.float64))
+    return np.where(np.asarray(idx) >= 0, lw, 0.0)
+
+
+def loglik(w, idx, counts, mask):
+    """L[r,d] = sum_p mask_p (K[d,p] log W[r,p] - W[r,p])   (north_star stage 2; the -log K! term of
+    the Poisson pmf is constant in r and dropped, G2).
+
+    Also returns A[r,d] = sum_p mask_p (K |log W| + W), the scale the L tolerance refers to
+    (DESIGN.md §4 T1).  Returns (L float64 [R,N], A float64 [R,N])."""
+    use = _use(mask, np.asarray(w).shape[1])
+    wd = np.asarray(w, dtype=np.float32).astype(np.float64)[:, use]
+    lw = log_slices(w, idx)[:, use]
+    k = np.asarray(counts)[:, use].astype(np.float64)           # [N,Pu]
+    s = wd.sum(axis=1)
+    big_l = lw @ k.T - s[:, None]
+    big_a = np.abs(lw) @ k.T + np.abs(wd).sum(axis=1)[:, None]
+    return big_l, big_a
+
+
+def _use(mask, n_pix):
+    if mask is None:
+        return np.ones(n_pix, dtype=bool)
+    return np.asarray(mask).astype(bool)
+
+
+# ----------------------------------------------------------------------------------------------
+# Stage 3: normalisation over rotations (reconstructed eq. 2.4)
+# ----------------------------------------------------------------------------------------------
+
+def normalize(big_l, weight):
+    """P[r,d] = w_r T_rd / sum_r' w_r' T_r'd with T = exp(L), evaluated max-subtracted
+    ("some care ... finite precision"; only max and sum are needed):
+        a = L + log w_r;  m_d = max_r a;  e = exp(a - m_d);  P = e / sum_r e.
+    Also s[r] = sum_d P[r,d] and the total log-likelihood LL = sum_d (m_d + log sum_r e).
+    `big_l` is taken as given (tests feed the float32-rounded L, DESIGN.md §4 T2).
+    Returns (P float64 [R,N], s float64 [R], LL float)."""
+    a = np.asarray(big_l).astype(np.float64) + np.log(np.asarray(weight).astype(np.float64))[:, None]
+    m = a.max(axis=0)
+    e = np.exp(a - m[None, :])
+    z = e.sum(axis=0)
+    p = e / z[None, :]
+    return p, p.sum(axis=1), float((m + np.log(z)).sum())
+
+
+# ----------------------------------------------------------------------------------------------
+# Stage 4: slice update (M-step), eq. (2.5) with phi == 1 / eq. (2.11)
+# ----------------------------------------------------------------------------------------------
+
+def update(p, counts, mask):
+    """W'[r,p] = sum_d P[r,d] K[d,p] / sum_d P[r,d]   (eq. 2.5 with the printed index typo read as
+    P_jk, G10).  Masked pixels give 0 (G16); rows with s[r] = 0 give 0 (G17).
+    `p` is taken as given (the float32 responsibilities).  Returns (W' float32 [R,P], s float64)."""
+    pd = np.asarray(p).astype(np.float64)
+    k = np.asarray(counts)
+    use = _use(mask, k.shape[1])
+    s = pd.sum(axis=1)
+    num = pd @ np.where(use[None, :], k, 0).astype(np.float64)  # eq. (2.11)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        wn = np.where(s[:, None] > 0, num / s[:, None], 0.0)
+    wn[:, ~use] = 0.0
+    return wn.astype(np.float32), s
+
+
+# ----------------------------------------------------------------------------------------------
+# Stage 5: Compress (c-step), eq. (2.10) / (2.12)
+# ----------------------------------------------------------------------------------------------
+
+def compress(wn, q, quat, mask, n, slice_w=None, chunk=64):
+    """model'[l] = sum_{r,p} f(p_l - R_r q_p) om_r W'[r,p] / sum_{r,p} f(p_l - R_r q_p) om_r
+    over unmasked samples inside the grid, 0 where the denominator is 0 (G17).
+
+    om_r = 1 (and slices with slice_w[r] == 0 skipped) is eq. (2.10); om_r = s[r] = sum_d P[r,d]
+    applied to numerator and denominator is exactly eq. (2.12) with W' normalised (G6).  The
+    numerator and denominator are accumulated separately, the division is last.
+    `slice_w` None = all ones.  `weighted` selection is the caller's: pass om_r itself.
+    Returns (model' float32 [n,n,n], num float64 [G], den float64 [G])."""
+    wn = np.asarray(wn, dtype=np.float32)
+    quat = np.asarray(quat, dtype=np.float32)
+    n_rot, n_pix = wn.shape
+    use = _use(mask, n_pix)
+    om = np.ones(n_rot, dtype=np.float64) if slice_w is None else np.asarray(slice_w).astype(np.float64)
+    g = n * n * n
+    num = np.zeros(g, dtype=np.float64)
+    den = np.zeros(g, dtype=np.float64)
+    off = _corner_offsets(n)
+    for r0 in range(0, n_rot, chunk):
+        r1 = min(n_rot, r0 + chunk)
+        _, t, valid, idx = base_corner(sample_coords(quat[r0:r1], q, n), n)
+        take = valid & use[None, :] & (om[r0:r1, None] > 0)
+        f = _corner_weights(t)[take] * np.broadcast_to(om[r0:r1, None], valid.shape)[take][:, None]
+        tgt = idx[take].astype(np.int64)[:, None] + off[None, :]
+        val = wn[r0:r1].astype(np.float64)[take]
+        num += np.bincount(tgt.reshape(-1), weights=(f * val[:, None]).reshape(-1), minlength=g)
+        den += np.bincount(tgt.reshape(-1), weights=f.reshape(-1), minlength=g)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        model = np.where(den > 0, num / den, 0.0)
+    return model.astype(np.float32).reshape(n, n, n), num, den
+
+
+# ----------------------------------------------------------------------------------------------
+# One iteration (Algorithm 1), with pattern chunks (config 4, G9)
+# ----------------------------------------------------------------------------------------------
+
+def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=False):
+    """expand -> [per pattern chunk: loglik -> normalize] -> update -> compress.
+
+    Stage boundaries carry float32 (W, L, P, W'), as the C-ABI does.  The soft-max is over
+    rotations per pattern, so pattern chunks are independent in stages 2-3; s[r] and the update
+    numerators add up over chunks and are divided after the last one (G9).
+    `weighted` selects eq. (2.12) (om_r = s[r]) instead of eq. (2.10) (om_r = 1).
+    Returns dict(model, W, idx, L, P, s, Wn, LL)."""
+    counts = np.asarray(counts)
+    n = np.asarray(model).shape[0]
+    n_pat = counts.shape[0]
+    chunk = n_pat if not n_pat_chunk else n_pat_chunk
+    w, idx = expand(model, q, quat)
+    use = _use(mask, counts.shape[1])
+    l_all = np.empty((w.shape[0], n_pat), dtype=np.float32)
+    p_all = np.empty((w.shape[0], n_pat), dtype=np.float32)
+    s = np.zeros(w.shape[0], dtype=np.float64)
+    num = np.zeros(w.shape, dtype=np.float64)
+    ll = 0.0
+    for d0 in range(0, n_pat, chunk):
+        d1 = min(n_pat, d0 + chunk)
+        big_l, _ = loglik(w, idx, counts[d0:d1], mask)
+        l32 = big_l.astype(np.float32)
+        p, _, ll_c = normalize(l32, weight)
+        p32 = p.astype(np.float32)
+        l_all[:, d0:d1] = l32
+        p_all[:, d0:d1] = p32
+        ll += ll_c
+        pd = p32.astype(np.float64)
+        s += pd.sum(axis=1)
+        num += pd @ np.where(use[None, :], counts[d0:d1], 0).astype(np.float64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        wn = np.where(s[:, None] > 0, num / s[:, None], 0.0)
+    wn[:, ~use] = 0.0
+    wn = wn.astype(np.float32)
+    om = s.astype(np.float32) if weighted else (s > 0).astype(np.float32)
+    new_model, _, den = compress(wn, q, quat, mask, n, slice_w=om)
+    return dict(model=new_model, W=w, idx=idx, L=l_all, P=p_all, s=s, Wn=wn, LL=ll, den=den)
