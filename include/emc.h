@@ -1,0 +1,183 @@
+/*
+ * emc.h -- C ABI of libemc: one iteration of the Expansion-Maximization-Compression (EMC)
+ * algorithm of arXiv 1409.4256 (Ekeberg, Engblom, Liu) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are "PAPER.md:<line>" (= /root/reference/PAPER.md of the build container) plus the
+ * equation they fall in, and "DESIGN.md §3 Gn" for the readings taken where the paper is silent.
+ *
+ * Notation (paper -> here): M_rot -> R (index r), M_data -> N (index d), M_pix -> P (index p),
+ * M_grid -> G = n^3 (index l); W_ij -> W[r,p]; model grid (blackboard W_l) -> model[l];
+ * P_jk -> P[r,d]; w_j -> weight[r].
+ *
+ * Conventions for EVERY entry point
+ *  - Every array pointer is a DEVICE pointer owned by the caller (the Python binding allocates
+ *    them with PyTorch) unless the comment says "host".  The library allocates nothing: scratch
+ *    comes from the caller's workspace `ws` of at least emc_workspace_bytes(...) bytes, 256-byte
+ *    aligned.  Nothing in the workspace survives a call except where stated.
+ *  - `stream` is a cudaStream_t.  Calls validate their arguments synchronously, enqueue their
+ *    kernels on `stream` and return without synchronising.
+ *  - Errors are returned as negative emc_status values, never thrown or aborted.  Conditions that
+ *    only the device can see (a photon count too large for the exact 16-bit operand format) are
+ *    recorded in the workspace header and reported by emc_check().
+ *  - Matrices are row-major: W is [R][P], L and P are [R][N] with row pitch `ld_n` floats
+ *    (ld_n >= N, a multiple of 4; the binding uses N rounded up to 64).  The model is
+ *    [n][n][n] with z fastest, voxel (i,j,k) at integer coordinates, origin c = n/2 on every axis
+ *    (DESIGN.md §3 G5).
+ */
+#ifndef EMC_H_
+#define EMC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define EMC_API __attribute__((visibility("default")))
+#else
+#define EMC_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    EMC_OK = 0,
+    EMC_ERR_ARG = -1,          /* null pointer, non-positive size, misaligned pointer or pitch */
+    EMC_ERR_UNSUPPORTED = -2,  /* a size outside what the kernels index (see each call) */
+    EMC_ERR_WORKSPACE = -3,    /* ws is NULL, misaligned or smaller than emc_workspace_bytes() */
+    EMC_ERR_CUDA = -4,         /* a CUDA runtime/driver call failed (emc_last_cuda_error()) */
+    EMC_ERR_COUNT_RANGE = -5   /* an unmasked photon count exceeds EMC_MAX_COUNT (emc_check) */
+} emc_status;
+
+typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
+
+/* Largest photon count in an unmasked pixel that the exact 16-bit tensor-core operands hold
+ * (bf16 holds every integer up to 256; DESIGN.md §6 "precision scheme").  Saturated pixels are
+ * expected to be masked. */
+#define EMC_MAX_COUNT 256
+
+/* flags */
+#define EMC_COMPRESS_WEIGHTED 0x1u /* eq. (2.12): slice r enters Compress with
+                                      weight s[r] = sum_d P[r,d]; default is eq. (2.10), weight 1 */
+#define EMC_ACCUMULATE        0x2u /* emc_normalize: add into s / loglik; emc_update: add into Wnew
+                                      (pattern chunks, DESIGN.md §3 G9) */
+#define EMC_UPDATE_RAW        0x4u /* emc_update: leave Wnew as the numerator of eq. (2.11),
+                                      do not divide by s[r] */
+#define EMC_PLANES_2          0x8u /* opt-in: 2 instead of 3 bf16 planes for P in emc_update
+                                      (reported separately) */
+#define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
+                                        bisecting aid for the tcgen05 path, never the default) */
+
+/* The 3D intensity model on its Cartesian grid (p_l). */
+typedef struct {
+    int n;              /* grid is n x n x n, 2 <= n <= 1024 */
+    const float *model; /* [n][n][n], z fastest */
+} emc_model;
+
+/* Detector geometry: the Ewald-sphere coordinates q_i of every pixel. */
+typedef struct {
+    int n_pix;           /* P */
+    const float *q;      /* [P][3] (x,y,z) in voxel units relative to the origin c */
+    const uint8_t *mask; /* [P], 1 = use, 0 = missing/saturated; NULL = use all */
+} emc_detector;
+
+/* The discretised rotation space (R_j) with prior weights w_j. */
+typedef struct {
+    int n_rot;           /* R */
+    const float *quat;   /* [R][4] unit quaternions (w,x,y,z), active rotation */
+    const float *weight; /* [R] prior weights w_j > 0, or NULL = 1/R */
+} emc_rotations;
+
+/* The measured frames K_k of photon counts. */
+typedef struct {
+    int n_pat;           /* N */
+    const void *counts;  /* [N][P] row-major; values in masked pixels are ignored */
+    emc_count_type type;
+} emc_patterns;
+
+/* Bytes of workspace sufficient for any call below at these sizes.  n_pat_chunk = patterns
+ * resident per chunk (= N when not chunked).  Returns 0 on invalid sizes. */
+EMC_API size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags);
+
+/* Stage 1, Expand (e-step), eq. (2.9), PAPER.md:113-116:
+ *   W[r,p] = sum_l f(p_l - R_r q_p) model[l],  f = trilinear weights of the 8 voxels around
+ *   x = R_r q_p + c.  Samples whose 8 neighbours are not all inside the grid give W = 0 (G7).
+ * Computed for every pixel, masked or not.
+ *   W   [R][P] float, out.
+ *   idx [R][P] int32, out, or NULL: linear index (b_x*n + b_y)*n + b_z of the base corner
+ *       b = floor(x), or -1 outside the grid.  The coordinate arithmetic is pinned (DESIGN.md §3
+ *       G4) so this map is bit-exact against the oracle. */
+EMC_API emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                      float *W, int32_t *idx, void *stream);
+
+/* Stage 2, Poisson log-likelihood (north_star stage 2; Poisson model of PAPER.md:68; the E-step
+ * numerator of PAPER.md:166):
+ *   L[r,d] = sum_{p: mask} ( K[d,p] * logW[r,p] - W[r,p] ),
+ *   logW = log(max(W, 1e-30)) inside the grid, 0 outside (G7, G8).
+ *   W   [R][P] float, in (as written by emc_expand).
+ *   idx [R][P] int32, in, or NULL = every sample is inside the grid.
+ *   L   [R][ld_n] float, out (columns >= N are not written). */
+EMC_API emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *det,
+                      const emc_patterns *pat, int n_rot, float *L, int ld_n, unsigned flags,
+                      void *ws, size_t ws_bytes, void *stream);
+
+/* Stage 3, normalisation over rotations (reconstructed eq. (2.4)):
+ *   a = L[r,d] + log w_r;  m_d = max_r a;  P[r,d] = exp(a - m_d) / sum_r exp(a - m_d).
+ *   L      [R][ld_n] float, in.
+ *   P      [R][ld_n] float, out.
+ *   s      [R] float, out: s[r] = sum_d P[r,d]            (added to with EMC_ACCUMULATE)
+ *   loglik device double, out: sum_d (m_d + log sum_r exp(a - m_d))   (added to with EMC_ACCUMULATE)
+ *   Either of s, loglik may be NULL. */
+EMC_API emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
+                         float *s, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
+                         void *stream);
+
+/* Stage 4, slice update (M-step), eq. (2.5) with phi == 1 / eq. (2.11), PAPER.md:84-85, 124-125:
+ *   Wnew[r,p] = sum_d P[r,d] K[d,p] / s[r]   for unmasked p, 0 for masked p and where s[r] = 0.
+ *   P [R][ld_n] float, in;  s [R] float, in (ignored with EMC_UPDATE_RAW);  Wnew [R][P] float, out.
+ *   EMC_UPDATE_RAW leaves the numerator; EMC_ACCUMULATE (implies RAW) adds it into Wnew. */
+EMC_API emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detector *det,
+                      const emc_patterns *pat, int n_rot, float *Wnew, unsigned flags, void *ws,
+                      size_t ws_bytes, void *stream);
+
+/* Stage 5, Compress (c-step), eq. (2.10) / (2.12), PAPER.md:118-130, 166, 192:
+ *   num[l] = sum_{r,p} f om_r Wnew[r,p],  den[l] = sum_{r,p} f om_r  over unmasked samples inside
+ *   the grid, same f as Expand;  model_out[l] = den > 0 ? num/den : 0 (division last).
+ *   om_r = 1 if slice_w == NULL; else slices with slice_w[r] == 0 are skipped and
+ *   om_r = slice_w[r] with EMC_COMPRESS_WEIGHTED (eq. 2.12), 1 without (eq. 2.10).
+ *   model_out [n^3] float, out;  den_out [n^3] float, out or NULL. */
+EMC_API emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detector *det,
+                        const emc_rotations *rot, int n, float *model_out, float *den_out,
+                        unsigned flags, void *ws, size_t ws_bytes, void *stream);
+
+/* Algorithm 1: `n_iter` iterations of stages 1-5 on one stream with no host
+ * synchronisation; model' of one iteration is the model of the next (same rotation list).
+ * Patterns are processed in chunks of n_pat_chunk (0 = all at once): stages 2-3 per chunk, s[r]
+ * and the update numerators summed over chunks, divided after the last (DESIGN.md §3 G9).
+ *   pat->counts may be a PINNED HOST pointer when flags has EMC_PATTERNS_ON_HOST: each chunk is
+ *   then copied to the device inside the call.
+ *   model_out [n^3] float, out (may not alias model->model).
+ *   P_out     [R][ld_n] float of the LAST iteration, out, or NULL (ld_n >= N; needs one chunk).
+ *   loglik    [n_iter] device doubles, out: total log-likelihood of each iteration. */
+#define EMC_PATTERNS_ON_HOST 0x10u
+EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                       const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
+                       float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
+                       size_t ws_bytes, void *stream);
+
+/* Synchronises `stream` and reports what only the device saw during calls that used `ws`:
+ * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (results are then undefined),
+ * EMC_ERR_CUDA if the stream is in error.  Clears the record. */
+EMC_API emc_status emc_check(void *ws, void *stream);
+
+/* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
+EMC_API uint64_t emc_launch_count(void);
+
+EMC_API const char *emc_strerror(emc_status status);
+EMC_API const char *emc_last_cuda_error(void); /* text of the last CUDA failure seen by this thread */
+EMC_API const char *emc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EMC_H_ */

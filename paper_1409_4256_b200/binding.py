@@ -1,0 +1,283 @@
+"""Thin ctypes binding of libemc (include/emc.h): same names, argument marshalling only.
+
+PyTorch provides device memory and streams; every step of the path runs in the library's CUDA
+kernels.  There is no CPU fallback: if libemc.so cannot be loaded or a call fails, an EmcError is
+raised.  Nothing here imports the oracle.
+"""
+from __future__ import annotations
+
+import ctypes
+import pathlib
+from ctypes import POINTER, Structure, c_char_p, c_double, c_int, c_size_t, c_uint, c_uint64, c_void_p
+
+import torch
+
+from . import build as _build
+
+EMC_OK = 0
+EMC_ERR_ARG, EMC_ERR_UNSUPPORTED, EMC_ERR_WORKSPACE, EMC_ERR_CUDA, EMC_ERR_COUNT_RANGE = -1, -2, -3, -4, -5
+EMC_I32, EMC_U16, EMC_U8 = 0, 1, 2
+EMC_MAX_COUNT = 256
+EMC_COMPRESS_WEIGHTED = 0x1
+EMC_ACCUMULATE = 0x2
+EMC_UPDATE_RAW = 0x4
+EMC_PLANES_2 = 0x8
+EMC_PATTERNS_ON_HOST = 0x10
+EMC_DEBUG_SIMT = 0x100
+
+# every symbol include/emc.h declares (tests check the library exports all of them)
+SYMBOLS = ("emc_workspace_bytes", "emc_expand", "emc_loglik", "emc_normalize", "emc_update", "emc_compress",
+           "emc_iterate", "emc_check", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+
+
+class EmcError(RuntimeError):
+    def __init__(self, status, where):
+        lib = load()
+        msg = lib.emc_strerror(status).decode()
+        if status == EMC_ERR_CUDA:
+            msg += ": " + lib.emc_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({status})")
+        self.status = status
+
+
+class _Model(Structure):
+    _fields_ = [("n", c_int), ("model", c_void_p)]
+
+
+class _Detector(Structure):
+    _fields_ = [("n_pix", c_int), ("q", c_void_p), ("mask", c_void_p)]
+
+
+class _Rotations(Structure):
+    _fields_ = [("n_rot", c_int), ("quat", c_void_p), ("weight", c_void_p)]
+
+
+class _Patterns(Structure):
+    _fields_ = [("n_pat", c_int), ("counts", c_void_p), ("type", c_int)]
+
+
+_LIB = None
+
+
+def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
+    """dlopen libemc.so (built in-tree by build.py) and declare the prototypes of include/emc.h."""
+    global _LIB
+    if _LIB is not None and path is None:
+        return _LIB
+    p = pathlib.Path(path) if path else _build.LIB
+    if not p.exists():
+        p = _build.build()          # needs nvcc; raises if it cannot be built -- no fallback
+    lib = ctypes.CDLL(str(p))
+    vp, sz, ci, cu = c_void_p, c_size_t, c_int, c_uint
+    lib.emc_workspace_bytes.restype = sz
+    lib.emc_workspace_bytes.argtypes = [ci, ci, ci, ci, cu]
+    lib.emc_expand.restype = ci
+    lib.emc_expand.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), vp, vp, vp]
+    lib.emc_loglik.restype = ci
+    lib.emc_loglik.argtypes = [vp, vp, POINTER(_Detector), POINTER(_Patterns), ci, vp, ci, cu, vp, sz, vp]
+    lib.emc_normalize.restype = ci
+    lib.emc_normalize.argtypes = [vp, POINTER(_Rotations), ci, ci, vp, vp, vp, cu, vp, sz, vp]
+    lib.emc_update.restype = ci
+    lib.emc_update.argtypes = [vp, ci, vp, POINTER(_Detector), POINTER(_Patterns), ci, vp, cu, vp, sz, vp]
+    lib.emc_compress.restype = ci
+    lib.emc_compress.argtypes = [vp, vp, POINTER(_Detector), POINTER(_Rotations), ci, vp, vp, cu, vp, sz, vp]
+    lib.emc_iterate.restype = ci
+    lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
+                                ci, ci, vp, vp, ci, vp, cu, vp, sz, vp]
+    lib.emc_check.restype = ci
+    lib.emc_check.argtypes = [vp, vp]
+    lib.emc_launch_count.restype = c_uint64
+    lib.emc_launch_count.argtypes = []
+    for name in ("emc_strerror", "emc_last_cuda_error", "emc_version"):
+        getattr(lib, name).restype = c_char_p
+    lib.emc_strerror.argtypes = [ci]
+    if path is None:
+        _LIB = lib
+    return lib
+
+
+# ---------------------------------------------------------------------------- marshalling helpers
+
+_COUNT_TYPES = {torch.int32: EMC_I32, torch.uint16: EMC_U16, torch.uint8: EMC_U8}
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> int:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def _opt(t, dtype, name):
+    return None if t is None else _dev(t, dtype, name)
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _check(status: int, where: str):
+    if status != EMC_OK:
+        raise EmcError(status, where)
+
+
+def ld_for(n_pat: int) -> int:
+    """Row pitch (floats) the binding uses for L and P: N rounded up to 64."""
+    return (n_pat + 63) // 64 * 64
+
+
+def _detector(q, mask):
+    n_pix = q.shape[0]
+    if mask is not None and mask.shape[0] != n_pix:
+        raise ValueError("mask length != number of pixels")
+    return _Detector(n_pix, _dev(q, torch.float32, "q"), _opt(mask, torch.uint8, "mask"))
+
+
+def _rotations(quat, weight):
+    if weight is not None and weight.shape[0] != quat.shape[0]:
+        raise ValueError("weight length != number of rotations")
+    return _Rotations(quat.shape[0], _dev(quat, torch.float32, "quat"), _opt(weight, torch.float32, "weight"))
+
+
+def _patterns(counts, n_pix, on_host=False):
+    if counts.dtype not in _COUNT_TYPES or counts.dim() != 2 or counts.shape[1] != n_pix or not counts.is_contiguous():
+        raise TypeError("counts: expected a contiguous [N, P] tensor of int32, uint16 or uint8")
+    if on_host:
+        if counts.is_cuda or not counts.is_pinned():
+            raise TypeError("counts: EMC_PATTERNS_ON_HOST needs a pinned host tensor")
+    elif not counts.is_cuda:
+        raise TypeError("counts: expected a CUDA tensor")
+    return _Patterns(counts.shape[0], counts.data_ptr(), _COUNT_TYPES[counts.dtype])
+
+
+def emc_workspace_bytes(n: int, n_pix: int, n_rot: int, n_pat_chunk: int, flags: int = 0) -> int:
+    return load().emc_workspace_bytes(n, n_pix, n_rot, n_pat_chunk, flags)
+
+
+def make_workspace(n, n_pix, n_rot, n_pat_chunk, flags=0, device="cuda") -> torch.Tensor:
+    nbytes = emc_workspace_bytes(n, n_pix, n_rot, n_pat_chunk, flags)
+    if nbytes == 0:
+        raise EmcError(EMC_ERR_UNSUPPORTED, "emc_workspace_bytes")
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def _ws(ws, n, n_pix, n_rot, n_chunk, flags=0):
+    if ws is None:
+        ws = make_workspace(n, n_pix, n_rot, n_chunk, flags)
+    return ws, ws.data_ptr(), ws.numel()
+
+
+# ---------------------------------------------------------------------------- the six calls
+
+def emc_expand(model, q, quat, want_idx=True):
+    """Stage 1 (eq. 2.9).  Returns (W [R,P] float32, idx [R,P] int32 or None)."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, None)
+    rot = _rotations(quat, None)
+    w = torch.empty((rot.n_rot, det.n_pix), dtype=torch.float32, device=model.device)
+    idx = torch.empty((rot.n_rot, det.n_pix), dtype=torch.int32, device=model.device) if want_idx else None
+    _check(load().emc_expand(m, det, rot, w.data_ptr(), idx.data_ptr() if want_idx else None, _stream()), "emc_expand")
+    return w, idx
+
+
+def emc_loglik(w, idx, q, mask, counts, flags=0, ws=None):
+    """Stage 2.  Returns L as a [R, N] view of a [R, ld_n] float32 tensor."""
+    n_rot, n_pix = w.shape
+    det = _detector(q, mask)
+    pat = _patterns(counts, n_pix)
+    ld = ld_for(pat.n_pat)
+    big_l = torch.empty((n_rot, ld), dtype=torch.float32, device=w.device)
+    ws, wp, wb = _ws(ws, 2, n_pix, n_rot, pat.n_pat)
+    _check(load().emc_loglik(_dev(w, torch.float32, "W"), _opt(idx, torch.int32, "idx"), det, pat, n_rot,
+                             big_l.data_ptr(), ld, flags, wp, wb, _stream()), "emc_loglik")
+    return big_l[:, :pat.n_pat]
+
+
+def _pitched(x, name):
+    """(base pointer, pitch) of a [R, N] float32 view whose rows are `pitch` floats apart."""
+    if x.dtype != torch.float32 or not x.is_cuda or x.dim() != 2 or x.stride(1) != 1:
+        raise TypeError(f"{name}: expected a 2-D CUDA float32 tensor with unit column stride")
+    return x.data_ptr(), x.stride(0)
+
+
+def emc_normalize(big_l, quat, weight, flags=0, s=None, loglik=None, ws=None):
+    """Stage 3.  Returns (P [R,N] view, s [R], loglik 1-element float64 tensor)."""
+    n_rot, n_pat = big_l.shape
+    lp, ld = _pitched(big_l, "L")
+    rot = _rotations(quat, weight)
+    p = torch.empty((n_rot, ld), dtype=torch.float32, device=big_l.device)
+    if s is None:
+        s = torch.zeros(n_rot, dtype=torch.float32, device=big_l.device)
+    if loglik is None:
+        loglik = torch.zeros(1, dtype=torch.float64, device=big_l.device)
+    ws, wp, wb = _ws(ws, 2, 1, n_rot, n_pat)
+    _check(load().emc_normalize(lp, rot, n_pat, ld, p.data_ptr(), s.data_ptr(), loglik.data_ptr(), flags, wp, wb,
+                                _stream()), "emc_normalize")
+    return p[:, :n_pat], s, loglik
+
+
+def emc_update(p, s, q, mask, counts, flags=0, wnew=None, ws=None):
+    """Stage 4 (eq. 2.5 / 2.11).  Returns W' [R,P] float32."""
+    n_rot, n_pat = p.shape
+    pp, ld = _pitched(p, "P")
+    det = _detector(q, mask)
+    pat = _patterns(counts, det.n_pix)
+    if pat.n_pat != n_pat:
+        raise ValueError("P columns != number of patterns")
+    if wnew is None:
+        wnew = torch.empty((n_rot, det.n_pix), dtype=torch.float32, device=p.device)
+    ws, wp, wb = _ws(ws, 2, det.n_pix, n_rot, n_pat)
+    _check(load().emc_update(pp, ld, _opt(s, torch.float32, "s"), det, pat, n_rot,
+                             _dev(wnew, torch.float32, "Wnew"), flags, wp, wb, _stream()), "emc_update")
+    return wnew
+
+
+def emc_compress(wnew, slice_w, q, mask, quat, n, flags=0, want_den=False, ws=None):
+    """Stage 5 (eq. 2.10 / 2.12).  Returns (model' [n,n,n] float32, den [n^3] or None)."""
+    n_rot, n_pix = wnew.shape
+    det = _detector(q, mask)
+    rot = _rotations(quat, None)
+    model = torch.empty((n, n, n), dtype=torch.float32, device=wnew.device)
+    den = torch.empty(n * n * n, dtype=torch.float32, device=wnew.device) if want_den else None
+    ws, wp, wb = _ws(ws, n, n_pix, n_rot, 1)
+    _check(load().emc_compress(_dev(wnew, torch.float32, "Wnew"), _opt(slice_w, torch.float32, "slice_w"), det, rot,
+                               n, model.data_ptr(), den.data_ptr() if want_den else None, flags, wp, wb, _stream()),
+           "emc_compress")
+    return model, den
+
+
+def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, flags=0, want_p=False, ws=None,
+                model_out=None, loglik=None):
+    """Algorithm 1: n_iter iterations of stages 1-5.  Returns dict(model, loglik [n_iter] float64, P or None)."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rot = _rotations(quat, weight)
+    on_host = bool(flags & EMC_PATTERNS_ON_HOST)
+    pat = _patterns(counts, det.n_pix, on_host)
+    chunk = pat.n_pat if (n_pat_chunk == 0 or n_pat_chunk > pat.n_pat) else n_pat_chunk
+    dev = model.device
+    if model_out is None:
+        model_out = torch.empty_like(model)
+    if loglik is None:
+        loglik = torch.zeros(n_iter, dtype=torch.float64, device=dev)
+    ld = ld_for(pat.n_pat)
+    p = torch.empty((rot.n_rot, ld), dtype=torch.float32, device=dev) if want_p else None
+    ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, chunk, flags)
+    _check(load().emc_iterate(m, det, rot, pat, n_iter, n_pat_chunk, _dev(model_out, torch.float32, "model_out"),
+                              p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
+           "emc_iterate")
+    return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
+
+
+def emc_check(ws):
+    """Synchronises and raises EmcError(EMC_ERR_COUNT_RANGE) if a count exceeded EMC_MAX_COUNT."""
+    _check(load().emc_check(ws.data_ptr(), _stream()), "emc_check")
+
+
+def emc_launch_count() -> int:
+    return load().emc_launch_count()
+
+
+def emc_version() -> str:
+    return load().emc_version().decode()

@@ -1,0 +1,276 @@
+// The C ABI of libemc (include/emc.h): argument validation, workspace carving and the stage order
+// of Algorithm 1.  All device work is in the launch_* functions of the other
+// translation units; nothing here touches the data.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+
+#include "emc_internal.cuh"
+
+namespace emc {
+
+static thread_local char g_err[512] = "";
+static std::atomic<uint64_t> g_launches{0};
+
+emc_status cuda_fail(cudaError_t e, const char *what) {
+    snprintf(g_err, sizeof(g_err), "%s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+    return EMC_ERR_CUDA;
+}
+void note_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+
+namespace {
+
+size_t count_size(emc_count_type t) { return t == EMC_I32 ? 4 : (t == EMC_U16 ? 2 : 1); }
+
+// One layout serves every entry point; a call uses the parts it needs.
+struct Layout {
+    WsHeader *hdr;
+    __half *planesL;          // [2][R][ld_p]  logW hi / lo
+    float *S;                 // [R]           sum_{p:mask} W
+    __half *Kc;               // [Nc][ld_p]    counts, row = pattern
+    __nv_bfloat16 *KT;        // [P][ld_n]     counts, row = pixel
+    float *L;                 // [R][ld_n]
+    __nv_bfloat16 *planesP;   // [3][R][ld_n]  P hi / mid / lo
+    float *s;                 // [R]
+    float *Wnum;              // [R][P]        update numerators -> W'
+    float2 *acc;              // [G]           (num, den)
+    float *scratch;           // normalise partials
+    void *stage;              // one chunk of raw counts (patterns on host)
+    int ld_p, ld_n;
+    size_t total;
+};
+
+Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_bytes) {
+    Layout l;
+    l.ld_p = (int)round_up((size_t)n_pix, 64);
+    l.ld_n = (int)round_up((size_t)n_chunk, 64);
+    Arena a(ws, (size_t)-1);
+    const size_t R = (size_t)n_rot;
+    l.hdr = a.take<WsHeader>(1);
+    l.planesL = a.take<__half>(2 * R * l.ld_p);
+    l.S = a.take<float>(R);
+    l.Kc = a.take<__half>((size_t)n_chunk * l.ld_p);
+    l.KT = a.take<__nv_bfloat16>((size_t)n_pix * l.ld_n);
+    l.L = a.take<float>(R * l.ld_n);
+    l.planesP = a.take<__nv_bfloat16>(3 * R * l.ld_n);
+    l.s = a.take<float>(R);
+    l.Wnum = a.take<float>(R * n_pix);
+    l.acc = a.take<float2>((size_t)n * n * n);
+    l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
+    l.stage = a.take<uint8_t>(stage_bytes);
+    l.total = a.off;
+    return l;
+}
+
+bool sizes_ok(int n, int n_pix, int n_rot, int n_pat) {
+    return n >= 2 && n <= 1024 && n_pix > 0 && n_rot > 0 && n_pat > 0 && (size_t)n_pix * 8 < (size_t)1 << 31;
+}
+
+emc_status check_ws(void *ws, size_t ws_bytes, size_t need) {
+    if (!ws || ((uintptr_t)ws & 255)) return EMC_ERR_WORKSPACE;
+    if (ws_bytes < need) return EMC_ERR_WORKSPACE;
+    return EMC_OK;
+}
+
+bool det_ok(const emc_detector *d) { return d && d->n_pix > 0 && d->q; }
+bool rot_ok(const emc_rotations *r) { return r && r->n_rot > 0 && r->quat; }
+bool pat_ok(const emc_patterns *p) {
+    return p && p->n_pat > 0 && p->counts && (p->type == EMC_I32 || p->type == EMC_U16 || p->type == EMC_U8);
+}
+
+emc_status reset_header(const Layout &l, cudaStream_t st) {
+    EMC_TRY_CUDA(cudaMemsetAsync(l.hdr, 0, sizeof(WsHeader), st));
+    return EMC_OK;
+}
+
+emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
+                           bool simt, cudaStream_t st) {
+    GemmProblem g;
+    g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
+    g.M = n_rot; g.N = n_pat; g.K = n_pix;
+    g.lda = l.ld_p; g.ldb = l.ld_p; g.plane_stride = (size_t)n_rot * l.ld_p;
+    g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
+    g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = EPI_SUB_ROW;
+    return launch_plane_gemm(g, simt, st);
+}
+
+emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, int n_planes, float *out,
+                           const float *s, int epilogue, bool simt, cudaStream_t st) {
+    GemmProblem g;
+    g.A = l.planesP; g.B = l.KT; g.n_planes = n_planes;
+    g.M = n_rot; g.N = n_pix; g.K = n_pat;
+    g.lda = l.ld_n; g.ldb = l.ld_n; g.plane_stride = (size_t)n_rot * l.ld_n;
+    g.a_fmt = FMT_BF16; g.b_fmt = FMT_BF16;
+    g.out = out; g.ld_out = n_pix; g.rowv = s; g.epilogue = epilogue;
+    return launch_plane_gemm(g, simt, st);
+}
+
+}  // namespace
+}  // namespace emc
+
+using namespace emc;
+
+extern "C" {
+
+size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags) {
+    if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return 0;
+    const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? (size_t)n_pat_chunk * n_pix * 4 : 0;
+    return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage).total;
+}
+
+emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                      float *W, int32_t *idx, void *stream) {
+    if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || (!W && !idx)) return EMC_ERR_ARG;
+    if (!sizes_ok(model->n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
+    return launch_expand(model->model, model->n, det->q, det->mask, det->n_pix, rot->quat, rot->n_rot, W, idx,
+                         nullptr, 0, nullptr, (cudaStream_t)stream);
+}
+
+emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *det,
+                      const emc_patterns *pat, int n_rot, float *L, int ld_n, unsigned flags,
+                      void *ws, size_t ws_bytes, void *stream) {
+    if (!W || !det_ok(det) || !pat_ok(pat) || n_rot <= 0 || !L || ld_n < pat->n_pat || (ld_n & 3) ||
+        ((uintptr_t)L & 15))
+        return EMC_ERR_ARG;
+    if (!sizes_ok(2, det->n_pix, n_rot, pat->n_pat)) return EMC_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, 0, det->n_pix, n_rot, pat->n_pat, 0).total));
+    const Layout l = carve(ws, 0, det->n_pix, n_rot, pat->n_pat, 0);
+    EMC_TRY(reset_header(l, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
+    EMC_TRY(launch_logw_split(W, idx, det->mask, det->n_pix, n_rot, l.planesL, l.ld_p, l.S, st));
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, 0,
+                        l.hdr, st));
+    return run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, (flags & EMC_DEBUG_SIMT) != 0, st);
+}
+
+emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
+                         float *s, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
+                         void *stream) {
+    if (!L || !rot || rot->n_rot <= 0 || n_pat <= 0 || ld_n < n_pat || !P) return EMC_ERR_ARG;
+    const size_t need = round_up(sizeof(float) * normalize_scratch_floats(rot->n_rot, ld_n), 1024);
+    EMC_TRY(check_ws(ws, ws_bytes, need));
+    return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, 0, 0, s, loglik,
+                            (flags & EMC_ACCUMULATE) != 0, (float *)ws, (cudaStream_t)stream);
+}
+
+emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detector *det,
+                      const emc_patterns *pat, int n_rot, float *Wnew, unsigned flags, void *ws,
+                      size_t ws_bytes, void *stream) {
+    const bool raw = (flags & (EMC_UPDATE_RAW | EMC_ACCUMULATE)) != 0;
+    if (!P || !det_ok(det) || !pat_ok(pat) || n_rot <= 0 || !Wnew || ld_n < pat->n_pat || (!raw && !s))
+        return EMC_ERR_ARG;
+    if (!sizes_ok(2, det->n_pix, n_rot, pat->n_pat)) return EMC_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, 0, det->n_pix, n_rot, pat->n_pat, 0).total));
+    const Layout l = carve(ws, 0, det->n_pix, n_rot, pat->n_pat, 0);
+    const int n_planes = (flags & EMC_PLANES_2) ? 2 : 3;
+    EMC_TRY(reset_header(l, st));
+    EMC_TRY(launch_p_split(P, n_rot, pat->n_pat, ld_n, l.planesP, l.ld_n, n_planes, (size_t)n_rot * l.ld_n, st));
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, l.ld_n,
+                        l.hdr, st));
+    const int epi = (flags & EMC_ACCUMULATE) ? EPI_ADD : (raw ? EPI_STORE : EPI_DIV_ROW);
+    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, n_planes, Wnew, s, epi,
+                           (flags & EMC_DEBUG_SIMT) != 0, st);
+}
+
+emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detector *det,
+                        const emc_rotations *rot, int n, float *model_out, float *den_out,
+                        unsigned flags, void *ws, size_t ws_bytes, void *stream) {
+    if (!Wnew || !det_ok(det) || !rot_ok(rot) || !model_out) return EMC_ERR_ARG;
+    if (!sizes_ok(n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
+    const size_t need = round_up(sizeof(float2) * (size_t)n * n * n, 1024);
+    EMC_TRY(check_ws(ws, ws_bytes, need));
+    return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, det->q, det->mask, det->n_pix,
+                           rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);
+}
+
+emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                       const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
+                       float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
+                       size_t ws_bytes, void *stream) {
+    if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_iter <= 0 || !model_out ||
+        model_out == model->model || !loglik || n_pat_chunk < 0)
+        return EMC_ERR_ARG;
+    const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
+    const int chunk = (n_pat_chunk == 0 || n_pat_chunk > n_pat) ? n_pat : n_pat_chunk;
+    if (!sizes_ok(n, n_pix, n_rot, chunk)) return EMC_ERR_UNSUPPORTED;
+    const int n_chunks = ceil_div(n_pat, chunk);
+    const bool on_host = (flags & EMC_PATTERNS_ON_HOST) != 0;
+    const size_t csz = count_size(pat->type);
+    const size_t stage_bytes = on_host ? (size_t)chunk * n_pix * 4 : 0;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes).total));
+    const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
+    if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
+    const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
+    const int n_planes = (flags & EMC_PLANES_2) ? 2 : 3;
+
+    EMC_TRY(reset_header(l, st));
+    const float *model_cur = model->model;
+    for (int it = 0; it < n_iter; ++it) {
+        // stage 1: Expand, with logW planes and S fused in
+        EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
+        EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
+                              l.planesL, l.ld_p, l.S, st));
+        EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
+        EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
+        for (int c = 0; c < n_chunks; ++c) {
+            const int d0 = c * chunk;
+            const int nc = n_pat - d0 < chunk ? n_pat - d0 : chunk;
+            if (n_chunks > 1 || it == 0) {          // one resident chunk is packed once for all iterations
+                const uint8_t *src = (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz;
+                if (on_host) {
+                    EMC_TRY_CUDA(cudaMemcpyAsync(l.stage, src, (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, st));
+                    src = (const uint8_t *)l.stage;
+                }
+                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, l.ld_n, l.hdr, st));
+            }
+            // stage 2: L = logW K^T - S
+            EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, simt, st));
+            // stage 3: responsibilities of this chunk; s and LL add up over chunks
+            float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
+            EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, n_planes,
+                                     (size_t)n_rot * l.ld_n, l.s, loglik + it, true, l.scratch, st));
+            // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
+            const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
+            EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, n_planes, l.Wnum, l.s, epi, simt, st));
+        }
+        if (n_chunks > 1) EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
+        // stage 5: Compress
+        EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
+                                model_out, nullptr, st));
+        model_cur = model_out;
+    }
+    return EMC_OK;
+}
+
+emc_status emc_check(void *ws, void *stream) {
+    if (!ws) return EMC_ERR_ARG;
+    WsHeader h;
+    EMC_TRY_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    EMC_TRY_CUDA(cudaMemcpy(&h, ws, sizeof(h), cudaMemcpyDeviceToHost));
+    EMC_TRY_CUDA(cudaMemset(ws, 0, sizeof(h)));
+    return h.max_count > EMC_MAX_COUNT ? EMC_ERR_COUNT_RANGE : EMC_OK;
+}
+
+uint64_t emc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char *emc_strerror(emc_status s) {
+    switch (s) {
+        case EMC_OK: return "ok";
+        case EMC_ERR_ARG: return "invalid argument";
+        case EMC_ERR_UNSUPPORTED: return "size not supported";
+        case EMC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+        case EMC_ERR_CUDA: return "CUDA error";
+        case EMC_ERR_COUNT_RANGE: return "unmasked photon count above EMC_MAX_COUNT";
+    }
+    return "unknown status";
+}
+
+const char *emc_last_cuda_error(void) { return g_err; }
+
+const char *emc_version(void) { return "libemc 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,139 @@
+// Stage 1, Expand (e-step), eq. (2.9), and the log-slice planes that feed the
+// log-likelihood contraction (north_star stage 2).
+//
+//   W[r,p] = sum over the 8 voxels around x = R_r q_p + c of (trilinear weight) * model[voxel]
+//
+// Fused into the same pass: logW = log(max(W,1e-30)) split into two fp16 planes
+// (hi, lo) with masked / outside samples zeroed, and S[r] = sum_{p:mask} W[r,p].
+#include "emc_geometry.cuh"
+#include "emc_internal.cuh"
+
+namespace emc {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kPixPerThread = 4;
+constexpr int kPixPerBlock = kThreads * kPixPerThread;
+
+__device__ __forceinline__ float block_sum(float v, float *red) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    float t = 0.f;
+    if (warp == 0) {
+        t = lane < (kThreads / 32) ? red[lane] : 0.f;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    }
+    return t;   // valid in thread 0
+}
+
+// logW -> two fp16 planes: hi = fp16(lw), lo = fp16(lw - hi); 22 significand bits in all.
+__device__ __forceinline__ void split_logw(float w, bool live, __half &hi, __half &lo) {
+    float lw = live ? logf(fmaxf(w, 1e-30f)) : 0.f;
+    hi = __float2half_rn(lw);
+    lo = __float2half_rn(lw - __half2float(hi));
+}
+
+// grid = (R, ceil(P / kPixPerBlock)); one rotation per block row.
+__global__ void __launch_bounds__(kThreads)
+expand_kernel(const float *__restrict__ model, int n, const float *__restrict__ q,
+              const uint8_t *__restrict__ mask, int n_pix, const float *__restrict__ quat,
+              float *__restrict__ W, int32_t *__restrict__ idx, __half *__restrict__ planes, int ld_p,
+              size_t plane_stride, float *__restrict__ S) {
+    __shared__ float rm[9];
+    __shared__ float red[kThreads / 32];
+    const int r = blockIdx.x;
+    if (threadIdx.x == 0) {
+        RotMat m = rotation_matrix(quat + 4 * (size_t)r);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
+    }
+    __syncthreads();
+    const int nn = n * n;
+    float part = 0.f;
+#pragma unroll
+    for (int j = 0; j < kPixPerThread; ++j) {
+        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
+        if (p >= n_pix) continue;
+        const Sample s = locate(rm, q[3 * p], q[3 * p + 1], q[3 * p + 2], n);
+        float w = 0.f;
+        if (s.base >= 0) {
+            const float *b = model + s.base;
+            const float z0 = 1.f - s.tz, y0 = 1.f - s.ty, x0 = 1.f - s.tx;
+            const float c00 = b[0] * z0 + b[1] * s.tz;
+            const float c01 = b[n] * z0 + b[n + 1] * s.tz;
+            const float c10 = b[nn] * z0 + b[nn + 1] * s.tz;
+            const float c11 = b[nn + n] * z0 + b[nn + n + 1] * s.tz;
+            w = (c00 * y0 + c01 * s.ty) * x0 + (c10 * y0 + c11 * s.ty) * s.tx;
+        }
+        const size_t o = (size_t)r * n_pix + p;
+        if (W) W[o] = w;
+        if (idx) idx[o] = s.base;
+        const bool use = mask ? (mask[p] != 0) : true;
+        if (planes) {
+            __half hi, lo;
+            split_logw(w, use && s.base >= 0, hi, lo);
+            const size_t po = (size_t)r * ld_p + p;
+            planes[po] = hi;
+            planes[plane_stride + po] = lo;
+        }
+        if (use) part += w;
+    }
+    if (S) {
+        const float t = block_sum(part, red);
+        if (threadIdx.x == 0) atomicAdd(S + r, t);
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
+                  const uint8_t *__restrict__ mask, int n_pix, __half *__restrict__ planes, int ld_p,
+                  size_t plane_stride, float *__restrict__ S) {
+    __shared__ float red[kThreads / 32];
+    const int r = blockIdx.x;
+    float part = 0.f;
+#pragma unroll
+    for (int j = 0; j < kPixPerThread; ++j) {
+        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
+        if (p >= n_pix) continue;
+        const size_t o = (size_t)r * n_pix + p;
+        const float w = W[o];
+        const bool inside = idx ? (idx[o] >= 0) : true;
+        const bool use = mask ? (mask[p] != 0) : true;
+        __half hi, lo;
+        split_logw(w, use && inside, hi, lo);
+        const size_t po = (size_t)r * ld_p + p;
+        planes[po] = hi;
+        planes[plane_stride + po] = lo;
+        if (use) part += w;
+    }
+    const float t = block_sum(part, red);
+    if (threadIdx.x == 0) atomicAdd(S + r, t);
+}
+
+}  // namespace
+
+emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
+                         const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
+                         int ld_p, float *S, cudaStream_t st) {
+    dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+    expand_kernel<<<grid, kThreads, 0, st>>>(model, n, q, mask, n_pix, quat, W, idx, planes, ld_p,
+                                             (size_t)n_rot * ld_p, S);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
+                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st) {
+    dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+    logw_split_kernel<<<grid, kThreads, 0, st>>>(W, idx, mask, n_pix, planes, ld_p,
+                                                 (size_t)n_rot * ld_p, S);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+}  // namespace emc

@@ -1,0 +1,432 @@
+// The two dense contractions of the EMC iteration on the 5th-generation tensor cores:
+//
+//   log-likelihood (north_star stage 2; E-step numerator):
+//        L[r,d]  = sum_p logW[r,p] K[d,p] - S[r]         M = R, N = patterns, K-dim = pixels
+//   update (eq. 2.5 / 2.11):
+//        W'[r,p] = sum_d P[r,d] K[d,p] / s[r]            M = R, N = pixels,   K-dim = patterns
+//
+// Both are "plane GEMMs": the real-valued operand A (logW or P) is a sum of n_planes 16-bit
+// planes (hi + lo [+ lo2]); the count operand B is exact in ONE 16-bit plane, so every product is
+// exact in fp32 and the only rounding is the fp32 accumulation in TMEM:
+//
+//        acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
+//
+// Kernel: persistent, one CTA per SM, warp-specialised.
+//   warp 0 lane 0 : TMA producer  (cp.async.bulk.tensor -> 128B-swizzled smem ring, mbarrier tx)
+//   warp 1 lane 0 : MMA issuer    (tcgen05.mma.cta_group::1.kind::f16, 128 x BN x 16, fp32 in TMEM)
+//   warps 2..5    : epilogue      (tcgen05.ld 32x32b -> registers -> fused row op -> global)
+// TMEM holds two accumulator stages of BN columns, so the epilogue of tile i overlaps the main
+// loop of tile i+1.
+#include "emc_internal.cuh"
+
+namespace emc {
+
+namespace {
+
+constexpr int BLOCK_M = 128;
+constexpr int BLOCK_K = 64;                    // 64 x 2 B = one 128-byte swizzle row
+constexpr int UMMA_K = 16;
+constexpr int A_PLANE_BYTES = BLOCK_M * BLOCK_K * 2;
+constexpr int kGemmThreads = 192;
+constexpr int kNumEpiWarps = 4;
+constexpr int kGroupM = 8;                     // tile rasterisation: 8 m-blocks share each n sweep
+
+template <int NP, int BN, int STAGES>
+struct Cfg {
+    static constexpr int B_BYTES = BN * BLOCK_K * 2;
+    static constexpr int STAGE_BYTES = NP * A_PLANE_BYTES + B_BYTES;
+    static constexpr int BAR_BYTES = 256;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;   // + alignment slack
+    static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory per CTA");
+    static_assert(2 * BN <= 512, "two accumulator stages must fit the 512 TMEM columns");
+    static_assert(BN % 16 == 0 && BN >= 16 && BN <= 256, "UMMA N for M = 128");
+    static_assert(BN % 32 == 0, "epilogue reads 32 columns at a time");
+};
+
+struct GemmArgs {
+    int M, N, K;
+    int num_m_tiles, num_n_tiles, num_k_blocks;
+    float *out;
+    int ld_out;
+    const float *rowv;
+    int epilogue;
+    int vec_ok;          // out rows are 16-byte aligned
+    uint32_t idesc;
+};
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrives on the mbarrier once every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t addr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(addr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// UMMA shared-memory descriptor of a K-major tile with 128-byte rows under SWIZZLE_128B:
+// start address >> 4 in bits [0,14), LBO (unused for swizzled K-major) = 1 in [16,30),
+// SBO = 1024 B (8 rows x 128 B) >> 4 in [32,46), version 1 in [46,48), layout SWIZZLE_128B = 2 in [61,64).
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    return (uint64_t)((smem_addr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) |
+           (1ull << 46) | (2ull << 61);
+}
+
+__device__ __forceinline__ void tile_coords(int tile, const GemmArgs &a, int &m_blk, int &n_blk) {
+    const int per_group = kGroupM * a.num_n_tiles;
+    const int group = tile / per_group;
+    const int first_m = group * kGroupM;
+    const int gm = min(a.num_m_tiles - first_m, kGroupM);
+    const int t = tile - group * per_group;
+    m_blk = first_m + t % gm;
+    n_blk = t / gm;
+}
+
+template <int NP, int BN, int STAGES>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                  const GemmArgs args) {
+    using C = Cfg<NP, BN, STAGES>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // SWIZZLE_128B atoms need 1024 B
+    const uint32_t bar_base = smem_base + STAGES * C::STAGE_BYTES;
+    // barrier map (8 B each): full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2], then the TMEM address
+    const uint32_t full_bar = bar_base, empty_bar = bar_base + 8 * STAGES;
+    const uint32_t tfull_bar = bar_base + 16 * STAGES, tempty_bar = tfull_bar + 16;
+    const uint32_t tmem_slot = tempty_bar + 16;
+    uint32_t *tmem_slot_ptr =
+        (uint32_t *)(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int num_tiles = args.num_m_tiles * args.num_n_tiles;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar + 8 * s, 1);
+            mbar_init(empty_bar + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(tfull_bar + 8 * a, 1);
+            mbar_init(tempty_bar + 8 * a, kNumEpiWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                int m_blk, n_blk;
+                tile_coords(tile, args, m_blk, n_blk);
+                for (int kb = 0; kb < args.num_k_blocks; ++kb) {
+                    mbar_wait(empty_bar + 8 * stage, phase ^ 1u);
+                    const uint32_t fb = full_bar + 8 * stage;
+                    mbar_expect_tx(fb, C::STAGE_BYTES);
+                    const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
+#pragma unroll
+                    for (int pl = 0; pl < NP; ++pl)
+                        tma_load_3d(sa + pl * A_PLANE_BYTES, &tmA, fb, kb * BLOCK_K, m_blk * BLOCK_M, pl);
+                    tma_load_2d(sa + NP * A_PLANE_BYTES, &tmB, fb, kb * BLOCK_K, n_blk * BN);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer =================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc = 0;
+            uint32_t acc_phase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                mbar_wait(tempty_bar + 8 * acc, acc_phase ^ 1u);     // epilogue has drained this stage
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+                for (int kb = 0; kb < args.num_k_blocks; ++kb) {
+                    mbar_wait(full_bar + 8 * stage, phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
+                    const uint64_t bdesc0 = umma_desc_sw128(sa + NP * A_PLANE_BYTES);
+#pragma unroll
+                    for (int pl = 0; pl < NP; ++pl) {
+                        const uint64_t adesc0 = umma_desc_sw128(sa + pl * A_PLANE_BYTES);
+#pragma unroll
+                        for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+                            // advancing 16 elements along K inside the swizzle row = +32 B = +2 in the
+                            // (>>4) start-address field
+                            umma_f16(d_tmem, adesc0 + (uint64_t)(2 * k), bdesc0 + (uint64_t)(2 * k), args.idesc,
+                                     (kb | pl | k) != 0 ? 1u : 0u);
+                        }
+                    }
+                    umma_commit(empty_bar + 8 * stage);              // smem slot free once these MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+                umma_commit(tfull_bar + 8 * acc);                    // accumulator complete
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+        }
+    } else {
+        // ================= epilogue warps 2..5 =================
+        const int quarter = warp & 3;                    // TMEM lanes 32*quarter .. +31 belong to this warp
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            int m_blk, n_blk;
+            tile_coords(tile, args, m_blk, n_blk);
+            mbar_wait(tfull_bar + 8 * acc, acc_phase);
+            tc_fence_after();
+            const int m = m_blk * BLOCK_M + quarter * 32 + lane;
+            const bool row_ok = m < args.M;
+            float rv = 0.f;
+            if (row_ok && args.rowv) rv = args.rowv[m];
+            float inv_ok = rv > 0.f ? 1.f : 0.f;
+            float *orow = args.out + (size_t)(row_ok ? m : 0) * args.ld_out;
+            const uint32_t t_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN);
+#pragma unroll 1
+            for (int c = 0; c < BN; c += 32) {
+                uint32_t v[32];
+                tmem_ld32(t_addr + (uint32_t)c, v);
+                const int n0 = n_blk * BN + c;
+                if (!row_ok || n0 >= args.N) continue;
+                float f[32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(v[j]);
+                if (args.epilogue == EPI_SUB_ROW) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) f[j] -= rv;
+                } else if (args.epilogue == EPI_DIV_ROW) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) f[j] = inv_ok != 0.f ? f[j] / rv : 0.f;
+                }
+                float *o = orow + n0;
+                if (args.vec_ok && n0 + 32 <= args.N) {
+                    float4 *o4 = reinterpret_cast<float4 *>(o);
+                    if (args.epilogue == EPI_ADD) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            float4 t = o4[j];
+                            t.x += f[4 * j]; t.y += f[4 * j + 1]; t.z += f[4 * j + 2]; t.w += f[4 * j + 3];
+                            o4[j] = t;
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) o4[j] = make_float4(f[4 * j], f[4 * j + 1], f[4 * j + 2], f[4 * j + 3]);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        if (n0 + j < args.N) {
+                            if (args.epilogue == EPI_ADD) o[j] += f[j];
+                            else o[j] = f[j];
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar + 8 * acc);
+            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// ------------------------------------------------------------------ plain CUDA-core version (EMC_DEBUG_SIMT)
+__device__ __forceinline__ float load16(const void *p, size_t i, int fmt) {
+    const uint16_t u = ((const uint16_t *)p)[i];
+    return fmt == FMT_F16 ? __half2float(__ushort_as_half(u)) : __uint_as_float((uint32_t)u << 16);
+}
+
+__global__ void simt_plane_gemm_kernel(GemmProblem g) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y;
+    if (n >= g.N || m >= g.M) return;
+    float acc = 0.f;
+    for (int pl = 0; pl < g.n_planes; ++pl)
+        for (int k = 0; k < g.K; ++k)
+            acc += load16(g.A, pl * g.plane_stride + (size_t)m * g.lda + k, g.a_fmt) *
+                   load16(g.B, (size_t)n * g.ldb + k, g.b_fmt);
+    float *o = g.out + (size_t)m * g.ld_out + n;
+    const float rv = g.rowv ? g.rowv[m] : 0.f;
+    switch (g.epilogue) {
+        case EPI_SUB_ROW: *o = acc - rv; break;
+        case EPI_STORE: *o = acc; break;
+        case EPI_ADD: *o += acc; break;
+        default: *o = rv > 0.f ? acc / rv : 0.f; break;
+    }
+}
+
+// ------------------------------------------------------------------ host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+emc_status get_encode_fn(EncodeTiledFn *out) {
+    static EncodeTiledFn cached = nullptr;
+    if (!cached) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        EMC_TRY_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !fn) return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled entry point");
+        cached = (EncodeTiledFn)fn;
+    }
+    *out = cached;
+    return EMC_OK;
+}
+
+emc_status make_map(CUtensorMap *map, const void *base, PlaneFormat fmt, int rank, const cuuint64_t *dims,
+                    const cuuint64_t *strides_bytes, const cuuint32_t *box) {
+    EncodeTiledFn enc;
+    EMC_TRY(get_encode_fn(&enc));
+    const cuuint32_t ones[3] = {1, 1, 1};
+    CUresult r = enc(map, fmt == FMT_F16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                     (cuuint32_t)rank, const_cast<void *>(base), dims, strides_bytes, box, ones,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cuda_fail(cudaErrorInvalidValue, "cuTensorMapEncodeTiled");
+    return EMC_OK;
+}
+
+int num_sms() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (sms <= 0) sms = 148;
+    }
+    return sms;
+}
+
+template <int NP, int BN, int STAGES>
+emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
+    using C = Cfg<NP, BN, STAGES>;
+    CUtensorMap tmA, tmB;
+    {
+        const cuuint64_t dims[3] = {(cuuint64_t)g.K, (cuuint64_t)g.M, (cuuint64_t)NP};
+        const cuuint64_t strides[2] = {(cuuint64_t)g.lda * 2, (cuuint64_t)g.plane_stride * 2};
+        const cuuint32_t box[3] = {BLOCK_K, BLOCK_M, 1};
+        EMC_TRY(make_map(&tmA, g.A, g.a_fmt, 3, dims, strides, box));
+    }
+    {
+        const cuuint64_t dims[2] = {(cuuint64_t)g.K, (cuuint64_t)g.N};
+        const cuuint64_t strides[1] = {(cuuint64_t)g.ldb * 2};
+        const cuuint32_t box[2] = {BLOCK_K, BN};
+        EMC_TRY(make_map(&tmB, g.B, g.b_fmt, 2, dims, strides, box));
+    }
+    GemmArgs a;
+    a.M = g.M; a.N = g.N; a.K = g.K;
+    a.num_m_tiles = ceil_div(g.M, BLOCK_M);
+    a.num_n_tiles = ceil_div(g.N, BN);
+    a.num_k_blocks = ceil_div(g.K, BLOCK_K);
+    a.out = g.out; a.ld_out = g.ld_out; a.rowv = g.rowv; a.epilogue = g.epilogue;
+    a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
+    // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
+    // N >> 3 in [17,23); M >> 4 in [24,29)
+    a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
+              ((uint32_t)(BLOCK_M >> 4) << 24);
+    auto kern = plane_gemm_kernel<NP, BN, STAGES>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        EMC_TRY_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        attr_set = true;
+    }
+    const int tiles = a.num_m_tiles * a.num_n_tiles;
+    const int grid = tiles < num_sms() ? tiles : num_sms();
+    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, a);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+}  // namespace
+
+emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st) {
+    if (g.M <= 0 || g.N <= 0 || g.K <= 0) return EMC_ERR_ARG;
+    if (g.lda % 8 || g.ldb % 8 || g.plane_stride % 8 || ((uintptr_t)g.A & 15) || ((uintptr_t)g.B & 15)) return EMC_ERR_ARG;
+    if (simt_debug) {
+        dim3 grid(ceil_div(g.N, 128), g.M);
+        simt_plane_gemm_kernel<<<grid, 128, 0, st>>>(g);
+        EMC_LAUNCHED();
+        return EMC_OK;
+    }
+    if (g.n_planes == 2) return launch_tc<2, 256, 3>(g, st);
+    if (g.n_planes == 3) return launch_tc<3, 192, 3>(g, st);
+    return EMC_ERR_UNSUPPORTED;
+}
+
+}  // namespace emc

@@ -1,0 +1,119 @@
+// Internal declarations shared by the translation units of libemc (sm_100a only).
+// Nothing here is part of the C ABI (include/emc.h) and nothing is shared with oracle/.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/emc.h"
+
+namespace emc {
+
+// ---------------------------------------------------------------- host-side plumbing
+emc_status cuda_fail(cudaError_t e, const char *what);
+void note_launch(int n = 1);
+
+#define EMC_TRY_CUDA(expr)                                        \
+    do {                                                          \
+        cudaError_t e__ = (expr);                                 \
+        if (e__ != cudaSuccess) return ::emc::cuda_fail(e__, #expr); \
+    } while (0)
+
+#define EMC_TRY(expr)                         \
+    do {                                      \
+        emc_status s__ = (expr);              \
+        if (s__ != EMC_OK) return s__;        \
+    } while (0)
+
+// after a kernel launch
+#define EMC_LAUNCHED()                        \
+    do {                                      \
+        ::emc::note_launch();                 \
+        EMC_TRY_CUDA(cudaGetLastError());     \
+    } while (0)
+
+static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// First 256 bytes of every workspace: what only the device can see (emc_check()).
+struct WsHeader {
+    int max_count;   // largest unmasked photon count seen by the pack kernel
+    int pad[63];
+};
+static_assert(sizeof(WsHeader) == 256, "header is one 256-byte line");
+
+// Bump allocator over the caller's workspace.
+struct Arena {
+    uint8_t *base;
+    size_t size, off;
+    bool ok;
+    Arena(void *p, size_t bytes) : base((uint8_t *)p), size(bytes), off(0), ok(true) {}
+    template <class T>
+    T *take(size_t count) {
+        size_t bytes = round_up(count * sizeof(T), 1024);
+        if (off + bytes > size) { ok = false; off += bytes; return nullptr; }
+        T *p = (T *)(base + off);
+        off += bytes;
+        return p;
+    }
+};
+
+enum PlaneFormat { FMT_F16 = 0, FMT_BF16 = 1 };   // = the UMMA instruction descriptor encoding
+
+// ---------------------------------------------------------------- stage launchers (device work)
+// Expand (emc_expand.cu).  Any of W, idx, planes may be null.  planes = [2][R][ld_p] fp16 (hi, lo)
+// of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).
+emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
+                         const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
+                         int ld_p, float *S, cudaStream_t st);
+// logW planes + S from a given W (stage API of emc_loglik).
+emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
+                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
+
+// Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] bf16
+// (row = pixel), masked pixels zeroed, largest unmasked count recorded in hdr->max_count.
+emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
+                       const uint8_t *mask, __half *Kc, int ld_p, __nv_bfloat16 *KT, int ld_n,
+                       WsHeader *hdr, cudaStream_t st);
+
+// Plane GEMM on tcgen05 (emc_gemm.cu):  acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
+struct GemmProblem {
+    const void *A;      // [n_planes][M][lda] 16-bit elements, K-major
+    const void *B;      // [N][ldb] 16-bit elements, K-major
+    int n_planes;       // 2 or 3
+    int M, N, K;
+    int lda, ldb;       // row pitches in elements (multiples of 8)
+    size_t plane_stride;  // elements between planes of A
+    PlaneFormat a_fmt, b_fmt;
+    float *out;         // [M][ld_out]
+    int ld_out;
+    const float *rowv;  // [M] row vector of the epilogue (S for loglik, s for update) or null
+    int epilogue;       // EPI_*
+};
+enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-likelihood)
+       EPI_STORE = 1,       // out = acc                                (raw update numerator)
+       EPI_ADD = 2,         // out += acc                               (numerator over chunks)
+       EPI_DIV_ROW = 3 };   // out = rowv[m] > 0 ? acc / rowv[m] : 0    (eq. 2.5)
+emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st);
+
+// Normalise (emc_normalize.cu).  scratch = 2 * row_splits * ld_n floats.
+size_t normalize_scratch_floats(int n_rot, int ld_n);
+emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
+                            float *P, __nv_bfloat16 *planes, int n_planes, size_t plane_stride,
+                            float *s, double *loglik, bool accumulate, float *scratch,
+                            cudaStream_t st);
+// bf16 planes of a given P (stage API of emc_update).
+emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __nv_bfloat16 *planes,
+                          int ld_pl, int n_planes, size_t plane_stride, cudaStream_t st);
+// rows of Wnew divided by s[r] (after the last pattern chunk).
+emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
+
+// Compress (emc_compress.cu).  acc = [G] float2 (num, den), zeroed inside.
+emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const float *q,
+                           const uint8_t *mask, int n_pix, const float *quat, int n_rot, int n,
+                           float2 *acc, float *model_out, float *den_out, cudaStream_t st);
+
+}  // namespace emc

@@ -1,0 +1,72 @@
+"""The C-ABI library loads on a box without a GPU and exports every symbol include/emc.h declares;
+argument validation is synchronous and needs no device.  No compute calls here."""
+import ctypes
+import pathlib
+import re
+
+import pytest
+
+import paper_1409_4256_b200 as emc
+from paper_1409_4256_b200 import binding
+
+ROOT = pathlib.Path(__file__).resolve().parents[1]
+
+
+def test_header_symbols_all_exported():
+    header = (ROOT / "include" / "emc.h").read_text()
+    declared = set(re.findall(r"EMC_API[^;(]*?\b(emc_\w+)\s*\(", header))
+    assert declared == set(binding.SYMBOLS)
+    lib = emc.load()
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_header_constants_match_binding():
+    header = (ROOT / "include" / "emc.h").read_text()
+    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_PLANES_2", "EMC_DEBUG_SIMT",
+                 "EMC_PATTERNS_ON_HOST", "EMC_MAX_COUNT"):
+        m = re.search(rf"#define {name}\s+(0x[0-9a-fA-F]+|\d+)u?", header)
+        assert m, name
+        assert int(m.group(1), 0) == getattr(binding, name)
+    for name in ("EMC_ERR_ARG", "EMC_ERR_UNSUPPORTED", "EMC_ERR_WORKSPACE", "EMC_ERR_CUDA", "EMC_ERR_COUNT_RANGE"):
+        m = re.search(rf"{name} = (-\d+)", header)
+        assert int(m.group(1)) == getattr(binding, name)
+
+
+def test_version_and_strerror():
+    lib = emc.load()
+    assert b"sm_100a" in lib.emc_version()
+    assert lib.emc_strerror(0) == b"ok"
+    assert b"workspace" in lib.emc_strerror(emc.EMC_ERR_WORKSPACE)
+
+
+def test_workspace_bytes_monotone_and_rejects_bad_sizes():
+    a = emc.emc_workspace_bytes(32, 1024, 480, 1000)
+    b = emc.emc_workspace_bytes(32, 1024, 960, 1000)
+    c = emc.emc_workspace_bytes(32, 1024, 480, 1000, emc.EMC_PATTERNS_ON_HOST)
+    assert 0 < a < b and c > a
+    assert emc.emc_workspace_bytes(1, 1024, 480, 1000) == 0
+    assert emc.emc_workspace_bytes(32, 0, 480, 1000) == 0
+    assert emc.emc_workspace_bytes(2048, 16, 4, 4) == 0
+
+
+def test_null_arguments_are_rejected_synchronously():
+    lib = emc.load()
+    assert lib.emc_expand(None, None, None, None, None, None) == emc.EMC_ERR_ARG
+    assert lib.emc_check(None, None) == emc.EMC_ERR_ARG
+    det = binding._Detector(16, 8, None)
+    pat = binding._Patterns(4, 8, emc.binding.EMC_U16)
+    # misaligned / missing workspace
+    assert lib.emc_loglik(8, None, det, pat, 4, 16, 64, 0, None, 0, None) == emc.EMC_ERR_WORKSPACE
+    assert lib.emc_loglik(8, None, det, pat, 4, 16, 3, 0, 256, 1 << 30, None) == emc.EMC_ERR_ARG   # ld_n < N
+    m = binding._Model(16, 8)
+    rot = binding._Rotations(4, 8, None)
+    # model_out aliasing the model is an argument error
+    assert lib.emc_iterate(m, det, rot, pat, 1, 0, 8, None, 64, 8, 0, 256, 1 << 30, None) == emc.EMC_ERR_ARG
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+
+    with pytest.raises(TypeError):
+        emc.emc_expand(torch.zeros(4, 4, 4), torch.zeros(3, 3), torch.zeros(2, 4))

@@ -1,0 +1,209 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the same
+seeded inputs (`-m gpu`).  Tolerances are the ones north_star states, read as DESIGN.md §4 T1-T4:
+
+  idx     bit-exact
+  L       |dL| <= 1e-5 * A[r,d],  A = sum_p mask (K |logW| + W)
+  P       |dP| <= 1e-6 stage-wise (both sides normalise the same float32 L)
+  model'  |dm| <= 1e-5 * |m| on voxels with den >= 1e-6 max den, stage-wise (same W' in)
+  W, W'   relative 1e-5 (not stated by north_star; same class as the model)
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+class Case:
+    """A workload on both sides: numpy for the oracle, CUDA tensors for libemc."""
+
+    def __init__(self, inp, stage=0):
+        self.inp, self.cfg = inp, inp.cfg
+        self.quat, self.weight = inp.quat[stage], inp.weight[stage]
+        self.d_model = dev(inp.model_init)
+        self.d_q = dev(inp.q)
+        self.d_mask = dev(inp.mask)
+        self.d_quat = dev(self.quat)
+        self.d_weight = dev(self.weight)
+        self.d_counts = dev(inp.counts)
+
+
+@pytest.fixture(scope="module", params=["T1", "T2", "C1"])
+def case(request, inputs_cache):
+    inp = inputs_cache(request.param)
+    return Case(inp, stage=len(inp.quat) - 1)
+
+
+@pytest.fixture(scope="module")
+def ref(case):
+    """The oracle's iteration on this case, stage by stage (float32 at the boundaries)."""
+    inp = case.inp
+    return o.iterate(inp.model_init, inp.q, inp.mask, case.quat, case.weight, inp.counts)
+
+
+def test_expand_index_map_bit_exact_and_slices(case, ref):
+    w, idx = emc.emc_expand(case.d_model, case.d_q, case.d_quat)
+    assert np.array_equal(host(idx), ref["idx"])                     # T4: bit-exact
+    w = host(w)
+    scale = np.abs(ref["W"]).max()
+    assert np.abs(w - ref["W"]).max() <= 1e-5 * scale
+    assert np.all(np.abs(w - ref["W"]) <= 1e-5 * np.abs(ref["W"]) + 1e-9 * scale)
+    assert np.all(w[ref["idx"] < 0] == 0)
+
+
+@pytest.mark.parametrize("flags", [0, emc.EMC_DEBUG_SIMT], ids=["tcgen05", "simt"])
+def test_loglik_within_1e5_of_A(case, ref, flags):
+    inp = case.inp
+    big_l, big_a = o.loglik(ref["W"], ref["idx"], inp.counts, inp.mask)
+    got = host(emc.emc_loglik(dev(ref["W"]), dev(ref["idx"]), case.d_q, case.d_mask, case.d_counts, flags=flags))
+    err = np.abs(got - big_l) / big_a
+    assert err.max() <= 1e-5, f"max |dL|/A = {err.max():.3e}"
+
+
+def test_normalize_stagewise_1e6(case, ref):
+    l32 = ref["L"]
+    p_ref, s_ref, ll_ref = o.normalize(l32, case.weight)
+    big_l = torch.zeros((l32.shape[0], emc.ld_for(l32.shape[1])), dtype=torch.float32, device="cuda")
+    big_l[:, : l32.shape[1]] = dev(l32)
+    p, s, ll = emc.emc_normalize(big_l[:, : l32.shape[1]], case.d_quat, case.d_weight)
+    p = host(p)
+    assert np.abs(p - p_ref).max() <= 1e-6                           # T2 stage-wise
+    assert np.abs(p.sum(axis=0) - 1).max() <= 1e-5
+    assert np.abs(host(s) - s_ref).max() <= 1e-5 * max(1.0, s_ref.max())
+    assert abs(float(host(ll)[0]) - ll_ref) <= 1e-6 * abs(ll_ref)
+    # uniform prior passed as NULL gives the same numbers
+    p2, _, _ = emc.emc_normalize(big_l[:, : l32.shape[1]], case.d_quat, None)
+    if np.allclose(case.weight, case.weight[0]):
+        assert np.abs(host(p2) - p_ref).max() <= 1e-6
+
+
+@pytest.mark.parametrize("flags", [0, emc.EMC_DEBUG_SIMT, emc.EMC_PLANES_2], ids=["tcgen05", "simt", "planes2"])
+def test_update_stagewise(case, ref, flags):
+    inp = case.inp
+    p32 = ref["P"]
+    wn_ref, s_ref = o.update(p32, inp.counts, inp.mask)
+    n_pat = p32.shape[1]
+    p = torch.zeros((p32.shape[0], emc.ld_for(n_pat)), dtype=torch.float32, device="cuda")
+    p[:, :n_pat] = dev(p32)
+    s = dev(s_ref.astype(np.float32))
+    wn = host(emc.emc_update(p[:, :n_pat], s, case.d_q, case.d_mask, case.d_counts, flags=flags))
+    tol = 1e-5 if flags != emc.EMC_PLANES_2 else 1e-4
+    # rows with a vanishing s[r] divide two tiny numbers: compare the numerators there
+    scale = np.abs(wn_ref).max()
+    assert np.all(np.abs(wn - wn_ref) <= tol * np.abs(wn_ref) + 1e-7 * scale), \
+        f"max rel {np.max(np.abs(wn - wn_ref) / (np.abs(wn_ref) + 1e-7 * scale)):.3e}"
+    assert np.all(wn[:, inp.mask == 0] == 0)
+
+
+@pytest.mark.parametrize("weighted", [False, True], ids=["eq2.10", "eq2.12"])
+def test_compress_stagewise(case, ref, weighted):
+    inp = case.inp
+    n = case.cfg.n
+    s32 = ref["s"].astype(np.float32)
+    om = s32 if weighted else (s32 > 0).astype(np.float32)
+    m_ref, _, den_ref = o.compress(ref["Wn"], inp.q, case.quat, inp.mask, n, slice_w=om)
+    flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
+    m, den = emc.emc_compress(dev(ref["Wn"]), dev(s32), case.d_q, case.d_mask, case.d_quat, n, flags=flags,
+                              want_den=True)
+    m, den = host(m).reshape(-1), host(den)
+    m_ref = m_ref.reshape(-1)
+    cov = den_ref >= 1e-6 * den_ref.max()
+    assert np.all(np.abs(den[cov] - den_ref[cov]) <= 1e-5 * den_ref[cov])
+    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12), \
+        f"max rel {np.max(np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-12)):.3e}"   # T3
+    assert np.all(m[den_ref == 0] == 0)
+
+
+@pytest.mark.parametrize("weighted", [False, True], ids=["eq2.10", "eq2.12"])
+def test_iterate_end_to_end(case, ref, weighted):
+    """Whole iteration through emc_iterate.  End to end the float32 rounding of L moves P by
+    2 P |dL| (DESIGN.md §4 T2), so P gets the derived bound and the model a loose one."""
+    inp = case.inp
+    r = o.iterate(inp.model_init, inp.q, inp.mask, case.quat, case.weight, inp.counts, weighted=weighted)
+    flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
+    out = emc.emc_iterate(case.d_model, case.d_q, case.d_mask, case.d_quat, case.d_weight, case.d_counts,
+                          flags=flags, want_p=True)
+    emc.emc_check(out["ws"])
+    _, big_a = o.loglik(r["W"], r["idx"], inp.counts, inp.mask)
+    bound = 1e-6 + 2.0 * r["P"] * (2e-5 * big_a.max(axis=0))[None, :]
+    p = host(out["P"])
+    assert np.all(np.abs(p - r["P"]) <= bound), f"max dP {np.abs(p - r['P']).max():.3e}"
+    ll = float(host(out["loglik"])[0])
+    assert abs(ll - r["LL"]) <= 1e-5 * abs(r["LL"])
+    m = host(out["model"]).reshape(-1)
+    cov = r["den"] >= 1e-3 * r["den"].max()
+    m_ref = r["model"].reshape(-1)
+    rel = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-6 * np.abs(m_ref).max())
+    assert rel.max() <= (2e-3 if weighted else 2e-2), f"max rel model error {rel.max():.3e}"
+    assert np.median(rel) <= 1e-4
+
+
+def test_iterate_chunked_matches_single_chunk(inputs_cache):
+    inp = inputs_cache("T2")
+    c = Case(inp, stage=1)
+    a = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts)
+    b = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_pat_chunk=200)
+    ma, mb = host(a["model"]), host(b["model"])
+    assert np.abs(ma - mb).max() <= 1e-4 * np.abs(ma).max()
+    assert abs(float(host(a["loglik"])[0]) - float(host(b["loglik"])[0])) <= 1e-6 * abs(float(host(a["loglik"])[0]))
+    # patterns streamed from pinned host memory
+    pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
+    h = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, n_pat_chunk=200,
+                        flags=emc.EMC_PATTERNS_ON_HOST)
+    assert np.abs(host(h["model"]) - mb).max() <= 1e-5 * np.abs(mb).max()
+
+
+def test_iterate_multi_iteration_matches_repeated_calls(inputs_cache):
+    inp = inputs_cache("T1")
+    c = Case(inp)
+    a = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=3)
+    m = c.d_model
+    lls = []
+    for _ in range(3):
+        out = emc.emc_iterate(m, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts)
+        m = out["model"]
+        lls.append(float(host(out["loglik"])[0]))
+    assert np.abs(host(a["model"]) - host(m)).max() <= 1e-3 * np.abs(host(m)).max()
+    assert np.allclose(host(a["loglik"]), lls, rtol=1e-6)
+
+
+def test_count_range_is_reported(inputs_cache):
+    inp = inputs_cache("T0")
+    c = Case(inp)
+    k = inp.counts.copy()
+    k[3, 5] = 5000
+    out = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, dev(k))
+    with pytest.raises(emc.EmcError) as e:
+        emc.emc_check(out["ws"])
+    assert e.value.status == emc.EMC_ERR_COUNT_RANGE
+    # a huge count under the mask is ignored
+    k = inp.counts.copy()
+    mask = inp.mask.copy()
+    mask[5] = 0
+    k[:, 5] = 2 ** 31 - 1
+    out = emc.emc_iterate(c.d_model, c.d_q, dev(mask), c.d_quat, c.d_weight, dev(k))
+    emc.emc_check(out["ws"])
+
+
+def test_degenerate_sizes(inputs_cache):
+    """One rotation, one pattern, sizes far below one tile."""
+    inp = inputs_cache("T0")
+    c = Case(inp)
+    out = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat[:1].contiguous(), None, c.d_counts[:1].contiguous(),
+                          want_p=True)
+    assert np.allclose(host(out["P"]), 1.0)
+    r = o.iterate(inp.model_init, inp.q, inp.mask, c.quat[:1], np.ones(1, np.float32), inp.counts[:1])
+    cov = r["den"] > 0
+    assert np.allclose(host(out["model"]).reshape(-1)[cov], r["model"].reshape(-1)[cov], rtol=1e-4, atol=1e-7)
