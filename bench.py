@@ -1,0 +1,414 @@
+#!/usr/bin/env python
+"""bench.py -- EMC iterations/s of the CUDA hot path on synthetic data shaped like the paper's.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over the config's workload: every EMC iteration the
+config names (C2: three, C5: five with a growing rotation list), each iteration = Expand ->
+log-likelihood -> normalise -> update -> Compress, through the C ABI (emc_iterate).
+
+Prints ONE JSON line (rank 0).  `value` = iterations/s with all inputs resident in HBM; `e2e` = the
+same through the C-ABI call with HOST buffers (pinned counts streamed by the library, model and
+geometry copied in, model and log-likelihood copied out inside the timed region); `roofline` is
+for the dominant kernel, timed live with CUDA events recorded by the library on the launching
+stream (EMC_PROFILE_STAGES); `cpu_baseline` is the CPU oracle timed on this box's host cores on a
+bounded sample (N = 1 only).  With --gpus N > 1 (torchrun) the path does not shard (north_star:
+one GPU, no collectives): every rank runs an independent replica, scaling = "weak".
+`--impl reference` times the oracle itself (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import pathlib
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = pathlib.Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import numpy as np  # noqa: E402
+
+METRIC = "emc_iterations_per_s"
+UNIT = "iterations/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", help="C1..C5 (BASELINE.json configs[0..4]); default C2 = configs[1]")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--planes2", action="store_true", help="opt-in 2-plane split of P (reported separately)")
+    ap.add_argument("--weighted", action="store_true", help="Compress by eq. (2.12) instead of eq. (2.10)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
+                    source="measured")
+    # fallback stated by /opt/skills/guides/B200_PROFILING.md
+    return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+# ------------------------------------------------------------------------------ CPU oracle leg
+
+def oracle_sample(inp, stage, n_rot_s, n_pat_s):
+    """Times the oracle's five stages on a bounded sample and extrapolates one full iteration
+    (stages 1, 5 are linear in R; stages 2-4 bilinear in R x N).  Returns (seconds_full, dict)."""
+    from oracle import emc_oracle as o
+
+    cfg = inp.cfg
+    quat, wgt = inp.quat[stage], inp.weight[stage]
+    n_rot, n_pat = len(quat), cfg.n_pat
+    rs, ns = min(n_rot, n_rot_s), min(n_pat, n_pat_s)
+    qs = quat[:rs]
+    ws = (wgt[:rs] / wgt[:rs].sum()).astype(np.float32)
+    ks = inp.counts[:ns]
+    t = {}
+    t0 = time.perf_counter()
+    w, idx = o.expand(inp.model_init, inp.q, qs)
+    t["expand"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    big_l, _ = o.loglik(w, idx, ks, inp.mask)
+    t["loglik"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    p, _, _ = o.normalize(big_l.astype(np.float32), ws)
+    t["normalize"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    wn, s = o.update(p.astype(np.float32), ks, inp.mask)
+    t["update"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.compress(wn, inp.q, qs, inp.mask, cfg.n, slice_w=(s > 0).astype(np.float32))
+    t["compress"] = time.perf_counter() - t0
+    lin = n_rot / rs
+    bil = (n_rot * n_pat) / (rs * ns)
+    full = (t["expand"] + t["compress"]) * lin + (t["loglik"] + t["normalize"] + t["update"]) * bil
+    return full, dict(times=t, sample_seconds=sum(t.values()), n_rot_sample=rs, n_pat_sample=ns)
+
+
+def sample_sizes(cfg):
+    """Bounded sample: about 10-30 s of oracle work on a few host cores."""
+    budget = 4.0e11                                         # multiply-adds of the three float64 matmuls
+    n_rot_s = min(max(cfg.n_rot), 2048)
+    n_pat_s = int(max(64, min(cfg.n_pat, budget / (3.0 * n_rot_s * cfg.n_pix))))
+    return n_rot_s, n_pat_s
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+
+        n = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+        return max(n) if n else 1
+    except Exception:
+        return 1
+
+
+def cpu_baseline(inp):
+    cfg = inp.cfg
+    n_rot_s, n_pat_s = sample_sizes(cfg)
+    total, parts = 0.0, []
+    for stage in range(cfg.n_iter):
+        if stage > 0 and cfg.n_rot[stage] == cfg.n_rot[stage - 1]:
+            full = parts[-1]["full"]                        # same rotation list: same cost
+        else:
+            full, info = oracle_sample(inp, stage, n_rot_s, n_pat_s)
+            parts.append(dict(full=full, **info))
+        total += full
+    value = cfg.n_iter / total
+    sample = (f"oracle/emc_oracle.py stage by stage on the first {parts[0]['n_rot_sample']} rotations x "
+              f"{parts[0]['n_pat_sample']} patterns x all {cfg.n_pix} pixels of {cfg.name} "
+              f"({sum(p['sample_seconds'] for p in parts):.1f} s of CPU work), extrapolated linearly in R "
+              f"(expand, compress) and bilinearly in R x N (loglik, normalize, update) to the full workload")
+    return dict(value=value, unit=UNIT, cores=host_threads(), kind="oracle", sample=sample)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from emc_inputs import CONFIGS, make_inputs
+
+    cfg = CONFIGS[args.config]
+    n_rot_s, n_pat_s = sample_sizes(cfg)
+    inp = make_inputs(cfg, n_pat=min(cfg.n_pat, max(n_pat_s, 512)))
+    inp.cfg = cfg                                           # extrapolate to the full pattern count
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        base = cpu_baseline(inp)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    line = dict(impl="reference", metric=METRIC, value=base["value"], unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * cfg.n_iter / base["value"], higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=workload_name(cfg), note="CPU oracle on a bounded sample, extrapolated"),
+                cpu_baseline=base, sample_wall_s=statistics.mean(times),
+                e2e=dict(value=base["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+def workload_name(cfg):
+    r = "->".join(str(x) for x in cfg.n_rot) if len(set(cfg.n_rot)) > 1 else str(cfg.n_rot[0])
+    return (f"{cfg.name}: model {cfg.n}^3 fp32, detector {cfg.n_det}x{cfg.n_det}, R={r}, N={cfg.n_pat} "
+            f"{cfg.count_dtype} patterns at {cfg.mean_photons} photons/pixel, {cfg.n_iter} iteration(s)"
+            + (f", pattern chunks of {cfg.n_pat_chunk}" if cfg.n_pat_chunk < cfg.n_pat else ""))
+
+
+# ------------------------------------------------------------------------------ clocks
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index):
+        import torch
+
+        self.path = tempfile.NamedTemporaryFile(prefix="emc_clocks_", suffix=".csv", delete=False).name
+        sel = str(device_index)
+        try:
+            sel = "GPU-" + str(torch.cuda.get_device_properties(device_index).uuid)
+        except Exception:
+            pass
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", sel, f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in open(self.path).read().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.path)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), power_w_max=max(power), samples=len(sm),
+                    reasons=sorted(reasons))
+
+
+# ------------------------------------------------------------------------------ our arm
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1409_4256_b200 as emc
+    from emc_inputs import CONFIGS, make_inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = CONFIGS[args.config]
+    inp = make_inputs(cfg)                                   # every rank: an independent replica
+    peaks = measured_peaks()
+
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    d_model0, d_q, d_mask, d_counts = dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.counts)
+    # consecutive iterations on the same rotation list go into one emc_iterate call
+    plan = []
+    for s in range(cfg.n_iter):
+        if plan and cfg.n_rot[s] == cfg.n_rot[s - 1]:
+            plan[-1][2] += 1
+        else:
+            plan.append([dev(inp.quat[s]), dev(inp.weight[s]), 1, inp.quat[s], inp.weight[s]])
+    flags = (emc.EMC_PLANES_2 if args.planes2 else 0) | (emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0)
+    chunk = cfg.n_pat_chunk if cfg.n_pat_chunk < cfg.n_pat else 0
+    ws_bytes = max(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, r, cfg.n_pat_chunk, emc.EMC_PATTERNS_ON_HOST)
+                   for r in cfg.n_rot)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    d_ll = torch.zeros(cfg.n_iter, dtype=torch.float64, device="cuda")
+    bufs = [torch.empty_like(d_model0), torch.empty_like(d_model0)]
+
+    def step(f):
+        """all iterations of the config, device-resident inputs"""
+        src, k, it0 = d_model0, 0, 0
+        for quat, wgt, n_it, _, _ in plan:
+            emc.emc_iterate(src, d_q, d_mask, quat, wgt, d_counts, n_iter=n_it, n_pat_chunk=chunk, flags=f, ws=ws,
+                            model_out=bufs[k], loglik=d_ll[it0:it0 + n_it])
+            src, k, it0 = bufs[k], 1 - k, it0 + n_it
+        return src
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step(flags)
+    emc.emc_check(ws)
+    emc.emc_profile_read()
+
+    clocks = ClockSampler(local)
+    launches0 = emc.emc_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step(flags | emc.EMC_PROFILE_STAGES)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = emc.emc_launch_count() - launches0
+    clk = clocks.stop()
+    prof = emc.emc_profile_read()
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * args.steps * cfg.n_iter / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers
+    h_counts = torch.from_numpy(inp.counts).pin_memory()
+    h_model = torch.from_numpy(inp.model_init).pin_memory()
+    h_q, h_mask = torch.from_numpy(inp.q).pin_memory(), torch.from_numpy(inp.mask).pin_memory()
+    h_rot = [(torch.from_numpy(np.ascontiguousarray(q)).pin_memory(), torch.from_numpy(w).pin_memory())
+             for _, _, _, q, w in plan]
+    h_out = torch.empty_like(h_model).pin_memory()
+    h_ll = torch.empty(cfg.n_iter, dtype=torch.float64).pin_memory()
+    e_model, e_q, e_mask = torch.empty_like(d_model0), torch.empty_like(d_q), torch.empty_like(d_mask)
+    e_rot = [(torch.empty_like(q), torch.empty_like(w)) for q, w, _, _, _ in plan]
+    h2d = (h_counts.numel() * h_counts.element_size() * (cfg.n_iter if chunk else len(plan))
+           + h_model.numel() * 4 + h_q.numel() * 4 + h_mask.numel()
+           + sum(q.numel() * 4 + w.numel() * 4 for q, w in h_rot))
+    d2h = h_out.numel() * 4 + h_ll.numel() * 8
+
+    def step_e2e():
+        e_model.copy_(h_model, non_blocking=True)
+        e_q.copy_(h_q, non_blocking=True)
+        e_mask.copy_(h_mask, non_blocking=True)
+        src, k, it0 = e_model, 0, 0
+        for (hq, hw), (dq, dw), (_, _, n_it, _, _) in zip(h_rot, e_rot, plan):
+            dq.copy_(hq, non_blocking=True)
+            dw.copy_(hw, non_blocking=True)
+            emc.emc_iterate(src, e_q, e_mask, dq, dw, h_counts, n_iter=n_it, n_pat_chunk=chunk,
+                            flags=flags | emc.EMC_PATTERNS_ON_HOST, ws=ws, model_out=bufs[k],
+                            loglik=d_ll[it0:it0 + n_it])
+            src, k, it0 = bufs[k], 1 - k, it0 + n_it
+        h_out.copy_(src, non_blocking=True)
+        h_ll.copy_(d_ll, non_blocking=True)
+        torch.cuda.current_stream().synchronize()           # the user reads the result
+
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step_e2e()
+    ev1.record()
+    barrier()
+    ms_e2e = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e_value = world * args.steps * cfg.n_iter / (ms_e2e * 1e-3)
+
+    # ---- rooflines from the live per-stage CUDA-event times
+    p_eff = int(inp.mask.sum())
+    n_planes_p = 2 if args.planes2 else 3
+    rn = sum(r * cfg.n_pat for r in cfg.n_rot) * args.steps            # (rotation, pattern) pairs processed
+    rp = sum(cfg.n_rot) * args.steps
+    g = cfg.n ** 3
+    stage_ms = {k: v[0] for k, v in prof.items()}
+    stage_spans = {k: v[1] for k, v in prof.items()}
+    useful = 2.0 * rn * p_eff                                           # flops of ONE contraction, all launches
+    tf = lambda fl, ms_: fl / (ms_ * 1e-3) / 1e12 if ms_ > 0 else 0.0
+    gbs = lambda by, ms_: by / (ms_ * 1e-3) / 1e9 if ms_ > 0 else 0.0
+    stages = {
+        "loglik": dict(ms=stage_ms["loglik"], launches=stage_spans["loglik"], bound="tensor",
+                       useful_tflops=tf(useful, stage_ms["loglik"]),
+                       issued_tflops=tf(2 * useful, stage_ms["loglik"]), planes=2, dtype="fp16x2"),
+        "update": dict(ms=stage_ms["update"], launches=stage_spans["update"], bound="tensor",
+                       useful_tflops=tf(useful, stage_ms["update"]),
+                       issued_tflops=tf(n_planes_p * useful, stage_ms["update"]), planes=n_planes_p,
+                       dtype=f"bf16x{n_planes_p}"),
+        "expand": dict(ms=stage_ms["expand"], bound="hbm",
+                       gbs=gbs(rp * cfg.n_pix * 4.0 + 4.0 * g * stage_spans["expand"], stage_ms["expand"])),
+        "normalize": dict(ms=stage_ms["normalize"], bound="hbm", gbs=gbs(8.0 * rn, stage_ms["normalize"])),
+        "compress": dict(ms=stage_ms["compress"], bound="hbm",
+                         gbs=gbs(rp * cfg.n_pix * 4.0 + 8.0 * g * stage_spans["compress"], stage_ms["compress"])),
+        "pack": dict(ms=stage_ms["pack"]),
+    }
+    for k in ("expand", "normalize", "compress"):
+        stages[k]["frac_of_hbm"] = stages[k]["gbs"] / peaks["hbm"]
+    for k in ("loglik", "update"):
+        stages[k]["frac_of_bf16_sustained"] = stages[k]["issued_tflops"] / peaks["bf16_sustained"]
+    dom = "update" if stage_ms["update"] >= stage_ms["loglik"] else "loglik"
+    traffic = None
+    tpath = ROOT / "profiles" / "traffic.json"
+    if tpath.exists():
+        traffic = json.loads(tpath.read_text()).get(f"{cfg.name}:{dom}")
+    roofline = dict(bound="tensor", kernel=f"plane_gemm_kernel ({dom}, {stages[dom]['dtype']})",
+                    achieved=stages[dom]["issued_tflops"], peak=peaks["bf16_sustained"], unit="TFLOP/s",
+                    frac=stages[dom]["issued_tflops"] / peaks["bf16_sustained"], traffic=traffic,
+                    peak_source=f"{peaks['source']} bf16 sustained (kernel timed inside a long step)",
+                    avg_launch_ms=stage_ms[dom] / max(1, stage_spans[dom]),
+                    note="achieved = 2*planes*R*N*P_eff flops per launch / CUDA-event launch time (issued MMA work of "
+                         "the split scheme on unmasked pixels); useful TFLOP/s is in stages")
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="fp16x2/bf16x3 operands, f32 accumulate", data="synthetic",
+                config=dict(workload=workload_name(cfg), parallelism="replicas only" if world > 1 else "1 GPU",
+                            l2="per-iteration working set exceeds the 126 MB L2, no flush" if cfg.name != "C1"
+                            else "working set fits L2 (launch-latency-bound config), no flush",
+                            compress="eq. (2.12)" if args.weighted else "eq. (2.10)", p_eff=p_eff),
+                clocks=clk,
+                e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                         ms_per_step=ms_e2e / args.steps),
+                gpu_launches=int(launches),
+                useful_tflops_loglik_plus_update=tf(2 * useful, stage_ms["loglik"] + stage_ms["update"]),
+                roofline=roofline, stages=stages,
+                loglik_per_iteration=[float(x) for x in d_ll.cpu().tolist()])
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(inp)
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -65,6 +65,8 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
                                       do not divide by s[r] */
 #define EMC_PLANES_2          0x8u /* opt-in: 2 instead of 3 bf16 planes for P in emc_update
                                       (reported separately) */
+#define EMC_PROFILE_STAGES    0x20u /* emc_iterate records CUDA events on `stream` around every stage;
+                                      read (and reset) the sums with emc_profile_read() */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
                                         bisecting aid for the tcgen05 path, never the default) */
 
@@ -169,6 +171,13 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
  * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (results are then undefined),
  * EMC_ERR_CUDA if the stream is in error.  Clears the record. */
 EMC_API emc_status emc_check(void *ws, void *stream);
+
+/* Stages timed under EMC_PROFILE_STAGES (one thread at a time; at most 8192 spans between reads). */
+enum { EMC_STAGE_EXPAND = 0, EMC_STAGE_PACK = 1, EMC_STAGE_LOGLIK = 2, EMC_STAGE_NORMALIZE = 3,
+       EMC_STAGE_UPDATE = 4, EMC_STAGE_COMPRESS = 5, EMC_N_STAGES = 6 };
+/* Waits for the recorded events, returns per stage the summed device time in milliseconds (HOST
+ * array ms[EMC_N_STAGES]) and the number of spans (HOST array spans[EMC_N_STAGES]), and resets. */
+EMC_API emc_status emc_profile_read(double *ms, int *spans);
 
 /* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
 EMC_API uint64_t emc_launch_count(void);

@@ -23,11 +23,13 @@ EMC_ACCUMULATE = 0x2
 EMC_UPDATE_RAW = 0x4
 EMC_PLANES_2 = 0x8
 EMC_PATTERNS_ON_HOST = 0x10
+EMC_PROFILE_STAGES = 0x20
 EMC_DEBUG_SIMT = 0x100
+STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_workspace_bytes", "emc_expand", "emc_loglik", "emc_normalize", "emc_update", "emc_compress",
-           "emc_iterate", "emc_check", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+           "emc_iterate", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
 class EmcError(RuntimeError):
@@ -86,6 +88,8 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
                                 ci, ci, vp, vp, ci, vp, cu, vp, sz, vp]
     lib.emc_check.restype = ci
     lib.emc_check.argtypes = [vp, vp]
+    lib.emc_profile_read.restype = ci
+    lib.emc_profile_read.argtypes = [POINTER(c_double), POINTER(c_int)]
     lib.emc_launch_count.restype = c_uint64
     lib.emc_launch_count.argtypes = []
     for name in ("emc_strerror", "emc_last_cuda_error", "emc_version"):
@@ -273,6 +277,14 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
 def emc_check(ws):
     """Synchronises and raises EmcError(EMC_ERR_COUNT_RANGE) if a count exceeded EMC_MAX_COUNT."""
     _check(load().emc_check(ws.data_ptr(), _stream()), "emc_check")
+
+
+def emc_profile_read() -> dict:
+    """Per-stage device milliseconds and span counts recorded under EMC_PROFILE_STAGES; resets."""
+    ms = (c_double * len(STAGES))()
+    spans = (c_int * len(STAGES))()
+    _check(load().emc_profile_read(ms, spans), "emc_profile_read")
+    return {name: (ms[i], spans[i]) for i, name in enumerate(STAGES)}
 
 
 def emc_launch_count() -> int:

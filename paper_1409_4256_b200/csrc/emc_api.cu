@@ -20,6 +20,35 @@ void note_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_re
 
 namespace {
 
+// ---- optional per-stage CUDA-event timing (EMC_PROFILE_STAGES): events are recorded on the caller's
+// stream around each stage of emc_iterate and summed by emc_profile_read().
+constexpr int kMaxSpans = 8192;
+struct Profiler {
+    cudaEvent_t beg[kMaxSpans], end[kMaxSpans];
+    int stage[kMaxSpans];
+    int created = 0, used = 0;
+};
+Profiler g_prof;
+
+struct Span {
+    int slot = -1;
+    cudaStream_t st;
+    Span(bool on, int stage, cudaStream_t stream) : st(stream) {
+        if (!on || g_prof.used >= kMaxSpans) return;
+        if (g_prof.used >= g_prof.created) {
+            if (cudaEventCreate(&g_prof.beg[g_prof.created]) != cudaSuccess) return;
+            if (cudaEventCreate(&g_prof.end[g_prof.created]) != cudaSuccess) return;
+            ++g_prof.created;
+        }
+        slot = g_prof.used++;
+        g_prof.stage[slot] = stage;
+        cudaEventRecord(g_prof.beg[slot], st);
+    }
+    ~Span() {
+        if (slot >= 0) cudaEventRecord(g_prof.end[slot], st);
+    }
+};
+
 size_t count_size(emc_count_type t) { return t == EMC_I32 ? 4 : (t == EMC_U16 ? 2 : 1); }
 
 // One layout serves every entry point; a call uses the parts it needs.
@@ -206,20 +235,25 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
     const int n_planes = (flags & EMC_PLANES_2) ? 2 : 3;
+    const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
 
     EMC_TRY(reset_header(l, st));
     const float *model_cur = model->model;
     for (int it = 0; it < n_iter; ++it) {
         // stage 1: Expand, with logW planes and S fused in
-        EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
-        EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                              l.planesL, l.ld_p, l.S, st));
+        {
+            Span sp(prof, EMC_STAGE_EXPAND, st);
+            EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
+            EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
+                                  l.planesL, l.ld_p, l.S, st));
+        }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
         for (int c = 0; c < n_chunks; ++c) {
             const int d0 = c * chunk;
             const int nc = n_pat - d0 < chunk ? n_pat - d0 : chunk;
             if (n_chunks > 1 || it == 0) {          // one resident chunk is packed once for all iterations
+                Span sp(prof, EMC_STAGE_PACK, st);
                 const uint8_t *src = (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz;
                 if (on_host) {
                     EMC_TRY_CUDA(cudaMemcpyAsync(l.stage, src, (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, st));
@@ -228,19 +262,34 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, l.ld_n, l.hdr, st));
             }
             // stage 2: L = logW K^T - S
-            EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, simt, st));
+            {
+                Span sp(prof, EMC_STAGE_LOGLIK, st);
+                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, simt, st));
+            }
             // stage 3: responsibilities of this chunk; s and LL add up over chunks
             float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
-            EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, n_planes,
-                                     (size_t)n_rot * l.ld_n, l.s, loglik + it, true, l.scratch, st));
+            {
+                Span sp(prof, EMC_STAGE_NORMALIZE, st);
+                EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, n_planes,
+                                         (size_t)n_rot * l.ld_n, l.s, loglik + it, true, l.scratch, st));
+            }
             // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
             const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
-            EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, n_planes, l.Wnum, l.s, epi, simt, st));
+            {
+                Span sp(prof, EMC_STAGE_UPDATE, st);
+                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, n_planes, l.Wnum, l.s, epi, simt, st));
+            }
         }
-        if (n_chunks > 1) EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
+        if (n_chunks > 1) {
+            Span sp(prof, EMC_STAGE_UPDATE, st);
+            EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
+        }
         // stage 5: Compress
-        EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
-                                model_out, nullptr, st));
+        {
+            Span sp(prof, EMC_STAGE_COMPRESS, st);
+            EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
+                                    model_out, nullptr, st));
+        }
         model_cur = model_out;
     }
     return EMC_OK;
@@ -253,6 +302,22 @@ emc_status emc_check(void *ws, void *stream) {
     EMC_TRY_CUDA(cudaMemcpy(&h, ws, sizeof(h), cudaMemcpyDeviceToHost));
     EMC_TRY_CUDA(cudaMemset(ws, 0, sizeof(h)));
     return h.max_count > EMC_MAX_COUNT ? EMC_ERR_COUNT_RANGE : EMC_OK;
+}
+
+emc_status emc_profile_read(double *ms, int *spans) {
+    if (!ms || !spans) return EMC_ERR_ARG;
+    for (int i = 0; i < EMC_N_STAGES; ++i) { ms[i] = 0.0; spans[i] = 0; }
+    emc_status rc = EMC_OK;
+    for (int i = 0; i < g_prof.used; ++i) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(g_prof.end[i]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, g_prof.beg[i], g_prof.end[i]);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "emc_profile_read"); break; }
+        ms[g_prof.stage[i]] += (double)t;
+        spans[g_prof.stage[i]] += 1;
+    }
+    g_prof.used = 0;
+    return rc;
 }
 
 uint64_t emc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
