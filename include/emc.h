@@ -56,6 +56,11 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
  * expected to be masked. */
 #define EMC_MAX_COUNT 256
 
+/* Responsibilities below 2^-100 are stored as 0 (DESIGN.md §3 G20): float32 P keeps full relative
+ * precision only down to there once it is split into three bf16 planes, and a rotation whose whole
+ * row lies below it has no data behind it (s[r] = 0: W'[r,:] = 0, slice skipped by Compress, G17). */
+#define EMC_P_MIN 7.888609052210118e-31f
+
 /* flags */
 #define EMC_COMPRESS_WEIGHTED 0x1u /* eq. (2.12): slice r enters Compress with
                                       weight s[r] = sum_d P[r,d]; default is eq. (2.10), weight 1 */
@@ -124,7 +129,8 @@ EMC_API emc_status emc_loglik(const float *W, const int32_t *idx, const emc_dete
                       void *ws, size_t ws_bytes, void *stream);
 
 /* Stage 3, normalisation over rotations (reconstructed eq. (2.4)):
- *   a = L[r,d] + log w_r;  m_d = max_r a;  P[r,d] = exp(a - m_d) / sum_r exp(a - m_d).
+ *   a = L[r,d] + log w_r;  m_d = max_r a;  P[r,d] = exp(a - m_d) / sum_r exp(a - m_d),
+ *   values below EMC_P_MIN stored as 0.
  *   L      [R][ld_n] float, in.
  *   P      [R][ld_n] float, out.
  *   s      [R] float, out: s[r] = sum_d P[r,d]            (added to with EMC_ACCUMULATE)

@@ -14,9 +14,10 @@
 // Kernel: persistent, one CTA per SM, warp-specialised.
 //   warp 0 lane 0 : TMA producer  (cp.async.bulk.tensor -> 128B-swizzled smem ring, mbarrier tx)
 //   warp 1 lane 0 : MMA issuer    (tcgen05.mma.cta_group::1.kind::f16, 128 x BN x 16, fp32 in TMEM)
-//   warps 2..5    : epilogue      (tcgen05.ld 32x32b -> registers -> fused row op -> global)
-// TMEM holds two accumulator stages of BN columns, so the epilogue of tile i overlaps the main
-// loop of tile i+1.
+//   warps 2..9    : epilogue      (tcgen05.ld 32x32b -> fp32 register accumulators -> fused row op -> global)
+// TMEM holds two accumulator stages of BN columns; the K loop alternates between them in chunks
+// of 512 elements so that the long sums are carried in round-to-nearest fp32 registers (tcgen05
+// accumulation truncates), and the drain of chunk i overlaps the MMAs of chunk i+1.
 #include "emc_internal.cuh"
 
 namespace emc {
@@ -27,8 +28,9 @@ constexpr int BLOCK_M = 128;
 constexpr int BLOCK_K = 64;                    // 64 x 2 B = one 128-byte swizzle row
 constexpr int UMMA_K = 16;
 constexpr int A_PLANE_BYTES = BLOCK_M * BLOCK_K * 2;
-constexpr int kGemmThreads = 192;
-constexpr int kNumEpiWarps = 4;
+constexpr int kGemmThreads = 320;             // TMA warp, MMA warp, 8 epilogue warps
+constexpr int kNumEpiWarps = 8;
+constexpr int kChunkKBlocks = 8;               // 8 x 64 = 512 K elements per TMEM accumulation chunk
 constexpr int kGroupM = 8;                     // tile rasterisation: 8 m-blocks share each n sweep
 
 template <int NP, int BN, int STAGES>
@@ -40,7 +42,7 @@ struct Cfg {
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory per CTA");
     static_assert(2 * BN <= 512, "two accumulator stages must fit the 512 TMEM columns");
     static_assert(BN % 16 == 0 && BN >= 16 && BN <= 256, "UMMA N for M = 128");
-    static_assert(BN % 32 == 0, "epilogue reads 32 columns at a time");
+    static_assert(BN % 64 == 0, "two epilogue warps per lane quarter read 32 columns at a time");
 };
 
 struct GemmArgs {
@@ -51,6 +53,7 @@ struct GemmArgs {
     const float *rowv;
     int epilogue;
     int vec_ok;          // out rows are 16-byte aligned
+    int k_chunk;         // k-blocks per TMEM accumulation chunk
     uint32_t idesc;
 };
 
@@ -157,6 +160,12 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int num_tiles = args.num_m_tiles * args.num_n_tiles;
+    // The K loop is cut into chunks of k_chunk k-blocks.  Each chunk is accumulated by the tensor
+    // core into one of the two TMEM stages (fresh accumulator), then drained by the epilogue warps
+    // into round-to-nearest fp32 register accumulators while the next chunk runs in the other
+    // stage.  Reason: tcgen05 accumulates with truncation, a bias of about -1.1e-9 per K element
+    // (measured); short chunks keep it at the level of fp32 rounding.
+    const int num_chunks = (args.num_k_blocks + args.k_chunk - 1) / args.k_chunk;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
@@ -207,93 +216,102 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             int acc = 0;
             uint32_t acc_phase = 0;
             for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                mbar_wait(tempty_bar + 8 * acc, acc_phase ^ 1u);     // epilogue has drained this stage
-                tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
-                for (int kb = 0; kb < args.num_k_blocks; ++kb) {
-                    mbar_wait(full_bar + 8 * stage, phase);
+                for (int ch = 0; ch < num_chunks; ++ch) {
+                    mbar_wait(tempty_bar + 8 * acc, acc_phase ^ 1u);     // epilogue has drained this stage
                     tc_fence_after();
-                    const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
-                    const uint64_t bdesc0 = umma_desc_sw128(sa + NP * A_PLANE_BYTES);
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+                    const int kb_end = min(args.num_k_blocks, (ch + 1) * args.k_chunk);
+                    for (int kb = ch * args.k_chunk; kb < kb_end; ++kb) {
+                        mbar_wait(full_bar + 8 * stage, phase);
+                        tc_fence_after();
+                        const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
+                        const uint64_t bdesc0 = umma_desc_sw128(sa + NP * A_PLANE_BYTES);
+                        const uint32_t first = (kb == ch * args.k_chunk) ? 0u : 1u;
 #pragma unroll
-                    for (int pl = 0; pl < NP; ++pl) {
-                        const uint64_t adesc0 = umma_desc_sw128(sa + pl * A_PLANE_BYTES);
+                        for (int pl = 0; pl < NP; ++pl) {
+                            const uint64_t adesc0 = umma_desc_sw128(sa + pl * A_PLANE_BYTES);
 #pragma unroll
-                        for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
-                            // advancing 16 elements along K inside the swizzle row = +32 B = +2 in the
-                            // (>>4) start-address field
-                            umma_f16(d_tmem, adesc0 + (uint64_t)(2 * k), bdesc0 + (uint64_t)(2 * k), args.idesc,
-                                     (kb | pl | k) != 0 ? 1u : 0u);
+                            for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+                                // advancing 16 elements along K inside the swizzle row = +32 B = +2 in the
+                                // (>>4) start-address field
+                                umma_f16(d_tmem, adesc0 + (uint64_t)(2 * k), bdesc0 + (uint64_t)(2 * k), args.idesc,
+                                         (pl | k) != 0 ? 1u : first);
+                            }
                         }
+                        umma_commit(empty_bar + 8 * stage);              // smem slot free once these MMAs retire
+                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                     }
-                    umma_commit(empty_bar + 8 * stage);              // smem slot free once these MMAs retire
-                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    umma_commit(tfull_bar + 8 * acc);                    // this chunk's partial sums are complete
+                    if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
                 }
-                umma_commit(tfull_bar + 8 * acc);                    // accumulator complete
-                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
         }
     } else {
-        // ================= epilogue warps 2..5 =================
-        const int quarter = warp & 3;                    // TMEM lanes 32*quarter .. +31 belong to this warp
+        // ================= epilogue warps 2..9 =================
+        // TMEM lanes 32*quarter .. +31 are the only ones this warp can read; two warps share a quarter
+        // and split the BN columns between them.
+        constexpr int CW = BN / 2;                       // columns per epilogue warp
+        const int quarter = warp & 3;
+        const int half = (warp - 2) >> 2;
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
             int m_blk, n_blk;
             tile_coords(tile, args, m_blk, n_blk);
-            mbar_wait(tfull_bar + 8 * acc, acc_phase);
-            tc_fence_after();
-            const int m = m_blk * BLOCK_M + quarter * 32 + lane;
-            const bool row_ok = m < args.M;
-            float rv = 0.f;
-            if (row_ok && args.rowv) rv = args.rowv[m];
-            float inv_ok = rv > 0.f ? 1.f : 0.f;
-            float *orow = args.out + (size_t)(row_ok ? m : 0) * args.ld_out;
-            const uint32_t t_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN);
-#pragma unroll 1
-            for (int c = 0; c < BN; c += 32) {
-                uint32_t v[32];
-                tmem_ld32(t_addr + (uint32_t)c, v);
-                const int n0 = n_blk * BN + c;
-                if (!row_ok || n0 >= args.N) continue;
-                float f[32];
+            float racc[CW];
 #pragma unroll
-                for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(v[j]);
-                if (args.epilogue == EPI_SUB_ROW) {
+            for (int j = 0; j < CW; ++j) racc[j] = 0.f;
+            for (int ch = 0; ch < num_chunks; ++ch) {
+                mbar_wait(tfull_bar + 8 * acc, acc_phase);
+                tc_fence_after();
+                const uint32_t t_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * CW);
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) f[j] -= rv;
-                } else if (args.epilogue == EPI_DIV_ROW) {
+                for (int c = 0; c < CW; c += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(t_addr + (uint32_t)c, v);
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) f[j] = inv_ok != 0.f ? f[j] / rv : 0.f;
+                    for (int j = 0; j < 32; ++j) racc[c + j] += __uint_as_float(v[j]);
                 }
-                float *o = orow + n0;
-                if (args.vec_ok && n0 + 32 <= args.N) {
-                    float4 *o4 = reinterpret_cast<float4 *>(o);
-                    if (args.epilogue == EPI_ADD) {
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tempty_bar + 8 * acc);
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+            const int m = m_blk * BLOCK_M + quarter * 32 + lane;
+            if (m < args.M) {
+                const float rv = args.rowv ? args.rowv[m] : 0.f;
+                float *orow = args.out + (size_t)m * args.ld_out;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            float4 t = o4[j];
-                            t.x += f[4 * j]; t.y += f[4 * j + 1]; t.z += f[4 * j + 2]; t.w += f[4 * j + 3];
-                            o4[j] = t;
+                for (int c = 0; c < CW; c += 4) {
+                    const int n0 = n_blk * BN + half * CW + c;
+                    if (n0 >= args.N) break;
+                    float f[4] = {racc[c], racc[c + 1], racc[c + 2], racc[c + 3]};
+                    if (args.epilogue == EPI_SUB_ROW) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) f[j] -= rv;
+                    } else if (args.epilogue == EPI_DIV_ROW) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) f[j] = rv > 0.f ? f[j] / rv : 0.f;
+                    }
+                    float *o = orow + n0;
+                    if (args.vec_ok && n0 + 4 <= args.N) {
+                        float4 *o4 = reinterpret_cast<float4 *>(o);
+                        if (args.epilogue == EPI_ADD) {
+                            float4 t = *o4;
+                            f[0] += t.x; f[1] += t.y; f[2] += t.z; f[3] += t.w;
                         }
+                        *o4 = make_float4(f[0], f[1], f[2], f[3]);
                     } else {
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) o4[j] = make_float4(f[4 * j], f[4 * j + 1], f[4 * j + 2], f[4 * j + 3]);
-                    }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        if (n0 + j < args.N) {
-                            if (args.epilogue == EPI_ADD) o[j] += f[j];
-                            else o[j] = f[j];
+                        for (int j = 0; j < 4; ++j) {
+                            if (n0 + j < args.N) {
+                                if (args.epilogue == EPI_ADD) o[j] += f[j];
+                                else o[j] = f[j];
+                            }
                         }
                     }
                 }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar + 8 * acc);
-            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
         }
     }
 
@@ -395,6 +413,7 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     a.num_n_tiles = ceil_div(g.N, BN);
     a.num_k_blocks = ceil_div(g.K, BLOCK_K);
     a.out = g.out; a.ld_out = g.ld_out; a.rowv = g.rowv; a.epilogue = g.epilogue;
+    a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
     // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
     // N >> 3 in [17,23); M >> 4 in [24,29)

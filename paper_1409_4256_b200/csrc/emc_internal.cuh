@@ -92,6 +92,7 @@ struct GemmProblem {
     int ld_out;
     const float *rowv;  // [M] row vector of the epilogue (S for loglik, s for update) or null
     int epilogue;       // EPI_*
+    int k_chunk = 0;    // k-blocks (of 64) per TMEM accumulation chunk, 0 = default
 };
 enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-likelihood)
        EPI_STORE = 1,       // out = acc                                (raw update numerator)

@@ -125,6 +125,7 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
         if (col_ok) {
             const float a = L[o] + log_weight(weight, r, log_uniform);
             p = expf(a - mt) * iz;
+            if (p < EMC_P_MIN) p = 0.f;          // DESIGN.md §3 G20
             if (P) P[o] = p;
             if (planes) split_bf16(p, n_planes, planes, plane_stride, o);
         }
@@ -142,7 +143,9 @@ p_split_kernel(const float *__restrict__ P, int n_pat, int ld_n, __nv_bfloat16 *
                int ld_pl, int n_planes, size_t plane_stride) {
     const int d = blockIdx.y * 256 + threadIdx.x;
     if (d >= n_pat) return;
-    split_bf16(P[(size_t)blockIdx.x * ld_n + d], n_planes, planes, plane_stride, (size_t)blockIdx.x * ld_pl + d);
+    float p = P[(size_t)blockIdx.x * ld_n + d];
+    if (p < EMC_P_MIN) p = 0.f;
+    split_bf16(p, n_planes, planes, plane_stride, (size_t)blockIdx.x * ld_pl + d);
 }
 
 __global__ void __launch_bounds__(256)

@@ -1,0 +1,80 @@
+"""Parity at BASELINE.json's full size in the launch configuration bench.py times (config C2:
+64^3 model, 64x64 detector, R = 5000, N = 10000): the oracle finishes one full iteration of C2 in
+about a minute, so every output is compared in full, not sampled.  (`-m gpu`)"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+@pytest.fixture(scope="module")
+def c2(inputs_cache):
+    inp = inputs_cache("C2")
+    ref = o.iterate(inp.model_init, inp.q, inp.mask, inp.quat[0], inp.weight[0], inp.counts)
+    return inp, ref
+
+
+def test_c2_stagewise_and_end_to_end(c2):
+    inp, ref = c2
+    cfg = inp.cfg
+    d_q, d_mask, d_quat, d_w, d_k = dev(inp.q), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]), dev(inp.counts)
+
+    # stage 1: index map bit-exact over all 5000 x 4096 samples
+    w, idx = emc.emc_expand(dev(inp.model_init), d_q, d_quat)
+    assert np.array_equal(host(idx), ref["idx"])
+    assert np.all(np.abs(host(w) - ref["W"]) <= 1e-5 * np.abs(ref["W"]) + 1e-9 * np.abs(ref["W"]).max())
+    del w, idx
+
+    # stage 2 on the oracle's W: |dL| <= 1e-5 A everywhere
+    big_l, big_a = o.loglik(ref["W"], ref["idx"], inp.counts, inp.mask)
+    got = host(emc.emc_loglik(dev(ref["W"]), dev(ref["idx"]), d_q, d_mask, d_k))
+    err = np.abs(got - big_l) / big_a
+    assert err.max() <= 1e-5, f"max |dL|/A = {err.max():.3e}"
+    del got, err
+
+    # stage 4 on the oracle's P (signed mean exposes an accumulation bias)
+    n_pat = cfg.n_pat
+    p = torch.zeros((cfg.n_rot[0], emc.ld_for(n_pat)), dtype=torch.float32, device="cuda")
+    p[:, :n_pat] = dev(ref["P"])
+    wn = host(emc.emc_update(p[:, :n_pat], dev(ref["s"].astype(np.float32)), d_q, d_mask, d_k))
+    scale = np.abs(ref["Wn"]).max()
+    rel = (wn - ref["Wn"]) / (np.abs(ref["Wn"]) + 1e-7 * scale)
+    assert np.abs(rel).max() <= 1e-5, f"max rel dW' = {np.abs(rel).max():.3e}"
+    big = ref["Wn"] > 1e-3 * scale
+    assert abs(rel[big].mean()) <= 2e-6, f"mean signed rel dW' = {rel[big].mean():+.3e}"
+    del p, wn, rel
+
+    # stage 5 on the oracle's W'
+    s32 = ref["s"].astype(np.float32)
+    m_ref, _, den_ref = o.compress(ref["Wn"], inp.q, inp.quat[0], inp.mask, cfg.n, slice_w=(s32 > 0).astype(np.float32))
+    m, den = emc.emc_compress(dev(ref["Wn"]), dev(s32), d_q, d_mask, d_quat, cfg.n, want_den=True)
+    m, den, m_ref = host(m).reshape(-1), host(den), m_ref.reshape(-1)
+    cov = den_ref >= 1e-6 * den_ref.max()
+    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12), \
+        f"max rel {np.max(np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-12)):.3e}"
+
+    # whole iteration, as bench.py launches it
+    out = emc.emc_iterate(dev(inp.model_init), d_q, d_mask, d_quat, d_w, d_k, want_p=True)
+    emc.emc_check(out["ws"])
+    bound = 1e-6 + 2.0 * ref["P"] * (2e-5 * big_a.max(axis=0))[None, :]
+    pg = host(out["P"])
+    assert np.all(np.abs(pg - ref["P"]) <= bound), f"max dP {np.abs(pg - ref['P']).max():.3e}"
+    assert abs(float(host(out["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"])
+    mg = host(out["model"]).reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    mr = ref["model"].reshape(-1)
+    rel = np.abs(mg[cov] - mr[cov]) / (np.abs(mr[cov]) + 1e-6 * np.abs(mr).max())
+    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2, f"model rel: median {np.median(rel):.2e} max {rel.max():.2e}"

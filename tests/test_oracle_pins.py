@@ -427,3 +427,12 @@ def test_masked_counts_never_matter():
     k2[:, inp.mask == 0] = 7
     b = o.iterate(inp.model_init, inp.q, inp.mask, inp.quat[0], inp.weight[0], k2)
     assert np.array_equal(a["model"], b["model"]) and np.array_equal(a["P"], b["P"])
+
+
+def test_normalize_flushes_below_p_min():
+    """G20: responsibilities below 2^-100 are stored as 0; a row made only of such values has s = 0."""
+    big_l = np.array([[0.0, 0.0], [-60.0, -80.0], [-69.0, -70.0]], np.float32)    # e^-69 > 2^-100 > e^-70
+    p, s, _ = o.normalize(big_l, np.full(3, 1 / 3, np.float32))
+    assert p[2, 0] > 0 and p[2, 1] == 0 and p[1, 1] == 0 and p[1, 0] > 0
+    assert abs(p[:, 0].sum() - 1) < 1e-12 and s[2] == p[2, 0]
+    assert o.P_MIN == 2.0 ** -100
