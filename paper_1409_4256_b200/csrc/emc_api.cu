@@ -62,7 +62,7 @@ struct Layout {
     __nv_bfloat16 *planesP;   // [3][R][ld_n]  P hi / mid / lo
     float *s;                 // [R]
     float *Wnum;              // [R][P]        update numerators -> W'
-    float2 *acc;              // [G]           (num, den)
+    float2 *acc;              // [2 G]         two staggered (num, den) grids
     float *scratch;           // normalise partials
     void *stage;              // one chunk of raw counts (patterns on host)
     int ld_p, ld_n;
@@ -84,7 +84,7 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.planesP = a.take<__nv_bfloat16>(3 * R * l.ld_n);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
-    l.acc = a.take<float2>((size_t)n * n * n);
+    l.acc = a.take<float2>((size_t)2 * n * n * n);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
@@ -176,7 +176,9 @@ emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *de
 emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
                          float *s, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
                          void *stream) {
-    if (!L || !rot || rot->n_rot <= 0 || n_pat <= 0 || ld_n < n_pat || !P) return EMC_ERR_ARG;
+    if (!L || !rot || rot->n_rot <= 0 || n_pat <= 0 || ld_n < n_pat || !P || (ld_n & 3) || ((uintptr_t)L & 15) ||
+        ((uintptr_t)P & 15))
+        return EMC_ERR_ARG;
     const size_t need = round_up(sizeof(float) * normalize_scratch_floats(rot->n_rot, ld_n), 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
     return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, 0, 0, s, loglik,
@@ -208,7 +210,7 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
                         unsigned flags, void *ws, size_t ws_bytes, void *stream) {
     if (!Wnew || !det_ok(det) || !rot_ok(rot) || !model_out) return EMC_ERR_ARG;
     if (!sizes_ok(n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
-    const size_t need = round_up(sizeof(float2) * (size_t)n * n * n, 1024);
+    const size_t need = round_up(sizeof(float2) * (size_t)2 * n * n * n, 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
     return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, det->q, det->mask, det->n_pix,
                            rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);
