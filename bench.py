@@ -44,7 +44,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2", help="C1..C5 (BASELINE.json configs[0..4]); default C2 = configs[1]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--planes2", action="store_true", help="opt-in 2-plane split of P (reported separately)")
+    ap.add_argument("--bf16x3", action="store_true", help="opt-in: P as three unscaled bf16 planes in the update (3 MMAs per k-step)")
     ap.add_argument("--weighted", action="store_true", help="Compress by eq. (2.12) instead of eq. (2.10)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -252,7 +252,7 @@ def main():
             plan[-1][2] += 1
         else:
             plan.append([dev(inp.quat[s]), dev(inp.weight[s]), 1, inp.quat[s], inp.weight[s]])
-    flags = (emc.EMC_PLANES_2 if args.planes2 else 0) | (emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0)
+    flags = (emc.EMC_UPDATE_BF16X3 if args.bf16x3 else 0) | (emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0)
     chunk = cfg.n_pat_chunk if cfg.n_pat_chunk < cfg.n_pat else 0
     ws_bytes = max(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, r, cfg.n_pat_chunk, emc.EMC_PATTERNS_ON_HOST)
                    for r in cfg.n_rot)
@@ -346,7 +346,7 @@ def main():
 
     # ---- rooflines from the live per-stage CUDA-event times
     p_eff = int(inp.mask.sum())
-    n_planes_p = 2 if args.planes2 else 3
+    n_planes_p = 3 if args.bf16x3 else 2
     rn = sum(r * cfg.n_pat for r in cfg.n_rot) * args.steps            # (rotation, pattern) pairs processed
     rp = sum(cfg.n_rot) * args.steps
     g = cfg.n ** 3
@@ -362,7 +362,7 @@ def main():
         "update": dict(ms=stage_ms["update"], launches=stage_spans["update"], bound="tensor",
                        useful_tflops=tf(useful, stage_ms["update"]),
                        issued_tflops=tf(n_planes_p * useful, stage_ms["update"]), planes=n_planes_p,
-                       dtype=f"bf16x{n_planes_p}"),
+                       dtype="bf16x3" if args.bf16x3 else "fp16x2 chunk-scaled"),
         "expand": dict(ms=stage_ms["expand"], bound="hbm",
                        gbs=gbs(rp * cfg.n_pix * 4.0 + 4.0 * g * stage_spans["expand"], stage_ms["expand"])),
         "normalize": dict(ms=stage_ms["normalize"], bound="hbm", gbs=gbs(8.0 * rn, stage_ms["normalize"])),
@@ -389,7 +389,7 @@ def main():
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="fp16x2/bf16x3 operands, f32 accumulate", data="synthetic",
+                dtype="fp16x2 operand planes, f32 accumulate", data="synthetic",
                 config=dict(workload=workload_name(cfg), parallelism="replicas only" if world > 1 else "1 GPU",
                             l2="per-iteration working set exceeds the 126 MB L2, no flush" if cfg.name != "C1"
                             else "working set fits L2 (launch-latency-bound config), no flush",

@@ -52,9 +52,9 @@ typedef enum {
 typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
 
 /* Largest photon count in an unmasked pixel that the exact 16-bit tensor-core operands hold
- * (bf16 holds every integer up to 256; DESIGN.md §6 "precision scheme").  Saturated pixels are
- * expected to be masked. */
-#define EMC_MAX_COUNT 256
+ * (fp16 holds every integer up to 2048; DESIGN.md §6 "precision scheme"; 256 with
+ * EMC_UPDATE_BF16X3).  Saturated pixels are expected to be masked. */
+#define EMC_MAX_COUNT 2048
 
 /* Responsibilities below 2^-100 are stored as 0 (DESIGN.md §3 G20): float32 P keeps full relative
  * precision only down to there once it is split into three bf16 planes, and a rotation whose whole
@@ -68,8 +68,9 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
                                       (pattern chunks, DESIGN.md §3 G9) */
 #define EMC_UPDATE_RAW        0x4u /* emc_update: leave Wnew as the numerator of eq. (2.11),
                                       do not divide by s[r] */
-#define EMC_PLANES_2          0x8u /* opt-in: 2 instead of 3 bf16 planes for P in emc_update
-                                      (reported separately) */
+#define EMC_UPDATE_BF16X3     0x8u /* opt-in: P enters the update contraction as three unscaled bf16
+                                      planes (3 MMAs per k-step) instead of two chunk-scaled fp16
+                                      planes (2 MMAs) */
 #define EMC_PROFILE_STAGES    0x20u /* emc_iterate records CUDA events on `stream` around every stage;
                                       read (and reset) the sums with emc_profile_read() */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
@@ -113,9 +114,11 @@ EMC_API size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk,
  *   W   [R][P] float, out.
  *   idx [R][P] int32, out, or NULL: linear index (b_x*n + b_y)*n + b_z of the base corner
  *       b = floor(x), or -1 outside the grid.  The coordinate arithmetic is pinned (DESIGN.md §3
- *       G4) so this map is bit-exact against the oracle. */
+ *       G4) so this map is bit-exact against the oracle.
+ *   ws  workspace or NULL.  With a workspace (n even) the model is first re-laid as blocked
+ *       staggered copies so that a sample is two 16-byte loads; without, plain gathers. */
 EMC_API emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
-                      float *W, int32_t *idx, void *stream);
+                      float *W, int32_t *idx, void *ws, size_t ws_bytes, void *stream);
 
 /* Stage 2, Poisson log-likelihood (north_star stage 2; Poisson model of PAPER.md:68; the E-step
  * numerator of PAPER.md:166):

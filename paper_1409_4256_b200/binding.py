@@ -17,11 +17,11 @@ from . import build as _build
 EMC_OK = 0
 EMC_ERR_ARG, EMC_ERR_UNSUPPORTED, EMC_ERR_WORKSPACE, EMC_ERR_CUDA, EMC_ERR_COUNT_RANGE = -1, -2, -3, -4, -5
 EMC_I32, EMC_U16, EMC_U8 = 0, 1, 2
-EMC_MAX_COUNT = 256
+EMC_MAX_COUNT = 2048
 EMC_COMPRESS_WEIGHTED = 0x1
 EMC_ACCUMULATE = 0x2
 EMC_UPDATE_RAW = 0x4
-EMC_PLANES_2 = 0x8
+EMC_UPDATE_BF16X3 = 0x8
 EMC_PATTERNS_ON_HOST = 0x10
 EMC_PROFILE_STAGES = 0x20
 EMC_DEBUG_SIMT = 0x100
@@ -74,7 +74,7 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_workspace_bytes.restype = sz
     lib.emc_workspace_bytes.argtypes = [ci, ci, ci, ci, cu]
     lib.emc_expand.restype = ci
-    lib.emc_expand.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), vp, vp, vp]
+    lib.emc_expand.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), vp, vp, vp, sz, vp]
     lib.emc_loglik.restype = ci
     lib.emc_loglik.argtypes = [vp, vp, POINTER(_Detector), POINTER(_Patterns), ci, vp, ci, cu, vp, sz, vp]
     lib.emc_normalize.restype = ci
@@ -172,15 +172,18 @@ def _ws(ws, n, n_pix, n_rot, n_chunk, flags=0):
 
 # ---------------------------------------------------------------------------- the six calls
 
-def emc_expand(model, q, quat, want_idx=True):
-    """Stage 1 (eq. 2.9).  Returns (W [R,P] float32, idx [R,P] int32 or None)."""
+def emc_expand(model, q, quat, want_idx=True, use_ws=True):
+    """Stage 1 (eq. 2.9).  Returns (W [R,P] float32, idx [R,P] int32 or None).  use_ws=False takes the
+    library's plain-gather kernel instead of the blocked-copy one."""
     n = model.shape[0]
     m = _Model(n, _dev(model, torch.float32, "model"))
     det = _detector(q, None)
     rot = _rotations(quat, None)
     w = torch.empty((rot.n_rot, det.n_pix), dtype=torch.float32, device=model.device)
     idx = torch.empty((rot.n_rot, det.n_pix), dtype=torch.int32, device=model.device) if want_idx else None
-    _check(load().emc_expand(m, det, rot, w.data_ptr(), idx.data_ptr() if want_idx else None, _stream()), "emc_expand")
+    ws = make_workspace(n, det.n_pix, rot.n_rot, 1) if use_ws else None
+    _check(load().emc_expand(m, det, rot, w.data_ptr(), idx.data_ptr() if want_idx else None,
+                             ws.data_ptr() if use_ws else None, ws.numel() if use_ws else 0, _stream()), "emc_expand")
     return w, idx
 
 

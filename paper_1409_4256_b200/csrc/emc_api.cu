@@ -57,12 +57,14 @@ struct Layout {
     __half *planesL;          // [2][R][ld_p]  logW hi / lo
     float *S;                 // [R]           sum_{p:mask} W
     __half *Kc;               // [Nc][ld_p]    counts, row = pattern
-    __nv_bfloat16 *KT;        // [P][ld_n]     counts, row = pixel
+    void *KT;                 // [P][ld_n]     counts, row = pixel (fp16; bf16 for EMC_UPDATE_BF16X3)
     float *L;                 // [R][ld_n]
-    __nv_bfloat16 *planesP;   // [3][R][ld_n]  P hi / mid / lo
+    void *planesP;            // [2][R][ld_n]  fp16 hi / lo of chunk-scaled P  (or [3] bf16 hi / mid / lo)
+    float *pscale;            // [ld_n/512][R] inverse chunk scales of planesP
     float *s;                 // [R]
     float *Wnum;              // [R][P]        update numerators -> W'
     float2 *acc;              // [2 G]         two staggered (num, den) grids
+    float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
     void *stage;              // one chunk of raw counts (patterns on host)
     int ld_p, ld_n;
@@ -79,12 +81,14 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.planesL = a.take<__half>(2 * R * l.ld_p);
     l.S = a.take<float>(R);
     l.Kc = a.take<__half>((size_t)n_chunk * l.ld_p);
-    l.KT = a.take<__nv_bfloat16>((size_t)n_pix * l.ld_n);
+    l.KT = a.take<uint16_t>((size_t)n_pix * l.ld_n);
     l.L = a.take<float>(R * l.ld_n);
-    l.planesP = a.take<__nv_bfloat16>(3 * R * l.ld_n);
+    l.planesP = a.take<uint16_t>(3 * R * l.ld_n);
+    l.pscale = a.take<float>((size_t)ceil_div(l.ld_n, 512) * R);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
     l.acc = a.take<float2>((size_t)2 * n * n * n);
+    l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
@@ -123,13 +127,14 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     return launch_plane_gemm(g, simt, st);
 }
 
-emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, int n_planes, float *out,
+emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, bool bf16x3, float *out,
                            const float *s, int epilogue, bool simt, cudaStream_t st) {
     GemmProblem g;
-    g.A = l.planesP; g.B = l.KT; g.n_planes = n_planes;
+    g.A = l.planesP; g.B = l.KT; g.n_planes = bf16x3 ? 3 : 2;
     g.M = n_rot; g.N = n_pix; g.K = n_pat;
     g.lda = l.ld_n; g.ldb = l.ld_n; g.plane_stride = (size_t)n_rot * l.ld_n;
-    g.a_fmt = FMT_BF16; g.b_fmt = FMT_BF16;
+    g.a_fmt = g.b_fmt = bf16x3 ? FMT_BF16 : FMT_F16;
+    g.chunk_scale = bf16x3 ? nullptr : l.pscale;
     g.out = out; g.ld_out = n_pix; g.rowv = s; g.epilogue = epilogue;
     return launch_plane_gemm(g, simt, st);
 }
@@ -148,11 +153,16 @@ size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigne
 }
 
 emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
-                      float *W, int32_t *idx, void *stream) {
+                      float *W, int32_t *idx, void *ws, size_t ws_bytes, void *stream) {
     if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || (!W && !idx)) return EMC_ERR_ARG;
     if (!sizes_ok(model->n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
+    float *blocked = nullptr;
+    if (ws) {
+        EMC_TRY(check_ws(ws, ws_bytes, round_up(sizeof(float) * expand_scratch_floats(model->n), 1024)));
+        blocked = (float *)ws;
+    }
     return launch_expand(model->model, model->n, det->q, det->mask, det->n_pix, rot->quat, rot->n_rot, W, idx,
-                         nullptr, 0, nullptr, (cudaStream_t)stream);
+                         nullptr, 0, nullptr, blocked, (cudaStream_t)stream);
 }
 
 emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *det,
@@ -168,7 +178,7 @@ emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *de
     EMC_TRY(reset_header(l, st));
     EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
     EMC_TRY(launch_logw_split(W, idx, det->mask, det->n_pix, n_rot, l.planesL, l.ld_p, l.S, st));
-    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, 0,
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, false, 0,
                         l.hdr, st));
     return run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, (flags & EMC_DEBUG_SIMT) != 0, st);
 }
@@ -181,7 +191,7 @@ emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, in
         return EMC_ERR_ARG;
     const size_t need = round_up(sizeof(float) * normalize_scratch_floats(rot->n_rot, ld_n), 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
-    return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, 0, 0, s, loglik,
+    return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, false, 0, nullptr, s, loglik,
                             (flags & EMC_ACCUMULATE) != 0, (float *)ws, (cudaStream_t)stream);
 }
 
@@ -195,13 +205,13 @@ emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detect
     cudaStream_t st = (cudaStream_t)stream;
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, 0, det->n_pix, n_rot, pat->n_pat, 0).total));
     const Layout l = carve(ws, 0, det->n_pix, n_rot, pat->n_pat, 0);
-    const int n_planes = (flags & EMC_PLANES_2) ? 2 : 3;
+    const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
     EMC_TRY(reset_header(l, st));
-    EMC_TRY(launch_p_split(P, n_rot, pat->n_pat, ld_n, l.planesP, l.ld_n, n_planes, (size_t)n_rot * l.ld_n, st));
-    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, l.ld_n,
+    EMC_TRY(launch_p_split(P, n_rot, pat->n_pat, ld_n, l.planesP, l.ld_n, bf16x3, (size_t)n_rot * l.ld_n, l.pscale, st));
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, bf16x3, l.ld_n,
                         l.hdr, st));
     const int epi = (flags & EMC_ACCUMULATE) ? EPI_ADD : (raw ? EPI_STORE : EPI_DIV_ROW);
-    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, n_planes, Wnew, s, epi,
+    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, bf16x3, Wnew, s, epi,
                            (flags & EMC_DEBUG_SIMT) != 0, st);
 }
 
@@ -236,7 +246,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     cudaStream_t st = (cudaStream_t)stream;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
-    const int n_planes = (flags & EMC_PLANES_2) ? 2 : 3;
+    const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
     const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
 
     EMC_TRY(reset_header(l, st));
@@ -247,7 +257,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
             Span sp(prof, EMC_STAGE_EXPAND, st);
             EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
             EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                                  l.planesL, l.ld_p, l.S, st));
+                                  l.planesL, l.ld_p, l.S, l.blocked, st));
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
@@ -261,7 +271,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                     EMC_TRY_CUDA(cudaMemcpyAsync(l.stage, src, (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, st));
                     src = (const uint8_t *)l.stage;
                 }
-                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, l.ld_n, l.hdr, st));
+                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, bf16x3, l.ld_n, l.hdr, st));
             }
             // stage 2: L = logW K^T - S
             {
@@ -272,14 +282,14 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
             float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
             {
                 Span sp(prof, EMC_STAGE_NORMALIZE, st);
-                EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, n_planes,
-                                         (size_t)n_rot * l.ld_n, l.s, loglik + it, true, l.scratch, st));
+                EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, bf16x3,
+                                         (size_t)n_rot * l.ld_n, l.pscale, l.s, loglik + it, true, l.scratch, st));
             }
             // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
             const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
             {
                 Span sp(prof, EMC_STAGE_UPDATE, st);
-                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, n_planes, l.Wnum, l.s, epi, simt, st));
+                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, simt, st));
             }
         }
         if (n_chunks > 1) {
@@ -303,7 +313,7 @@ emc_status emc_check(void *ws, void *stream) {
     EMC_TRY_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
     EMC_TRY_CUDA(cudaMemcpy(&h, ws, sizeof(h), cudaMemcpyDeviceToHost));
     EMC_TRY_CUDA(cudaMemset(ws, 0, sizeof(h)));
-    return h.max_count > EMC_MAX_COUNT ? EMC_ERR_COUNT_RANGE : EMC_OK;
+    return h.max_count > 0 ? EMC_ERR_COUNT_RANGE : EMC_OK;      // the pack kernel records only counts over its limit
 }
 
 emc_status emc_profile_read(double *ms, int *spans) {

@@ -63,7 +63,7 @@ compress_scatter_pairs_kernel(const float *__restrict__ Wn, const float *__restr
         const float v = Wn[(size_t)r * n_pix + p];
         const float x1 = s.tx * om, x0 = (1.f - s.tx) * om;
         const float y1 = s.ty, y0 = 1.f - s.ty, z1 = s.tz, z0 = 1.f - s.tz;
-        const int bz = s.base % n, row = s.base / n;          // row = b_x * n + b_y
+        const int bz = s.bz, row = s.bx * n + s.by;
         float4 *b = acc + (bz & 1 ? layer : 0) + (size_t)row * h + (bz >> 1);
         float f0, f1;
         f0 = x0 * y0 * z0; f1 = x0 * y0 * z1; red_add_v4(b, f0 * v, f0, f1 * v, f1);

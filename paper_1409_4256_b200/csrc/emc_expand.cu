@@ -89,6 +89,89 @@ expand_kernel(const float *__restrict__ model, int n, const float *__restrict__ 
     }
 }
 
+// ---- blocked, staggered copies of the model (n even) -----------------------------------------
+// A sample reads the 2x2x2 voxels at its base corner b.  In the plain [n][n][n] layout these are 8
+// gathers on 4 different cache lines.  Here the model is re-laid as 8 copies, one per parity
+// (b_x&1, b_y&1, b_z&1) of the base; copy c holds, for every base of that parity, the 8 corner values
+// as one aligned 32-byte block (corner order 4*dx + 2*dy + dz), blocks ordered [b_x/2][b_y/2][b_z/2].
+// One sample = two 16-byte loads from one sector-aligned block; z-adjacent bases share a cache line.
+// Cost: 32 G bytes written once per iteration (8 MB at 64^3), L2-resident up to n = 128.
+__global__ void __launch_bounds__(256)
+build_blocked_kernel(const float *__restrict__ model, int n, float4 *__restrict__ blocked) {
+    const int h = n >> 1;
+    const size_t per_copy = (size_t)h * h * h;
+    const size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (t >= 8 * per_copy) return;
+    const int c = (int)(t / per_copy);
+    size_t i = t - (size_t)c * per_copy;
+    const int bk = 2 * (int)(i % h) + (c & 1);
+    i /= h;
+    const int bj = 2 * (int)(i % h) + ((c >> 1) & 1);
+    const int bi = 2 * (int)(i / h) + ((c >> 2) & 1);
+    float v[8];
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        const int x = bi + (d >> 2), y = bj + ((d >> 1) & 1), z = bk + (d & 1);
+        v[d] = (x < n && y < n && z < n) ? model[((size_t)x * n + y) * n + z] : 0.f;
+    }
+    blocked[2 * t] = make_float4(v[0], v[1], v[2], v[3]);
+    blocked[2 * t + 1] = make_float4(v[4], v[5], v[6], v[7]);
+}
+
+__global__ void __launch_bounds__(kThreads)
+expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float *__restrict__ q,
+                      const uint8_t *__restrict__ mask, int n_pix, const float *__restrict__ quat,
+                      float *__restrict__ W, int32_t *__restrict__ idx, __half *__restrict__ planes, int ld_p,
+                      size_t plane_stride, float *__restrict__ S) {
+    __shared__ float rm[9];
+    __shared__ float red[kThreads / 32];
+    const int r = blockIdx.x;
+    if (threadIdx.x == 0) {
+        RotMat m = rotation_matrix(quat + 4 * (size_t)r);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
+    }
+    __syncthreads();
+    const unsigned h = (unsigned)n >> 1;
+    const unsigned per_copy = h * h * h;                    // 8 * per_copy <= 2^30 for n <= 1024
+    float part = 0.f;
+#pragma unroll
+    for (int j = 0; j < kPixPerThread; ++j) {
+        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
+        if (p >= n_pix) continue;
+        const Sample s = locate(rm, q[3 * p], q[3 * p + 1], q[3 * p + 2], n);
+        float w = 0.f;
+        if (s.base >= 0) {
+            const unsigned c = ((s.bx & 1u) << 2) | ((s.by & 1u) << 1) | (s.bz & 1u);
+            const unsigned blk = c * per_copy + (((unsigned)s.bx >> 1) * h + ((unsigned)s.by >> 1)) * h + ((unsigned)s.bz >> 1);
+            const float4 *bp = blocked + 2 * (size_t)blk;
+            const float4 lo4 = __ldg(bp), hi4 = __ldg(bp + 1);
+            const float z0 = 1.f - s.tz, y0 = 1.f - s.ty, x0 = 1.f - s.tx;
+            const float c00 = lo4.x * z0 + lo4.y * s.tz;
+            const float c01 = lo4.z * z0 + lo4.w * s.tz;
+            const float c10 = hi4.x * z0 + hi4.y * s.tz;
+            const float c11 = hi4.z * z0 + hi4.w * s.tz;
+            w = (c00 * y0 + c01 * s.ty) * x0 + (c10 * y0 + c11 * s.ty) * s.tx;
+        }
+        const size_t o = (size_t)r * n_pix + p;
+        if (W) W[o] = w;
+        if (idx) idx[o] = s.base;
+        const bool use = mask ? (mask[p] != 0) : true;
+        if (planes) {
+            __half hi, lo;
+            split_logw(w, use && s.base >= 0, hi, lo);
+            const size_t po = (size_t)r * ld_p + p;
+            planes[po] = hi;
+            planes[plane_stride + po] = lo;
+        }
+        if (use) part += w;
+    }
+    if (S) {
+        const float t = block_sum(part, red);
+        if (threadIdx.x == 0) atomicAdd(S + r, t);
+    }
+}
+
 __global__ void __launch_bounds__(kThreads)
 logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
                   const uint8_t *__restrict__ mask, int n_pix, __half *__restrict__ planes, int ld_p,
@@ -117,10 +200,21 @@ logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
 
 }  // namespace
 
+size_t expand_scratch_floats(int n) { return (n & 1) ? 0 : (size_t)8 * n * n * n; }
+
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, cudaStream_t st) {
+                         int ld_p, float *S, float *blocked, cudaStream_t st) {
     dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+    if (blocked && (n & 1) == 0) {
+        const size_t blocks = (size_t)n * n * n;              // 8 copies x (n/2)^3 blocks
+        build_blocked_kernel<<<(unsigned)((blocks + 255) / 256), 256, 0, st>>>(model, n, (float4 *)blocked);
+        EMC_LAUNCHED();
+        expand_blocked_kernel<<<grid, kThreads, 0, st>>>((const float4 *)blocked, n, q, mask, n_pix, quat, W, idx,
+                                                         planes, ld_p, (size_t)n_rot * ld_p, S);
+        EMC_LAUNCHED();
+        return EMC_OK;
+    }
     expand_kernel<<<grid, kThreads, 0, st>>>(model, n, q, mask, n_pix, quat, W, idx, planes, ld_p,
                                              (size_t)n_rot * ld_p, S);
     EMC_LAUNCHED();

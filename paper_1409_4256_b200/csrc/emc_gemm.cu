@@ -54,6 +54,7 @@ struct GemmArgs {
     int epilogue;
     int vec_ok;          // out rows are 16-byte aligned
     int k_chunk;         // k-blocks per TMEM accumulation chunk
+    const float *chunk_scale;   // [num_chunks][M] factor applied to a chunk when it is drained, or null
     uint32_t idesc;
 };
 
@@ -261,7 +262,10 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             float racc[CW];
 #pragma unroll
             for (int j = 0; j < CW; ++j) racc[j] = 0.f;
+            const int m = m_blk * BLOCK_M + quarter * 32 + lane;
             for (int ch = 0; ch < num_chunks; ++ch) {
+                // per-(row, chunk) power-of-two factor of the scaled fp16 planes (exact); loaded before the wait
+                const float sc = (args.chunk_scale && m < args.M) ? args.chunk_scale[(size_t)ch * args.M + m] : 1.f;
                 mbar_wait(tfull_bar + 8 * acc, acc_phase);
                 tc_fence_after();
                 const uint32_t t_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * CW);
@@ -270,14 +274,13 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                     uint32_t v[32];
                     tmem_ld32(t_addr + (uint32_t)c, v);
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) racc[c + j] += __uint_as_float(v[j]);
+                    for (int j = 0; j < 32; ++j) racc[c + j] = fmaf(__uint_as_float(v[j]), sc, racc[c + j]);
                 }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tempty_bar + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
-            const int m = m_blk * BLOCK_M + quarter * 32 + lane;
             if (m < args.M) {
                 const float rv = args.rowv ? args.rowv[m] : 0.f;
                 float *orow = args.out + (size_t)m * args.ld_out;
@@ -334,10 +337,15 @@ __global__ void simt_plane_gemm_kernel(GemmProblem g) {
     const int m = blockIdx.y;
     if (n >= g.N || m >= g.M) return;
     float acc = 0.f;
-    for (int pl = 0; pl < g.n_planes; ++pl)
-        for (int k = 0; k < g.K; ++k)
-            acc += load16(g.A, pl * g.plane_stride + (size_t)m * g.lda + k, g.a_fmt) *
-                   load16(g.B, (size_t)n * g.ldb + k, g.b_fmt);
+    const int chunk = kChunkKBlocks * BLOCK_K;
+    for (int k0 = 0; k0 < g.K; k0 += chunk) {
+        float part = 0.f;
+        for (int pl = 0; pl < g.n_planes; ++pl)
+            for (int k = k0; k < min(g.K, k0 + chunk); ++k)
+                part += load16(g.A, pl * g.plane_stride + (size_t)m * g.lda + k, g.a_fmt) *
+                        load16(g.B, (size_t)n * g.ldb + k, g.b_fmt);
+        acc += part * (g.chunk_scale ? g.chunk_scale[(size_t)(k0 / chunk) * g.M + m] : 1.f);
+    }
     float *o = g.out + (size_t)m * g.ld_out + n;
     const float rv = g.rowv ? g.rowv[m] : 0.f;
     switch (g.epilogue) {
@@ -414,6 +422,7 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     a.num_k_blocks = ceil_div(g.K, BLOCK_K);
     a.out = g.out; a.ld_out = g.ld_out; a.rowv = g.rowv; a.epilogue = g.epilogue;
     a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
+    a.chunk_scale = g.chunk_scale;
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
     // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
     // N >> 3 in [17,23); M >> 4 in [24,29)
@@ -443,7 +452,13 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         EMC_LAUNCHED();
         return EMC_OK;
     }
-    if (g.n_planes == 2) return launch_tc<2, 256, 3>(g, st);
+    if (g.n_planes == 2) {
+        // tile width by wave quantisation: time ~ waves(BN) x BN (one CTA per SM, tiles of equal cost)
+        const int mt = ceil_div(g.M, BLOCK_M), sms = num_sms();
+        const long c256 = (long)ceil_div(mt * ceil_div(g.N, 256), sms) * 256;
+        const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), sms) * 192;
+        return c192 < c256 ? launch_tc<2, 192, 4>(g, st) : launch_tc<2, 256, 3>(g, st);
+    }
     if (g.n_planes == 3) return launch_tc<3, 192, 3>(g, st);
     return EMC_ERR_UNSUPPORTED;
 }

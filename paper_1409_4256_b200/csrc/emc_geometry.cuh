@@ -32,7 +32,8 @@ __device__ __forceinline__ RotMat rotation_matrix(const float *__restrict__ quat
 }
 
 struct Sample {
-    int base;        // linear index of the base corner, -1 outside the grid
+    int base;          // linear index of the base corner, -1 outside the grid
+    int bx, by, bz;    // the base corner itself (meaningful when base >= 0)
     float tx, ty, tz;  // fractional offsets in [0,1)
 };
 
@@ -56,7 +57,10 @@ __device__ __forceinline__ Sample locate(const float *__restrict__ m, float qx, 
     s.ty = __fsub_rn(x[1], by);
     s.tz = __fsub_rn(x[2], bz);
     const bool valid = (bx >= 0.f) && (bx <= hi) && (by >= 0.f) && (by <= hi) && (bz >= 0.f) && (bz <= hi);
-    s.base = valid ? ((int)bx * n + (int)by) * n + (int)bz : -1;
+    s.bx = (int)bx;
+    s.by = (int)by;
+    s.bz = (int)bz;
+    s.base = valid ? (s.bx * n + s.by) * n + s.bz : -1;
     return s;
 }
 

@@ -66,17 +66,19 @@ enum PlaneFormat { FMT_F16 = 0, FMT_BF16 = 1 };   // = the UMMA instruction desc
 // ---------------------------------------------------------------- stage launchers (device work)
 // Expand (emc_expand.cu).  Any of W, idx, planes may be null.  planes = [2][R][ld_p] fp16 (hi, lo)
 // of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).
+// `blocked` = scratch of expand_scratch_floats(n) floats for the blocked model copies, or null (plain gathers).
+size_t expand_scratch_floats(int n);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, cudaStream_t st);
+                         int ld_p, float *S, float *blocked, cudaStream_t st);
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
 
-// Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] bf16
+// Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] fp16 or bf16
 // (row = pixel), masked pixels zeroed, largest unmasked count recorded in hdr->max_count.
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
-                       const uint8_t *mask, __half *Kc, int ld_p, __nv_bfloat16 *KT, int ld_n,
+                       const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
                        WsHeader *hdr, cudaStream_t st);
 
 // Plane GEMM on tcgen05 (emc_gemm.cu):  acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
@@ -92,7 +94,8 @@ struct GemmProblem {
     int ld_out;
     const float *rowv;  // [M] row vector of the epilogue (S for loglik, s for update) or null
     int epilogue;       // EPI_*
-    int k_chunk = 0;    // k-blocks (of 64) per TMEM accumulation chunk, 0 = default
+    int k_chunk = 0;    // k-blocks (of 64) per TMEM accumulation chunk, 0 = default (8 = 512 elements)
+    const float *chunk_scale = nullptr;   // [ceil(K/512)][M] factor applied when a chunk is drained, or null
 };
 enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-likelihood)
        EPI_STORE = 1,       // out = acc                                (raw update numerator)
@@ -100,15 +103,17 @@ enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-lik
        EPI_DIV_ROW = 3 };   // out = rowv[m] > 0 ? acc / rowv[m] : 0    (eq. 2.5)
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st);
 
-// Normalise (emc_normalize.cu).  scratch = 2 * row_splits * ld_n floats.
+// Normalise (emc_normalize.cu).  scratch = normalize_scratch_floats() floats.  `planes` (optional) receives the
+// operand planes of P for the update GEMM: two fp16 planes scaled per (row, 512-column chunk) with the inverse
+// scales in chunk_inv_scale [ceil(ld_n/512)][R], or (bf16x3) three unscaled bf16 planes.
 size_t normalize_scratch_floats(int n_rot, int ld_n);
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
-                            float *P, __nv_bfloat16 *planes, int n_planes, size_t plane_stride,
+                            float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch,
                             cudaStream_t st);
-// bf16 planes of a given P (stage API of emc_update).
-emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __nv_bfloat16 *planes,
-                          int ld_pl, int n_planes, size_t plane_stride, cudaStream_t st);
+// operand planes of a given P (stage API of emc_update).
+emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
+                          size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
 

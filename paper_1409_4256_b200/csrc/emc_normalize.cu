@@ -6,7 +6,7 @@
 //
 // Two sweeps over L (column-wise reductions on a row-major matrix): (1) per-column online
 // (max, sum) in warp-shuffle-free lane-per-column form, split over row ranges for parallelism;
-// (2) write P, its three bf16 planes for the update GEMM, s[r] = sum_d P[r,d] and the total
+// (2) write P, its operand planes for the update GEMM, s[r] = sum_d P[r,d] and the total
 // log-likelihood.  HBM-bound: 8 algorithmic bytes per (r,d).
 #include "emc_internal.cuh"
 
@@ -104,126 +104,225 @@ colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, i
     }
 }
 
-// p -> hi + mid (+ lo) bf16 planes, four columns at a time (8-byte stores)
-__device__ __forceinline__ void split4_bf16(const float (&p)[kVec], int n_planes, __nv_bfloat16 *__restrict__ planes,
-                                            size_t plane_stride, size_t o) {
-    float rem[kVec];
-    __nv_bfloat16 h[kVec];
+// ---- operand planes of P for the update contraction -------------------------------------------
+// Default (PLANES_F16_SCALED): two fp16 planes with one power-of-two scale per (row, 512-column
+// chunk): the chunk is scaled so that its largest value lies in [2^14, 2^15), then hi = fp16(v),
+// lo = fp16(v - hi).  The update GEMM accumulates each 512-element K chunk separately and applies
+// the inverse scale when it drains the chunk (exact), so fp16's narrow exponent only has to span
+// one chunk of one row: 22 significand bits for every value within 2^-17 of the chunk maximum and
+// an absolute error below 2^-40 of the chunk maximum for the rest.
+// Opt-in (EMC_UPDATE_BF16X3): three unscaled bf16 planes (24 bits at every magnitude, 3 MMAs).
+constexpr int kChunkCols = 512;               // = the GEMM's K chunk (kChunkKBlocks * 64)
+constexpr int kGroups = kChunkCols / kColsPerBlock;   // float4 groups per lane per row
+
+__device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
-    for (int j = 0; j < kVec; ++j) { h[j] = __float2bfloat16_rn(p[j]); rem[j] = p[j] - __bfloat162float(h[j]); }
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// scale = 2^(14 - floor(log2 mx)) and its inverse; mx = 0 gives 1, 1
+__device__ __forceinline__ void chunk_scale_of(float mx, float &scale, float &inv) {
+    if (mx > 0.f) {
+        const int ex = (int)((__float_as_uint(mx) >> 23) & 0xffu) - 127;      // mx >= 2^-100: normal
+        scale = __uint_as_float((uint32_t)(14 - ex + 127) << 23);
+        inv = __uint_as_float((uint32_t)(ex - 14 + 127) << 23);
+    } else {
+        scale = 1.f;
+        inv = 1.f;
+    }
+}
+
+__device__ __forceinline__ void store4_f16_pair(const float (&v)[4], __half *__restrict__ planes, size_t plane_stride,
+                                                size_t o) {
+    __half h[4], l[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        h[j] = __float2half_rn(v[j]);
+        l[j] = __float2half_rn(v[j] - __half2float(h[j]));
+    }
+    *reinterpret_cast<uint2 *>(planes + o) = *reinterpret_cast<const uint2 *>(h);
+    *reinterpret_cast<uint2 *>(planes + plane_stride + o) = *reinterpret_cast<const uint2 *>(l);
+}
+
+__device__ __forceinline__ void store4_bf16_x3(const float (&p)[4], __nv_bfloat16 *__restrict__ planes,
+                                               size_t plane_stride, size_t o) {
+    float rem[4];
+    __nv_bfloat16 h[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { h[j] = __float2bfloat16_rn(p[j]); rem[j] = p[j] - __bfloat162float(h[j]); }
     *reinterpret_cast<uint2 *>(planes + o) = *reinterpret_cast<const uint2 *>(h);
 #pragma unroll
-    for (int j = 0; j < kVec; ++j) { h[j] = __float2bfloat16_rn(rem[j]); rem[j] -= __bfloat162float(h[j]); }
+    for (int j = 0; j < 4; ++j) { h[j] = __float2bfloat16_rn(rem[j]); rem[j] -= __bfloat162float(h[j]); }
     *reinterpret_cast<uint2 *>(planes + plane_stride + o) = *reinterpret_cast<const uint2 *>(h);
-    if (n_planes > 2) {
 #pragma unroll
-        for (int j = 0; j < kVec; ++j) h[j] = __float2bfloat16_rn(rem[j]);
-        *reinterpret_cast<uint2 *>(planes + 2 * plane_stride + o) = *reinterpret_cast<const uint2 *>(h);
+    for (int j = 0; j < 4; ++j) h[j] = __float2bfloat16_rn(rem[j]);
+    *reinterpret_cast<uint2 *>(planes + 2 * plane_stride + o) = *reinterpret_cast<const uint2 *>(h);
+}
+
+// One row x one 512-column chunk held by a warp (p[g][4] = columns d0 + g*128 + lane*4 ..+3): writes the
+// operand planes and, for the scaled format, the chunk's inverse scale.
+__device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int lane, int ld_pl, size_t row_off,
+                                             void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                                             float *__restrict__ inv_scale_out) {
+    if (bf16x3) {
+#pragma unroll
+        for (int g = 0; g < kGroups; ++g) {
+            const int d = d0 + g * kColsPerBlock + lane * kVec;
+            if (d < ld_pl) store4_bf16_x3(p[g], (__nv_bfloat16 *)planes, plane_stride, row_off + d);
+        }
+        return;
+    }
+    float mx = 0.f;
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g)
+        mx = fmaxf(mx, fmaxf(fmaxf(p[g][0], p[g][1]), fmaxf(p[g][2], p[g][3])));
+    mx = warp_max(mx);
+    float scale, inv;
+    chunk_scale_of(mx, scale, inv);
+    if (lane == 0) *inv_scale_out = inv;
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g) {
+        const int d = d0 + g * kColsPerBlock + lane * kVec;
+        if (d < ld_pl) {
+            const float v[4] = {p[g][0] * scale, p[g][1] * scale, p[g][2] * scale, p[g][3] * scale};
+            store4_f16_pair(v, (__half *)planes, plane_stride, row_off + d);
+        }
     }
 }
 
-__device__ __forceinline__ void split_bf16(float p, int n_planes, __nv_bfloat16 *__restrict__ planes,
-                                           size_t plane_stride, size_t o) {
-    const __nv_bfloat16 h = __float2bfloat16_rn(p);
-    planes[o] = h;
-    float rem = p - __bfloat162float(h);
-    const __nv_bfloat16 m = __float2bfloat16_rn(rem);
-    planes[plane_stride + o] = m;
-    if (n_planes > 2) {
-        rem -= __bfloat162float(m);
-        planes[2 * plane_stride + o] = __float2bfloat16_rn(rem);
+// between the sweeps: per column, combine the split partials into (max, 1/sum) and add up the total
+// log-likelihood  LL = sum_d (m_d + log z_d).
+__global__ void __launch_bounds__(256)
+colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_z, int n_pat, int ld_n,
+                        int n_splits, float *__restrict__ col_m, float *__restrict__ col_iz,
+                        double *__restrict__ loglik) {
+    const int d = blockIdx.x * 256 + threadIdx.x;
+    double ll = 0.0;
+    if (d < n_pat) {
+        float mt = -INFINITY, zt = 0.f;
+        for (int k = 0; k < n_splits; ++k) mt = fmaxf(mt, part_m[(size_t)k * ld_n + d]);
+        for (int k = 0; k < n_splits; ++k) {
+            const float zk = part_z[(size_t)k * ld_n + d];
+            if (zk > 0.f) zt += zk * expf(part_m[(size_t)k * ld_n + d] - mt);
+        }
+        col_m[d] = mt;
+        col_iz[d] = 1.f / zt;
+        ll = (double)mt + (double)logf(zt);
+    } else if (d < ld_n) {
+        col_m[d] = 0.f;
+        col_iz[d] = 0.f;
+    }
+    if (loglik) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ll += __shfl_xor_sync(0xffffffffu, ll, o);
+        __shared__ double red[8];
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ll;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int w = 0; w < 8; ++w) t += red[w];
+            atomicAdd(loglik, t);
+        }
     }
 }
 
-// sweep 2: combine the partials, write P / planes / s / LL
+// sweep 2: write P / planes / s.  grid = (ceil(N/512), row splits); a warp owns one row x 512 columns at a
+// time and prefetches the next row while it works on the current one.
 __global__ void __launch_bounds__(kThreads)
 normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
-                 int ld_n, int rows_per_split, int n_splits, const float *__restrict__ part_m,
-                 const float *__restrict__ part_z, float *__restrict__ P,
-                 __nv_bfloat16 *__restrict__ planes, int n_planes, size_t plane_stride,
-                 float *__restrict__ s, double *__restrict__ loglik) {
+                 int ld_n, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_iz,
+                 float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                 float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int d = blockIdx.x * kColsPerBlock + lane * kVec;
+    const int d0 = blockIdx.x * kChunkCols;
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
     const float log_uniform = -logf((float)n_rot);
-    const bool col_ok = d < n_pat;
-    // every warp combines the split partials of its own 4 columns (L2-resident, n_splits <= 64)
-    float mt[kVec], iz[kVec];
-    double ll = 0.0;
+    float4 mt[kGroups], iz[kGroups];
+    bool ok[kGroups];
 #pragma unroll
-    for (int j = 0; j < kVec; ++j) { mt[j] = -INFINITY; iz[j] = 0.f; }
-    if (col_ok) {
-        float zt[kVec] = {0.f, 0.f, 0.f, 0.f};
-        for (int k = 0; k < n_splits; ++k) {
-            const float4 a = *reinterpret_cast<const float4 *>(part_m + (size_t)k * ld_n + d);
-            mt[0] = fmaxf(mt[0], a.x); mt[1] = fmaxf(mt[1], a.y); mt[2] = fmaxf(mt[2], a.z); mt[3] = fmaxf(mt[3], a.w);
-        }
-        for (int k = 0; k < n_splits; ++k) {
-            const float4 a = *reinterpret_cast<const float4 *>(part_m + (size_t)k * ld_n + d);
-            const float4 b = *reinterpret_cast<const float4 *>(part_z + (size_t)k * ld_n + d);
-            if (b.x > 0.f) zt[0] += b.x * expf(a.x - mt[0]);
-            if (b.y > 0.f) zt[1] += b.y * expf(a.y - mt[1]);
-            if (b.z > 0.f) zt[2] += b.z * expf(a.z - mt[2]);
-            if (b.w > 0.f) zt[3] += b.w * expf(a.w - mt[3]);
-        }
-#pragma unroll
-        for (int j = 0; j < kVec; ++j) {
-            iz[j] = 1.f / zt[j];
-            if (d + j < n_pat) ll += (double)mt[j] + (double)logf(zt[j]);
-        }
+    for (int g = 0; g < kGroups; ++g) {
+        const int d = d0 + g * kColsPerBlock + lane * kVec;
+        ok[g] = d < n_pat;                              // col_m / col_iz are defined (0) up to ld_n
+        mt[g] = ok[g] ? *reinterpret_cast<const float4 *>(col_m + d) : make_float4(0.f, 0.f, 0.f, 0.f);
+        iz[g] = ok[g] ? *reinterpret_cast<const float4 *>(col_iz + d) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    if (loglik && blockIdx.y == 0 && warp == 0) {
+    float4 nxt[kGroups];
+    int r = r_lo + warp;
+    if (r < r_hi) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) ll += __shfl_xor_sync(0xffffffffu, ll, o);
-        if (lane == 0) atomicAdd(loglik, ll);
+        for (int g = 0; g < kGroups; ++g)
+            if (ok[g]) nxt[g] = *reinterpret_cast<const float4 *>(L + (size_t)r * ld_n + d0 + g * kColsPerBlock + lane * kVec);
     }
-    for (int r0 = r_lo + warp; r0 < r_hi; r0 += kWarps * kBatch) {
-        float4 v[kBatch];
-        float lw[kBatch];
+    for (; r < r_hi; r += kWarps) {
+        float4 v[kGroups];
 #pragma unroll
-        for (int b = 0; b < kBatch; ++b) {
-            const int r = r0 + b * kWarps;
-            if (r < r_hi && col_ok) {
-                v[b] = *reinterpret_cast<const float4 *>(L + (size_t)r * ld_n + d);
-                lw[b] = log_weight(weight, r, log_uniform);
-            }
+        for (int g = 0; g < kGroups; ++g) v[g] = nxt[g];
+        if (r + kWarps < r_hi) {
+#pragma unroll
+            for (int g = 0; g < kGroups; ++g)
+                if (ok[g])
+                    nxt[g] = *reinterpret_cast<const float4 *>(L + (size_t)(r + kWarps) * ld_n + d0 + g * kColsPerBlock + lane * kVec);
         }
+        const float lw = log_weight(weight, r, log_uniform);
+        const size_t row_off = (size_t)r * ld_n;
+        float p[kGroups][4];
+        float sum = 0.f;
 #pragma unroll
-        for (int b = 0; b < kBatch; ++b) {
-            const int r = r0 + b * kWarps;
-            if (r >= r_hi) break;                       // warp-uniform
-            float p[kVec] = {0.f, 0.f, 0.f, 0.f};
-            if (col_ok) {
-                const float a[kVec] = {v[b].x + lw[b], v[b].y + lw[b], v[b].z + lw[b], v[b].w + lw[b]};
+        for (int g = 0; g < kGroups; ++g) {
+            const int d = d0 + g * kColsPerBlock + lane * kVec;
+            const float a[4] = {v[g].x + lw, v[g].y + lw, v[g].z + lw, v[g].w + lw};
+            const float m4[4] = {mt[g].x, mt[g].y, mt[g].z, mt[g].w};
+            const float z4[4] = {iz[g].x, iz[g].y, iz[g].z, iz[g].w};
 #pragma unroll
-                for (int j = 0; j < kVec; ++j) {
-                    float pj = expf(a[j] - mt[j]) * iz[j];
-                    if (pj < EMC_P_MIN || d + j >= n_pat) pj = 0.f;      // DESIGN.md §3 G20
-                    p[j] = pj;
+            for (int j = 0; j < 4; ++j) {
+                float pj = 0.f;
+                if (d + j < n_pat) {
+                    pj = expf(a[j] - m4[j]) * z4[j];
+                    if (pj < EMC_P_MIN) pj = 0.f;                      // DESIGN.md §3 G20
                 }
-                const size_t o = (size_t)r * ld_n + d;
-                if (P) *reinterpret_cast<float4 *>(P + o) = make_float4(p[0], p[1], p[2], p[3]);
-                if (planes) split4_bf16(p, n_planes, planes, plane_stride, o);
+                p[g][j] = pj;
+                sum += pj;
             }
-            if (s) {
-                float t = (p[0] + p[1]) + (p[2] + p[3]);
-#pragma unroll
-                for (int off = 16; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
-                if (lane == 0) atomicAdd(s + r, t);
-            }
+            if (P && ok[g]) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
+        }
+        if (planes)
+            write_planes(p, d0, lane, ld_n, row_off, planes, bf16x3, plane_stride,
+                         chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
+        if (s) {
+            sum = warp_sum(sum);
+            if (lane == 0) atomicAdd(s + r, sum);
         }
     }
 }
 
-__global__ void __launch_bounds__(256)
-p_split_kernel(const float *__restrict__ P, int n_pat, int ld_n, __nv_bfloat16 *__restrict__ planes,
-               int ld_pl, int n_planes, size_t plane_stride) {
-    const int d = blockIdx.y * 256 + threadIdx.x;
-    if (d >= n_pat) return;
-    float p = P[(size_t)blockIdx.x * ld_n + d];
-    if (p < EMC_P_MIN) p = 0.f;
-    split_bf16(p, n_planes, planes, plane_stride, (size_t)blockIdx.x * ld_pl + d);
+// operand planes of a given P (stage API of emc_update).  grid = (ceil(N/512), ceil(R/8)); warp per row.
+__global__ void __launch_bounds__(kThreads)
+p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, void *__restrict__ planes, int ld_pl,
+               int bf16x3, size_t plane_stride, float *__restrict__ chunk_inv_scale) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int r = blockIdx.y * kWarps + warp;
+    if (r >= n_rot) return;
+    const int d0 = blockIdx.x * kChunkCols;
+    float p[kGroups][4];
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g) {
+        const int d = d0 + g * kColsPerBlock + lane * kVec;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            float pj = (d + j < n_pat) ? P[(size_t)r * ld_n + d + j] : 0.f;
+            if (pj < EMC_P_MIN) pj = 0.f;
+            p[g][j] = pj;
+        }
+    }
+    write_planes(p, d0, lane, ld_pl, (size_t)r * ld_pl, planes, bf16x3, plane_stride,
+                 chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
 }
 
 __global__ void __launch_bounds__(256)
@@ -239,11 +338,11 @@ div_rows_kernel(float *__restrict__ Wn, const float *__restrict__ s, int n_pix) 
 
 size_t normalize_scratch_floats(int n_rot, int ld_n) {
     (void)n_rot;
-    return (size_t)2 * 64 * (size_t)ld_n;
+    return (size_t)(2 * 64 + 2) * (size_t)ld_n;      // split partials (max, sum) + combined (max, 1/sum)
 }
 
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
-                            float *P, __nv_bfloat16 *planes, int n_planes, size_t plane_stride,
+                            float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch,
                             cudaStream_t st) {
     const int col_blocks = ceil_div(n_pat, kColsPerBlock);
@@ -255,19 +354,32 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
         if (s) EMC_TRY_CUDA(cudaMemsetAsync(s, 0, sizeof(float) * n_rot, st));
         if (loglik) EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
     }
-    dim3 grid(col_blocks, n_splits);
-    colstats_kernel<<<grid, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split, part_m, part_z);
+    colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split,
+                                                                     part_m, part_z);
     EMC_LAUNCHED();
-    normalize_kernel<<<grid, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split, n_splits, part_m,
-                                                part_z, P, planes, n_planes, plane_stride, s, loglik);
+    float *col_m = scratch + (size_t)128 * ld_n, *col_iz = col_m + ld_n;
+    colstats_combine_kernel<<<ceil_div(ld_n, 256), 256, 0, st>>>(part_m, part_z, n_pat, ld_n, n_splits, col_m, col_iz,
+                                                                 loglik);
+    EMC_LAUNCHED();
+    // second sweep: 512-column chunks; enough row splits for about six resident blocks per SM
+    const int chunks = ceil_div(n_pat, kChunkCols);
+    int splits2 = ceil_div(6 * 148, chunks);
+    const int cap2 = ceil_div(n_rot, 4 * kWarps);
+    if (splits2 > cap2) splits2 = cap2;
+    if (splits2 < 1) splits2 = 1;
+    const int rows2 = ceil_div(n_rot, splits2);
+    normalize_kernel<<<dim3(chunks, ceil_div(n_rot, rows2)), kThreads, 0, st>>>(
+        L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_iz, P, planes, bf16x3 ? 1 : 0, plane_stride,
+        chunk_inv_scale, s);
     EMC_LAUNCHED();
     return EMC_OK;
 }
 
-emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __nv_bfloat16 *planes,
-                          int ld_pl, int n_planes, size_t plane_stride, cudaStream_t st) {
-    dim3 grid(n_rot, ceil_div(n_pat, 256));
-    p_split_kernel<<<grid, 256, 0, st>>>(P, n_pat, ld_n, planes, ld_pl, n_planes, plane_stride);
+emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
+                          size_t plane_stride, float *chunk_inv_scale, cudaStream_t st) {
+    dim3 grid(ceil_div(n_pat, kChunkCols), ceil_div(n_rot, kWarps));
+    p_split_kernel<<<grid, kThreads, 0, st>>>(P, n_rot, n_pat, ld_n, planes, ld_pl, bf16x3 ? 1 : 0, plane_stride,
+                                              chunk_inv_scale);
     EMC_LAUNCHED();
     return EMC_OK;
 }

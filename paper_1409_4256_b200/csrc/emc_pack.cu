@@ -1,8 +1,9 @@
 // Photon counts K[d][p] -> the exact 16-bit operands of the two contractions:
 //   Kc [N][ld_p] fp16, row = pattern  (B operand of the log-likelihood GEMM, K-dim = pixels)
-//   KT [P][ld_n] bf16, row = pixel    (B operand of the update GEMM,         K-dim = patterns)
-// Masked pixels become 0 in both (G16).  Small integers are exact in fp16 (<= 2048) and bf16
-// (<= 256 = EMC_MAX_COUNT); the largest unmasked count is recorded for emc_check().
+//   KT [P][ld_n] fp16, row = pixel    (B operand of the update GEMM,         K-dim = patterns)
+//      (bf16 for the opt-in bf16x3 update)
+// Masked pixels become 0 in both (G16).  Small integers are exact in fp16 up to 2048 = EMC_MAX_COUNT
+// (bf16: 256); the largest unmasked count is recorded for emc_check().
 #include "emc_internal.cuh"
 
 namespace emc {
@@ -14,7 +15,7 @@ constexpr int kTile = 64;
 template <class T>
 __global__ void __launch_bounds__(256)
 pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *__restrict__ mask,
-            __half *__restrict__ Kc, int ld_p, __nv_bfloat16 *__restrict__ KT, int ld_n,
+            __half *__restrict__ Kc, int ld_p, void *__restrict__ KT, int kt_bf16, int ld_n,
             WsHeader *__restrict__ hdr) {
     __shared__ float tile[kTile][kTile + 1];
     const int p0 = blockIdx.x * kTile, d0 = blockIdx.y * kTile;
@@ -41,32 +42,37 @@ pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *_
 #pragma unroll 4
         for (int j = ty; j < kTile; j += 4) {
             const int p = p0 + j, d = d0 + tx;
-            if (p < n_pix && d < n_pat) KT[(size_t)p * ld_n + d] = __float2bfloat16_rn(tile[tx][j]);
+            if (p < n_pix && d < n_pat) {
+                const size_t o = (size_t)p * ld_n + d;
+                if (kt_bf16) ((__nv_bfloat16 *)KT)[o] = __float2bfloat16_rn(tile[tx][j]);
+                else ((__half *)KT)[o] = __float2half_rn(tile[tx][j]);
+            }
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
-    if ((threadIdx.x & 31) == 0 && vmax > EMC_MAX_COUNT) atomicMax(&hdr->max_count, vmax);
+    if ((threadIdx.x & 31) == 0 && vmax > (kt_bf16 ? 256 : EMC_MAX_COUNT)) atomicMax(&hdr->max_count, vmax);
 }
 
 }  // namespace
 
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
-                       const uint8_t *mask, __half *Kc, int ld_p, __nv_bfloat16 *KT, int ld_n,
+                       const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
                        WsHeader *hdr, cudaStream_t st) {
+    const int fb = kt_bf16 ? 1 : 0;
     dim3 grid(ceil_div(n_pix, kTile), ceil_div(n_pat, kTile));
     switch (type) {
         case EMC_I32:
             pack_kernel<int32_t><<<grid, 256, 0, st>>>((const int32_t *)counts, n_pat, n_pix, mask, Kc,
-                                                       ld_p, KT, ld_n, hdr);
+                                                       ld_p, KT, fb, ld_n, hdr);
             break;
         case EMC_U16:
             pack_kernel<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc,
-                                                        ld_p, KT, ld_n, hdr);
+                                                        ld_p, KT, fb, ld_n, hdr);
             break;
         case EMC_U8:
             pack_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)counts, n_pat, n_pix, mask, Kc,
-                                                       ld_p, KT, ld_n, hdr);
+                                                       ld_p, KT, fb, ld_n, hdr);
             break;
         default:
             return EMC_ERR_ARG;

@@ -23,7 +23,7 @@ def test_header_symbols_all_exported():
 
 def test_header_constants_match_binding():
     header = (ROOT / "include" / "emc.h").read_text()
-    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_PLANES_2", "EMC_DEBUG_SIMT",
+    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_UPDATE_BF16X3", "EMC_DEBUG_SIMT",
                  "EMC_PATTERNS_ON_HOST", "EMC_PROFILE_STAGES", "EMC_MAX_COUNT"):
         m = re.search(rf"#define {name}\s+(0x[0-9a-fA-F]+|\d+)u?", header)
         assert m, name
@@ -52,7 +52,7 @@ def test_workspace_bytes_monotone_and_rejects_bad_sizes():
 
 def test_null_arguments_are_rejected_synchronously():
     lib = emc.load()
-    assert lib.emc_expand(None, None, None, None, None, None) == emc.EMC_ERR_ARG
+    assert lib.emc_expand(None, None, None, None, None, None, 0, None) == emc.EMC_ERR_ARG
     assert lib.emc_check(None, None) == emc.EMC_ERR_ARG
     det = binding._Detector(16, 8, None)
     pat = binding._Patterns(4, 8, emc.binding.EMC_U16)

@@ -25,10 +25,10 @@ def test_update_sum_bias_is_flat_in_k(n_pat):
     pp = torch.zeros((n_rot, emc.ld_for(n_pat)), dtype=torch.float32, device="cuda")
     pp[:, :n_pat] = dev(p)
     q, mask = dev(np.zeros((n_pix, 3), np.float32)), dev(np.ones(n_pix, np.uint8))
-    for flags, name in ((0, "bf16x3"), (emc.EMC_PLANES_2, "bf16x2")):
+    for flags, name in ((0, "fp16x2 scaled"), (emc.EMC_UPDATE_BF16X3, "bf16x3")):
         got = emc.emc_update(pp[:, :n_pat], None, q, mask, dev(k), flags=flags | emc.EMC_UPDATE_RAW).cpu().numpy()
         rel = (got.astype(np.float64) - ref) / ref
-        print(f"update K={n_pat:6d} {name}: mean signed rel {rel.mean():+.3e}  max |rel| {np.abs(rel).max():.3e}")
+        print(f"update K={n_pat:6d} {name:13s}: mean signed rel {rel.mean():+.3e}  max |rel| {np.abs(rel).max():.3e}")
         assert abs(rel.mean()) <= 2e-6 and np.abs(rel).max() <= 4e-6
 
 
