@@ -73,6 +73,8 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
                                       planes (2 MMAs) */
 #define EMC_PROFILE_STAGES    0x20u /* emc_iterate records CUDA events on `stream` around every stage;
                                       read (and reset) the sums with emc_profile_read() */
+#define EMC_GEMM_1CTA         0x200u /* run the two contractions with one CTA per tile (cta_group::1)
+                                        instead of CTA pairs (cta_group::2); a comparison / bisecting aid */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
                                         bisecting aid for the tcgen05 path, never the default) */
 

@@ -25,6 +25,7 @@ EMC_UPDATE_BF16X3 = 0x8
 EMC_PATTERNS_ON_HOST = 0x10
 EMC_PROFILE_STAGES = 0x20
 EMC_DEBUG_SIMT = 0x100
+EMC_GEMM_1CTA = 0x200
 STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)

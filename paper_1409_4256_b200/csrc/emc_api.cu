@@ -117,18 +117,19 @@ emc_status reset_header(const Layout &l, cudaStream_t st) {
 }
 
 emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
-                           bool simt, cudaStream_t st) {
+                           unsigned flags, cudaStream_t st) {
     GemmProblem g;
     g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
     g.M = n_rot; g.N = n_pat; g.K = n_pix;
     g.lda = l.ld_p; g.ldb = l.ld_p; g.plane_stride = (size_t)n_rot * l.ld_p;
     g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
     g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = EPI_SUB_ROW;
-    return launch_plane_gemm(g, simt, st);
+    g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
+    return launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st);
 }
 
 emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, bool bf16x3, float *out,
-                           const float *s, int epilogue, bool simt, cudaStream_t st) {
+                           const float *s, int epilogue, unsigned flags, cudaStream_t st) {
     GemmProblem g;
     g.A = l.planesP; g.B = l.KT; g.n_planes = bf16x3 ? 3 : 2;
     g.M = n_rot; g.N = n_pix; g.K = n_pat;
@@ -136,7 +137,8 @@ emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, boo
     g.a_fmt = g.b_fmt = bf16x3 ? FMT_BF16 : FMT_F16;
     g.chunk_scale = bf16x3 ? nullptr : l.pscale;
     g.out = out; g.ld_out = n_pix; g.rowv = s; g.epilogue = epilogue;
-    return launch_plane_gemm(g, simt, st);
+    g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
+    return launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st);
 }
 
 }  // namespace
@@ -180,7 +182,7 @@ emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *de
     EMC_TRY(launch_logw_split(W, idx, det->mask, det->n_pix, n_rot, l.planesL, l.ld_p, l.S, st));
     EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, false, 0,
                         l.hdr, st));
-    return run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, (flags & EMC_DEBUG_SIMT) != 0, st);
+    return run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, flags, st);
 }
 
 emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
@@ -211,8 +213,7 @@ emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detect
     EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, bf16x3, l.ld_n,
                         l.hdr, st));
     const int epi = (flags & EMC_ACCUMULATE) ? EPI_ADD : (raw ? EPI_STORE : EPI_DIV_ROW);
-    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, bf16x3, Wnew, s, epi,
-                           (flags & EMC_DEBUG_SIMT) != 0, st);
+    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, bf16x3, Wnew, s, epi, flags, st);
 }
 
 emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detector *det,
@@ -244,7 +245,6 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
     const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
     const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
@@ -276,7 +276,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
             // stage 2: L = logW K^T - S
             {
                 Span sp(prof, EMC_STAGE_LOGLIK, st);
-                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, simt, st));
+                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st));
             }
             // stage 3: responsibilities of this chunk; s and LL add up over chunks
             float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
@@ -289,7 +289,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
             const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
             {
                 Span sp(prof, EMC_STAGE_UPDATE, st);
-                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, simt, st));
+                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, flags, st));
             }
         }
         if (n_chunks > 1) {

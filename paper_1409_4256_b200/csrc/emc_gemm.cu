@@ -144,6 +144,42 @@ __device__ __forceinline__ void tile_coords(int tile, const GemmArgs &a, int &m_
     n_blk = t / gm;
 }
 
+// Fused row operation + store of one accumulator row (CW columns starting at column n_base).
+template <int CW>
+__device__ __forceinline__ void store_row(const float (&racc)[CW], const GemmArgs &args, int m, int n_base, float rv) {
+    float *orow = args.out + (size_t)m * args.ld_out;
+#pragma unroll
+    for (int c = 0; c < CW; c += 4) {
+        const int n0 = n_base + c;
+        if (n0 >= args.N) break;
+        float f[4] = {racc[c], racc[c + 1], racc[c + 2], racc[c + 3]};
+        if (args.epilogue == EPI_SUB_ROW) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) f[j] -= rv;
+        } else if (args.epilogue == EPI_DIV_ROW) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) f[j] = rv > 0.f ? f[j] / rv : 0.f;
+        }
+        float *o = orow + n0;
+        if (args.vec_ok && n0 + 4 <= args.N) {
+            float4 *o4 = reinterpret_cast<float4 *>(o);
+            if (args.epilogue == EPI_ADD) {
+                float4 t = *o4;
+                f[0] += t.x; f[1] += t.y; f[2] += t.z; f[3] += t.w;
+            }
+            *o4 = make_float4(f[0], f[1], f[2], f[3]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (n0 + j < args.N) {
+                    if (args.epilogue == EPI_ADD) o[j] += f[j];
+                    else o[j] = f[j];
+                }
+            }
+        }
+    }
+}
+
 template <int NP, int BN, int STAGES>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
@@ -283,37 +319,7 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             }
             if (m < args.M) {
                 const float rv = args.rowv ? args.rowv[m] : 0.f;
-                float *orow = args.out + (size_t)m * args.ld_out;
-#pragma unroll
-                for (int c = 0; c < CW; c += 4) {
-                    const int n0 = n_blk * BN + half * CW + c;
-                    if (n0 >= args.N) break;
-                    float f[4] = {racc[c], racc[c + 1], racc[c + 2], racc[c + 3]};
-                    if (args.epilogue == EPI_SUB_ROW) {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) f[j] -= rv;
-                    } else if (args.epilogue == EPI_DIV_ROW) {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) f[j] = rv > 0.f ? f[j] / rv : 0.f;
-                    }
-                    float *o = orow + n0;
-                    if (args.vec_ok && n0 + 4 <= args.N) {
-                        float4 *o4 = reinterpret_cast<float4 *>(o);
-                        if (args.epilogue == EPI_ADD) {
-                            float4 t = *o4;
-                            f[0] += t.x; f[1] += t.y; f[2] += t.z; f[3] += t.w;
-                        }
-                        *o4 = make_float4(f[0], f[1], f[2], f[3]);
-                    } else {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            if (n0 + j < args.N) {
-                                if (args.epilogue == EPI_ADD) o[j] += f[j];
-                                else o[j] = f[j];
-                            }
-                        }
-                    }
-                }
+                store_row<CW>(racc, args, m, n_blk * BN + half * CW, rv);
             }
         }
     }
@@ -323,6 +329,244 @@ plane_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// ------------------------------------------------------------------ CTA-pair version (cta_group::2)
+// The one-CTA kernel above is bound by the L2 -> shared-memory feed, not by the tensor pipe: a
+// 128 x 256 tile with two A planes pulls 64 KB per k-block of 1024 MMA cycles = 64 B/clk/SM, and
+// the chip delivers about 6300 B/clk in all = 43 B/clk/SM (B300_MICROARCH.md "TMA chip-throughput").
+// Here two CTAs of a cluster (the two SMs of a TPC) share one 256 x BN tile: each loads its own 128
+// rows of the A planes and HALF of the B tile, and one tcgen05.mma.cta_group::2 (M = 256) issued by
+// the leader CTA reads both halves of B, so the feed drops to 48 B/clk/SM for BN = 256.
+// Same roles, same K-chunked TMEM accumulation; what changes is the synchronisation:
+//   full[s]    lives in the leader; the TMA of BOTH CTAs signals it (.cta_group::2, peer bit cleared)
+//   empty[s]   one per CTA, released by a multicast tcgen05.commit from the leader
+//   tfull[a]   one per CTA, same multicast commit
+//   tempty[a]  lives in the leader, counts the epilogue warps of both CTAs (remote arrive)
+constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;      // shared::cluster address of the same offset in the even CTA
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_id_x() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t num_clusters_x() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_2d_2sm(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar & kPeerBitMask), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_2sm(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar & kPeerBitMask), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void umma_f16_2sm(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrives on the barrier at this offset in BOTH CTAs once every MMA issued so far has completed
+__device__ __forceinline__ void umma_commit_2sm(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_leader(uint32_t bar) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar & kPeerBitMask) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_2sm(uint32_t dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_2sm(uint32_t addr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+}
+
+constexpr int PAIR_M = 2 * BLOCK_M;            // rows of a pair tile
+constexpr int kGroupPairM = 4;                 // rasterisation: 4 pair-rows (1024 rows) share each n sweep
+
+template <int NP, int BN, int STAGES>
+struct Cfg2 {
+    static constexpr int HB = BN / 2;                                 // B rows held by each CTA
+    static constexpr int B_BYTES = HB * BLOCK_K * 2;
+    static constexpr int STAGE_BYTES = NP * A_PLANE_BYTES + B_BYTES;  // per CTA
+    static constexpr int BAR_BYTES = 256;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;
+    static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory per CTA");
+    static_assert(2 * BN <= 512, "two accumulator stages must fit the 512 TMEM columns");
+    static_assert(BN % 64 == 0 && BN <= 256, "UMMA N for M = 256; two epilogue warps per lane quarter");
+    static_assert(HB % 8 == 0, "whole swizzle atoms");
+};
+
+__device__ __forceinline__ void pair_tile_coords(int tile, const GemmArgs &a, int &m_blk, int &n_blk) {
+    const int per_group = kGroupPairM * a.num_n_tiles;
+    const int group = tile / per_group;
+    const int first_m = group * kGroupPairM;
+    const int gm = min(a.num_m_tiles - first_m, kGroupPairM);
+    const int t = tile - group * per_group;
+    m_blk = first_m + t % gm;
+    n_blk = t / gm;
+}
+
+// args.num_m_tiles counts PAIR tiles (256 rows)
+template <int NP, int BN, int STAGES>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
+plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                       const GemmArgs args) {
+    using C = Cfg2<NP, BN, STAGES>;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + STAGES * C::STAGE_BYTES;
+    const uint32_t full_bar = bar_base, empty_bar = bar_base + 8 * STAGES;
+    const uint32_t tfull_bar = bar_base + 16 * STAGES, tempty_bar = tfull_bar + 16;
+    const uint32_t tmem_slot = tempty_bar + 16;
+    uint32_t *tmem_slot_ptr = (uint32_t *)(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const bool leader = rank == 0;
+    const int num_tiles = args.num_m_tiles * args.num_n_tiles;
+    const int first_tile = (int)cluster_id_x(), tile_step = (int)num_clusters_x();
+    const int num_chunks = (args.num_k_blocks + args.k_chunk - 1) / args.k_chunk;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar + 8 * s, 1);
+            mbar_init(empty_bar + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(tfull_bar + 8 * a, 1);
+            mbar_init(tempty_bar + 8 * a, 2 * kNumEpiWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc_2sm(tmem_slot, 512);
+    tc_fence_before();
+    cluster_sync_all();                           // both CTAs' barriers exist before anyone signals them
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ================= TMA producer (both CTAs) =================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+                int m_blk, n_blk;
+                pair_tile_coords(tile, args, m_blk, n_blk);
+                const int m0 = m_blk * PAIR_M + (int)rank * BLOCK_M;
+                const int n0 = n_blk * BN + (int)rank * C::HB;
+                for (int kb = 0; kb < args.num_k_blocks; ++kb) {
+                    mbar_wait(empty_bar + 8 * stage, phase ^ 1u);
+                    const uint32_t fb = full_bar + 8 * stage;
+                    if (leader) mbar_expect_tx(fb, 2 * C::STAGE_BYTES);   // the bytes of both CTAs
+                    const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
+#pragma unroll
+                    for (int pl = 0; pl < NP; ++pl)
+                        tma_load_3d_2sm(sa + pl * A_PLANE_BYTES, &tmA, fb, kb * BLOCK_K, m0, pl);
+                    tma_load_2d_2sm(sa + NP * A_PLANE_BYTES, &tmB, fb, kb * BLOCK_K, n0);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (leader CTA only) =================
+        if (leader && lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc = 0;
+            uint32_t acc_phase = 0;
+            for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+                for (int ch = 0; ch < num_chunks; ++ch) {
+                    mbar_wait(tempty_bar + 8 * acc, acc_phase ^ 1u);     // both epilogues have drained this stage
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+                    const int kb_end = min(args.num_k_blocks, (ch + 1) * args.k_chunk);
+                    for (int kb = ch * args.k_chunk; kb < kb_end; ++kb) {
+                        mbar_wait(full_bar + 8 * stage, phase);
+                        tc_fence_after();
+                        const uint32_t sa = smem_base + stage * C::STAGE_BYTES;
+                        const uint64_t bdesc0 = umma_desc_sw128(sa + NP * A_PLANE_BYTES);
+                        const uint32_t first = (kb == ch * args.k_chunk) ? 0u : 1u;
+#pragma unroll
+                        for (int pl = 0; pl < NP; ++pl) {
+                            const uint64_t adesc0 = umma_desc_sw128(sa + pl * A_PLANE_BYTES);
+#pragma unroll
+                            for (int k = 0; k < BLOCK_K / UMMA_K; ++k)
+                                umma_f16_2sm(d_tmem, adesc0 + (uint64_t)(2 * k), bdesc0 + (uint64_t)(2 * k), args.idesc,
+                                             (pl | k) != 0 ? 1u : first);
+                        }
+                        umma_commit_2sm(empty_bar + 8 * stage);          // frees the slot in both CTAs
+                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    }
+                    umma_commit_2sm(tfull_bar + 8 * acc);                // partial sums complete in both CTAs
+                    if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+                }
+            }
+        }
+    } else {
+        // ================= epilogue warps 2..9 (both CTAs; each drains its own 128 rows) =================
+        constexpr int CW = BN / 2;
+        const int quarter = warp & 3;
+        const int half = (warp - 2) >> 2;
+        int acc = 0;
+        uint32_t acc_phase = 0;
+        for (int tile = first_tile; tile < num_tiles; tile += tile_step) {
+            int m_blk, n_blk;
+            pair_tile_coords(tile, args, m_blk, n_blk);
+            float racc[CW];
+#pragma unroll
+            for (int j = 0; j < CW; ++j) racc[j] = 0.f;
+            const int m = m_blk * PAIR_M + (int)rank * BLOCK_M + quarter * 32 + lane;
+            for (int ch = 0; ch < num_chunks; ++ch) {
+                const float sc = (args.chunk_scale && m < args.M) ? args.chunk_scale[(size_t)ch * args.M + m] : 1.f;
+                mbar_wait(tfull_bar + 8 * acc, acc_phase);
+                tc_fence_after();
+                const uint32_t t_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * CW);
+#pragma unroll
+                for (int c = 0; c < CW; c += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(t_addr + (uint32_t)c, v);
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) racc[c + j] = fmaf(__uint_as_float(v[j]), sc, racc[c + j]);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_leader(tempty_bar + 8 * acc);
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+            if (m < args.M) {
+                const float rv = args.rowv ? args.rowv[m] : 0.f;
+                store_row<CW>(racc, args, m, n_blk * BN + half * CW, rv);
+            }
+        }
+    }
+
+    tc_fence_before();
+    cluster_sync_all();                           // the peer may still be reading operands / signalling barriers here
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc_2sm(tmem_base, 512);
     }
 }
 
@@ -441,6 +685,64 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     return EMC_OK;
 }
 
+int max_pair_clusters(const void *kern, int smem_bytes) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * 74);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = (size_t)smem_bytes;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n <= 0) {
+        cudaGetLastError();
+        n = num_sms() / 2;
+    }
+    return n;
+}
+
+template <int NP, int BN, int STAGES>
+emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
+    using C = Cfg2<NP, BN, STAGES>;
+    CUtensorMap tmA, tmB;
+    {
+        const cuuint64_t dims[3] = {(cuuint64_t)g.K, (cuuint64_t)g.M, (cuuint64_t)NP};
+        const cuuint64_t strides[2] = {(cuuint64_t)g.lda * 2, (cuuint64_t)g.plane_stride * 2};
+        const cuuint32_t box[3] = {BLOCK_K, BLOCK_M, 1};
+        EMC_TRY(make_map(&tmA, g.A, g.a_fmt, 3, dims, strides, box));
+    }
+    {
+        const cuuint64_t dims[2] = {(cuuint64_t)g.K, (cuuint64_t)g.N};
+        const cuuint64_t strides[1] = {(cuuint64_t)g.ldb * 2};
+        const cuuint32_t box[2] = {BLOCK_K, C::HB};
+        EMC_TRY(make_map(&tmB, g.B, g.b_fmt, 2, dims, strides, box));
+    }
+    GemmArgs a;
+    a.M = g.M; a.N = g.N; a.K = g.K;
+    a.num_m_tiles = ceil_div(g.M, PAIR_M);
+    a.num_n_tiles = ceil_div(g.N, BN);
+    a.num_k_blocks = ceil_div(g.K, BLOCK_K);
+    a.out = g.out; a.ld_out = g.ld_out; a.rowv = g.rowv; a.epilogue = g.epilogue;
+    a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
+    a.chunk_scale = g.chunk_scale;
+    a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
+    a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
+              ((uint32_t)(PAIR_M >> 4) << 24);
+    auto kern = plane_gemm_pair_kernel<NP, BN, STAGES>;
+    static int clusters = 0;
+    if (!clusters) {
+        EMC_TRY_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        clusters = max_pair_clusters((const void *)kern, C::SMEM_BYTES);
+    }
+    const int tiles = a.num_m_tiles * a.num_n_tiles;
+    const int grid = 2 * (tiles < clusters ? tiles : clusters);
+    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, a);     // cluster size is a kernel attribute
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
 }  // namespace
 
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st) {
@@ -451,6 +753,13 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         simt_plane_gemm_kernel<<<grid, 128, 0, st>>>(g);
         EMC_LAUNCHED();
         return EMC_OK;
+    }
+    if (g.n_planes == 2 && !g.one_cta) {
+        // CTA pairs; tile width by wave quantisation: time ~ waves(BN) x BN (one pair per TPC, tiles of equal cost)
+        const int mt = ceil_div(g.M, PAIR_M), pairs = num_sms() / 2;
+        const long c256 = (long)ceil_div(mt * ceil_div(g.N, 256), pairs) * 256;
+        const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), pairs) * 192;
+        return c192 < c256 ? launch_tc_pair<2, 192, 5>(g, st) : launch_tc_pair<2, 256, 4>(g, st);
     }
     if (g.n_planes == 2) {
         // tile width by wave quantisation: time ~ waves(BN) x BN (one CTA per SM, tiles of equal cost)

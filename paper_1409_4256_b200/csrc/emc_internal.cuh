@@ -96,6 +96,7 @@ struct GemmProblem {
     int epilogue;       // EPI_*
     int k_chunk = 0;    // k-blocks (of 64) per TMEM accumulation chunk, 0 = default (8 = 512 elements)
     const float *chunk_scale = nullptr;   // [ceil(K/512)][M] factor applied when a chunk is drained, or null
+    bool one_cta = false;   // EMC_GEMM_1CTA: the one-CTA kernel instead of CTA pairs (cta_group::2)
 };
 enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-likelihood)
        EPI_STORE = 1,       // out = acc                                (raw update numerator)

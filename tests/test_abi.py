@@ -23,7 +23,7 @@ def test_header_symbols_all_exported():
 
 def test_header_constants_match_binding():
     header = (ROOT / "include" / "emc.h").read_text()
-    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_UPDATE_BF16X3", "EMC_DEBUG_SIMT",
+    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_UPDATE_BF16X3", "EMC_DEBUG_SIMT", "EMC_GEMM_1CTA",
                  "EMC_PATTERNS_ON_HOST", "EMC_PROFILE_STAGES", "EMC_MAX_COUNT"):
         m = re.search(rf"#define {name}\s+(0x[0-9a-fA-F]+|\d+)u?", header)
         assert m, name

@@ -64,7 +64,7 @@ def test_expand_index_map_bit_exact_and_slices(case, ref, use_ws):
     assert np.all(w[ref["idx"] < 0] == 0)
 
 
-@pytest.mark.parametrize("flags", [0, emc.EMC_DEBUG_SIMT], ids=["tcgen05", "simt"])
+@pytest.mark.parametrize("flags", [0, emc.EMC_GEMM_1CTA, emc.EMC_DEBUG_SIMT], ids=["tcgen05-pair", "tcgen05-1cta", "simt"])
 def test_loglik_within_1e5_of_A(case, ref, flags):
     inp = case.inp
     big_l, big_a = o.loglik(ref["W"], ref["idx"], inp.counts, inp.mask)
@@ -90,7 +90,8 @@ def test_normalize_stagewise_1e6(case, ref):
         assert np.abs(host(p2) - p_ref).max() <= 1e-6
 
 
-@pytest.mark.parametrize("flags", [0, emc.EMC_DEBUG_SIMT, emc.EMC_UPDATE_BF16X3], ids=["tcgen05", "simt", "bf16x3"])
+@pytest.mark.parametrize("flags", [0, emc.EMC_GEMM_1CTA, emc.EMC_DEBUG_SIMT, emc.EMC_UPDATE_BF16X3],
+                         ids=["tcgen05-pair", "tcgen05-1cta", "simt", "bf16x3"])
 def test_update_stagewise(case, ref, flags):
     inp = case.inp
     p32 = ref["P"]
