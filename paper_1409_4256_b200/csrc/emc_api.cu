@@ -63,7 +63,7 @@ struct Layout {
     float *pscale;            // [ld_n/512][R] inverse chunk scales of planesP
     float *s;                 // [R]
     float *Wnum;              // [R][P]        update numerators -> W'
-    float2 *acc;              // [2 G]         two staggered (num, den) grids
+    float2 *acc;              // [8 G]         8 staggered grids of 64-byte (num, den) corner blocks
     float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
     void *stage;              // one chunk of raw counts (patterns on host)
@@ -87,7 +87,7 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.pscale = a.take<float>((size_t)ceil_div(l.ld_n, 512) * R);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
-    l.acc = a.take<float2>((size_t)2 * n * n * n);
+    l.acc = a.take<float2>((size_t)8 * n * n * n);
     l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.stage = a.take<uint8_t>(stage_bytes);
@@ -221,7 +221,7 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
                         unsigned flags, void *ws, size_t ws_bytes, void *stream) {
     if (!Wnew || !det_ok(det) || !rot_ok(rot) || !model_out) return EMC_ERR_ARG;
     if (!sizes_ok(n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
-    const size_t need = round_up(sizeof(float2) * (size_t)2 * n * n * n, 1024);
+    const size_t need = round_up(sizeof(float2) * (size_t)8 * n * n * n, 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
     return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, det->q, det->mask, det->n_pix,
                            rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);

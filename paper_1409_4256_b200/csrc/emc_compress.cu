@@ -5,14 +5,17 @@
 //
 // with the same trilinear weights f and the same pinned sample geometry as Expand.
 //
-// The scatter is bound by the rate at which an SM issues global reductions (about one lane-operation
-// per 1.3 cycles), so the design minimises lane-operations: numerator and denominator
-// of a voxel are interleaved, and the two z-neighbours of a corner pair are adjacent in memory, so
-// one 16-byte red.global.add.v4.f32 carries {num,den}(z), {num,den}(z+1): 4 reductions per sample
-// instead of 16 scalar atomics.  A 16-byte reduction must be 16-byte aligned, which a pair starting
-// at an odd z is not; hence TWO accumulator grids, one holding pairs (2k,2k+1) and one holding pairs
-// (2k+1,2k+2); a sample uses the grid that matches the parity of its base z, and the final divide
-// kernel adds the two.  (n odd falls back to 8-byte reductions on a single grid.)
+// Measured on B200 (DESIGN.md §7 "Compress"): a global reduction costs the SM about 1.3 cycles per lane when the
+// lanes of a warp hit unrelated sectors and 0.8 when they are contiguous; 16 bytes per lane is the widest there
+// is.  So the design (a) moves a sample's 8 corners x (num, den) = 64 bytes in four 16-byte
+// red.global.add.v4.f32, and (b) makes those 64 bytes CONTIGUOUS and lets four adjacent lanes issue them in
+// one instruction: the accumulator is not a voxel grid but 8 staggered grids of 2x2x2 blocks, one per parity
+// (b_x&1, b_y&1, b_z&1) of the base corner; grid c holds, for every base of that parity, one aligned 64-byte
+// block {num, den} x corner (4 dx + 2 dy + dz), blocks ordered [b_x/2][b_y/2][b_z/2].  After computing its
+// own sample a lane hands (block, t_x, t_y, t_z, W') to its group of four by shuffles, and the group adds the
+// four samples' blocks one after the other, each lane carrying the corner pair (dx, dy, dz = 0..1) it owns.
+// The divide kernel gathers a voxel's 8 contributions.  64 G bytes of accumulators (16 MB at 64^3, 134 MB at
+// 128^3); n odd falls back to 8-byte reductions on a plain (num, den) grid.
 #include "emc_geometry.cuh"
 #include "emc_internal.cuh"
 
@@ -32,11 +35,11 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
-// grid = (R, ceil(P / kPixPerBlock)); n even.  acc = [2][n][n][n/2] float4 (even-z pairs, odd-z pairs).
+// grid = (R, ceil(P / kPixPerBlock)); n even.  acc = [8][(n/2)^3] blocks of 4 float4 (see the header).
 __global__ void __launch_bounds__(kThreads)
-compress_scatter_pairs_kernel(const float *__restrict__ Wn, const float *__restrict__ slice_w, int weighted,
-                              const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix,
-                              const float *__restrict__ quat, int n, float4 *__restrict__ acc) {
+compress_scatter_blocked_kernel(const float *__restrict__ Wn, const float *__restrict__ slice_w, int weighted,
+                                const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix,
+                                const float *__restrict__ quat, int n, float4 *__restrict__ acc) {
     __shared__ float rm[9];
     const int r = blockIdx.x;
     float om = 1.f;
@@ -51,51 +54,69 @@ compress_scatter_pairs_kernel(const float *__restrict__ Wn, const float *__restr
         for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
     }
     __syncthreads();
-    const int h = n >> 1;                        // float4 per z row
-    const size_t layer = (size_t)n * n * h;      // float4 per grid
+    const unsigned h = (unsigned)n >> 1;
+    const unsigned per_copy = h * h * h;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned sub = lane & 3u;              // which float4 of a 64-byte block this lane carries
+    const unsigned grp = lane & ~3u;
+    const bool sx = (sub & 2u) != 0, sy = (sub & 1u) != 0;
 #pragma unroll
     for (int j = 0; j < kPixPerThread; ++j) {
         const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
-        if (p >= n_pix) continue;
-        if (mask && mask[p] == 0) continue;
-        const Sample s = locate(rm, q[3 * p], q[3 * p + 1], q[3 * p + 2], n);
-        if (s.base < 0) continue;
-        const float v = Wn[(size_t)r * n_pix + p];
-        const float x1 = s.tx * om, x0 = (1.f - s.tx) * om;
-        const float y1 = s.ty, y0 = 1.f - s.ty, z1 = s.tz, z0 = 1.f - s.tz;
-        const int bz = s.bz, row = s.bx * n + s.by;
-        float4 *b = acc + (bz & 1 ? layer : 0) + (size_t)row * h + (bz >> 1);
-        float f0, f1;
-        f0 = x0 * y0 * z0; f1 = x0 * y0 * z1; red_add_v4(b, f0 * v, f0, f1 * v, f1);
-        f0 = x0 * y1 * z0; f1 = x0 * y1 * z1; red_add_v4(b + h, f0 * v, f0, f1 * v, f1);
-        f0 = x1 * y0 * z0; f1 = x1 * y0 * z1; red_add_v4(b + (size_t)n * h, f0 * v, f0, f1 * v, f1);
-        f0 = x1 * y1 * z0; f1 = x1 * y1 * z1; red_add_v4(b + (size_t)n * h + h, f0 * v, f0, f1 * v, f1);
+        // every lane stays in the loop (the exchange below is warp-wide); a lane without a sample carries blk = -1
+        const int pc = p < n_pix ? p : n_pix - 1;
+        const Sample s = locate(rm, q[3 * pc], q[3 * pc + 1], q[3 * pc + 2], n);
+        const bool ok = p < n_pix && s.base >= 0 && (!mask || mask[pc] != 0);
+        const float v = ok ? Wn[(size_t)r * n_pix + pc] : 0.f;
+        int blk = -1;
+        if (ok) {
+            const unsigned c = ((s.bx & 1u) << 2) | ((s.by & 1u) << 1) | (s.bz & 1u);
+            blk = (int)(c * per_copy + (((unsigned)s.bx >> 1) * h + ((unsigned)s.by >> 1)) * h + ((unsigned)s.bz >> 1));
+        }
+        // four rounds: in round k the four lanes of a group together add the 64-byte block of the sample held
+        // by lane grp + k; this lane carries corners (dx, dy) = (sx, sy), dz = 0 and 1
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int src = (int)grp + k;
+            const int b = __shfl_sync(0xffffffffu, blk, src);
+            const float tx = __shfl_sync(0xffffffffu, s.tx, src);
+            const float ty = __shfl_sync(0xffffffffu, s.ty, src);
+            const float tz = __shfl_sync(0xffffffffu, s.tz, src);
+            const float vv = __shfl_sync(0xffffffffu, v, src);
+            if (b >= 0) {
+                const float wx = (sx ? tx : 1.f - tx) * om;
+                const float wy = sy ? ty : 1.f - ty;
+                const float wxy = wx * wy;
+                const float f0 = wxy * (1.f - tz), f1 = wxy * tz;
+                red_add_v4(acc + 4 * (size_t)b + sub, f0 * vv, f0, f1 * vv, f1);
+            }
+        }
     }
 }
 
-// model'[l] = num/den with (num, den) = even-grid entry + odd-grid entry of voxel l
+// model'[l] = num/den, (num, den) gathered from the (up to) 8 blocks whose 2x2x2 corner set contains voxel l
 __global__ void __launch_bounds__(256)
-compress_divide_pairs_kernel(const float4 *__restrict__ acc, int n, float *__restrict__ model_out,
-                             float *__restrict__ den_out) {
-    const int h = n >> 1;
-    const size_t rows = (size_t)n * n;
-    const size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;   // one thread per even-grid float4 = voxels (2k, 2k+1)
-    if (t >= rows * h) return;
-    const int k2 = (int)(t % h);
-    const float4 e = acc[t];
-    const float4 *odd = acc + rows * h;
-    // odd grid entry m holds voxels (2m+1, 2m+2): voxel 2k is .zw of entry k-1, voxel 2k+1 is .xy of entry k
-    float n0 = e.x, d0 = e.y, n1 = e.z, d1 = e.w;
-    const float4 ok = odd[t];
-    n1 += ok.x; d1 += ok.y;
-    if (k2 > 0) {
-        const float4 om1 = odd[t - 1];
-        n0 += om1.z; d0 += om1.w;
+compress_divide_blocked_kernel(const float2 *__restrict__ acc, int n, float *__restrict__ model_out,
+                               float *__restrict__ den_out) {
+    const size_t l = (size_t)blockIdx.x * 256 + threadIdx.x;
+    const size_t g = (size_t)n * n * n;
+    if (l >= g) return;
+    const int z = (int)(l % n), y = (int)((l / n) % n), x = (int)(l / ((size_t)n * n));
+    const unsigned h = (unsigned)n >> 1;
+    const size_t per_copy = (size_t)h * h * h;
+    float num = 0.f, den = 0.f;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        const int bx = x - (d >> 2), by = y - ((d >> 1) & 1), bz = z - (d & 1);
+        if (bx < 0 || by < 0 || bz < 0 || bx > n - 2 || by > n - 2 || bz > n - 2) continue;
+        const unsigned c = ((bx & 1u) << 2) | ((by & 1u) << 1) | (bz & 1u);
+        const size_t blk = c * per_copy + (((size_t)(bx >> 1) * h + (by >> 1)) * h + (bz >> 1));
+        const float2 e = acc[8 * blk + d];
+        num += e.x;
+        den += e.y;
     }
-    const size_t l = (t / h) * n + 2 * (size_t)k2;
-    model_out[l] = d0 > 0.f ? n0 / d0 : 0.f;
-    model_out[l + 1] = d1 > 0.f ? n1 / d1 : 0.f;
-    if (den_out) { den_out[l] = d0; den_out[l + 1] = d1; }
+    model_out[l] = den > 0.f ? num / den : 0.f;
+    if (den_out) den_out[l] = den;
 }
 
 // grid = (R, ceil(P / kPixPerBlock))
@@ -159,12 +180,12 @@ emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighte
     const size_t g = (size_t)n * n * n;
     dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
     if ((n & 1) == 0) {
-        float4 *acc4 = reinterpret_cast<float4 *>(acc);          // 2 grids x G/2 float4 = 2 G float2
-        EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * sizeof(float4), st));
-        compress_scatter_pairs_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, weighted ? 1 : 0, q, mask, n_pix,
-                                                                 quat, n, acc4);
+        float4 *acc4 = reinterpret_cast<float4 *>(acc);          // 8 grids x (n/2)^3 blocks x 64 B = 8 G float2
+        EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * 8 * sizeof(float2), st));
+        compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, weighted ? 1 : 0, q, mask, n_pix,
+                                                                   quat, n, acc4);
         EMC_LAUNCHED();
-        compress_divide_pairs_kernel<<<(unsigned)((g / 2 + 255) / 256), 256, 0, st>>>(acc4, n, model_out, den_out);
+        compress_divide_blocked_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(acc, n, model_out, den_out);
         EMC_LAUNCHED();
         return EMC_OK;
     }

@@ -118,7 +118,7 @@ emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
 
-// Compress (emc_compress.cu).  acc = [2 G] float2 of scratch (two staggered (num, den) grids), zeroed inside.
+// Compress (emc_compress.cu).  acc = [8 G] float2 of scratch (8 staggered grids of corner blocks), zeroed inside.
 emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const float *q,
                            const uint8_t *mask, int n_pix, const float *quat, int n_rot, int n,
                            float2 *acc, float *model_out, float *den_out, cudaStream_t st);
