@@ -116,8 +116,11 @@ emc_status reset_header(const Layout &l, cudaStream_t st) {
     return EMC_OK;
 }
 
+// stats_ready (optional): the normalisation's column statistics go into l.scratch in the same pass, where the
+// kernel that runs supports it (weight = prior weights or null)
 emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
-                           unsigned flags, cudaStream_t st) {
+                           unsigned flags, cudaStream_t st, const float *weight = nullptr,
+                           bool *stats_ready = nullptr) {
     GemmProblem g;
     g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
     g.M = n_rot; g.N = n_pat; g.K = n_pix;
@@ -125,7 +128,16 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
     g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = EPI_SUB_ROW;
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
-    return launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st);
+    const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
+    if (stats_ready) {
+        g.stat_m = l.scratch;
+        g.stat_z = l.scratch + (size_t)normalize_stat_rows(n_rot) * l.ld_n;
+        g.ld_stat = l.ld_n;
+        g.weight = weight;
+        *stats_ready = ld_out == l.ld_n && gemm_fuses_stats(g, simt);
+        if (!*stats_ready) g.stat_m = g.stat_z = nullptr;
+    }
+    return launch_plane_gemm(g, simt, st);
 }
 
 emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, bool bf16x3, float *out,
@@ -194,7 +206,7 @@ emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, in
     const size_t need = round_up(sizeof(float) * normalize_scratch_floats(rot->n_rot, ld_n), 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
     return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, false, 0, nullptr, s, loglik,
-                            (flags & EMC_ACCUMULATE) != 0, (float *)ws, (cudaStream_t)stream);
+                            (flags & EMC_ACCUMULATE) != 0, (float *)ws, false, (cudaStream_t)stream);
 }
 
 emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detector *det,
@@ -273,17 +285,19 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                 }
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, bf16x3, l.ld_n, l.hdr, st));
             }
-            // stage 2: L = logW K^T - S
+            // stage 2: L = logW K^T - S  (+ the column max / sum-exp partials of stage 3 from the same epilogue)
+            bool stats_ready = false;
             {
                 Span sp(prof, EMC_STAGE_LOGLIK, st);
-                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st));
+                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st, rot->weight, &stats_ready));
             }
             // stage 3: responsibilities of this chunk; s and LL add up over chunks
             float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
             {
                 Span sp(prof, EMC_STAGE_NORMALIZE, st);
                 EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, bf16x3,
-                                         (size_t)n_rot * l.ld_n, l.pscale, l.s, loglik + it, true, l.scratch, st));
+                                         (size_t)n_rot * l.ld_n, l.pscale, l.s, loglik + it, true, l.scratch, stats_ready,
+                                         st));
             }
             // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
             const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);

@@ -56,6 +56,11 @@ struct GemmArgs {
     int k_chunk;         // k-blocks per TMEM accumulation chunk
     const float *chunk_scale;   // [num_chunks][M] factor applied to a chunk when it is drained, or null
     uint32_t idesc;
+    // fused column statistics of the log-likelihood epilogue (pair kernel, STATS = true), see store_row_and_col_stats()
+    float *stat_m, *stat_z;     // [ceil(M/32)][ld_stat]
+    int ld_stat;
+    const float *weight;        // [M] prior weights w_r or null = uniform
+    float log_uniform;          // -log(M)
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -402,18 +407,64 @@ __device__ __forceinline__ void tmem_dealloc_2sm(uint32_t addr, uint32_t cols) {
 constexpr int PAIR_M = 2 * BLOCK_M;            // rows of a pair tile
 constexpr int kGroupPairM = 4;                 // rasterisation: 4 pair-rows (1024 rows) share each n sweep
 
-template <int NP, int BN, int STAGES>
+constexpr int kStatPitch = 33;                 // floats per row of a warp's 32 x 32 transposition tile
+template <int NP, int BN, int STAGES, bool STATS>
 struct Cfg2 {
     static constexpr int HB = BN / 2;                                 // B rows held by each CTA
     static constexpr int B_BYTES = HB * BLOCK_K * 2;
     static constexpr int STAGE_BYTES = NP * A_PLANE_BYTES + B_BYTES;  // per CTA
     static constexpr int BAR_BYTES = 256;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;
+    static constexpr int STAT_BYTES = STATS ? kNumEpiWarps * 32 * kStatPitch * 4 : 0;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STAT_BYTES + 1024;
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory per CTA");
     static_assert(2 * BN <= 512, "two accumulator stages must fit the 512 TMEM columns");
     static_assert(BN % 64 == 0 && BN <= 256, "UMMA N for M = 256; two epilogue warps per lane quarter");
     static_assert(HB % 8 == 0, "whole swizzle atoms");
 };
+
+// Log-likelihood epilogue of the pair kernel: store + fused first sweep of the normalisation (stage 3).
+// The warp holds 32 rows (rotations) x CW columns (patterns), one row per lane.  Each 32 x 32 block goes
+// through a padded shared-memory tile private to the warp and comes back transposed (lane = column), so that
+//  - L = acc - S[r] leaves as one full 128-byte line per row instead of 32 scattered 16-byte pieces, and
+//  - the per-column max and sum of exp of a = L + log w_r over the 32 rows fall out of the same walk; they are
+//    written as one partial per (32-row block, column) for colstats_combine_kernel.
+// a is formed from the stored fp32 L exactly as normalize_kernel forms it, so the maximum is the maximum of
+// the values the second sweep sees.  Column 32 of the tile (the padding) carries log w of the row, -inf for
+// rows beyond M.
+template <int CW>
+__device__ __forceinline__ void store_row_and_col_stats(const float (&racc)[CW], const GemmArgs &args, int m, int row0,
+                                                        int n_base, float *tile, int lane) {
+    if (row0 >= args.M) return;                                     // warp-uniform: no valid row in this block
+    const bool live = m < args.M;
+    const float rv = live ? args.rowv[m] : 0.f;
+    tile[lane * kStatPitch + 32] = live ? (args.weight ? logf(args.weight[m]) : args.log_uniform) : -INFINITY;
+    const int rows = min(32, args.M - row0);
+    const size_t so = (size_t)(row0 >> 5) * args.ld_stat;
+#pragma unroll
+    for (int c = 0; c < CW; c += 32) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) tile[lane * kStatPitch + j] = racc[c + j] - rv;
+        __syncwarp();
+        const int col = n_base + c + lane;
+        const bool col_ok = col < args.N;
+        float *o = args.out + (size_t)row0 * args.ld_out + col;
+        float mx = -INFINITY;
+#pragma unroll 8
+        for (int i = 0; i < 32; ++i) {
+            const float v = tile[i * kStatPitch + lane];
+            if (col_ok && i < rows) o[(size_t)i * args.ld_out] = v;
+            mx = fmaxf(mx, v + tile[i * kStatPitch + 32]);
+        }
+        float z = 0.f;
+#pragma unroll 8
+        for (int i = 0; i < 32; ++i) z += __expf((tile[i * kStatPitch + lane] + tile[i * kStatPitch + 32]) - mx);
+        __syncwarp();
+        if (col_ok) {
+            args.stat_m[so + col] = mx;
+            args.stat_z[so + col] = z;
+        }
+    }
+}
 
 __device__ __forceinline__ void pair_tile_coords(int tile, const GemmArgs &a, int &m_blk, int &n_blk) {
     const int per_group = kGroupPairM * a.num_n_tiles;
@@ -426,11 +477,11 @@ __device__ __forceinline__ void pair_tile_coords(int tile, const GemmArgs &a, in
 }
 
 // args.num_m_tiles counts PAIR tiles (256 rows)
-template <int NP, int BN, int STAGES>
+template <int NP, int BN, int STAGES, bool STATS>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
 plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                        const GemmArgs args) {
-    using C = Cfg2<NP, BN, STAGES>;
+    using C = Cfg2<NP, BN, STAGES, STATS>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + STAGES * C::STAGE_BYTES;
@@ -555,7 +606,12 @@ plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_con
                 if (lane == 0) mbar_arrive_leader(tempty_bar + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
-            if (m < args.M) {
+            if constexpr (STATS) {                 // log-likelihood (EPI_SUB_ROW): transposed store + column statistics
+                float *tile = reinterpret_cast<float *>(smem_raw + (bar_base + C::BAR_BYTES - smem_u32(smem_raw))) +
+                              (warp - 2) * 32 * kStatPitch;
+                store_row_and_col_stats<CW>(racc, args, m, m_blk * PAIR_M + (int)rank * BLOCK_M + quarter * 32,
+                                            n_blk * BN + half * CW, tile, lane);
+            } else if (m < args.M) {
                 const float rv = args.rowv ? args.rowv[m] : 0.f;
                 store_row<CW>(racc, args, m, n_blk * BN + half * CW, rv);
             }
@@ -668,6 +724,7 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
     a.chunk_scale = g.chunk_scale;
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
+    a.stat_m = a.stat_z = nullptr; a.ld_stat = 0; a.weight = nullptr; a.log_uniform = 0.f;
     // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
     // N >> 3 in [17,23); M >> 4 in [24,29)
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
@@ -703,9 +760,9 @@ int max_pair_clusters(const void *kern, int smem_bytes) {
     return n;
 }
 
-template <int NP, int BN, int STAGES>
+template <int NP, int BN, int STAGES, bool STATS>
 emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
-    using C = Cfg2<NP, BN, STAGES>;
+    using C = Cfg2<NP, BN, STAGES, STATS>;
     CUtensorMap tmA, tmB;
     {
         const cuuint64_t dims[3] = {(cuuint64_t)g.K, (cuuint64_t)g.M, (cuuint64_t)NP};
@@ -730,7 +787,9 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
               ((uint32_t)(PAIR_M >> 4) << 24);
-    auto kern = plane_gemm_pair_kernel<NP, BN, STAGES>;
+    a.stat_m = g.stat_m; a.stat_z = g.stat_z; a.ld_stat = g.ld_stat; a.weight = g.weight;
+    a.log_uniform = -logf((float)g.M);
+    auto kern = plane_gemm_pair_kernel<NP, BN, STAGES, STATS>;
     static int clusters = 0;
     if (!clusters) {
         EMC_TRY_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
@@ -744,6 +803,10 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
 }
 
 }  // namespace
+
+bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug) {
+    return g.stat_m && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug;
+}
 
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st) {
     if (g.M <= 0 || g.N <= 0 || g.K <= 0) return EMC_ERR_ARG;
@@ -759,7 +822,9 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         const int mt = ceil_div(g.M, PAIR_M), pairs = num_sms() / 2;
         const long c256 = (long)ceil_div(mt * ceil_div(g.N, 256), pairs) * 256;
         const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), pairs) * 192;
-        return c192 < c256 ? launch_tc_pair<2, 192, 5>(g, st) : launch_tc_pair<2, 256, 4>(g, st);
+        if (g.stat_m)
+            return c192 < c256 ? launch_tc_pair<2, 192, 4, true>(g, st) : launch_tc_pair<2, 256, 4, true>(g, st);
+        return c192 < c256 ? launch_tc_pair<2, 192, 5, false>(g, st) : launch_tc_pair<2, 256, 4, false>(g, st);
     }
     if (g.n_planes == 2) {
         // tile width by wave quantisation: time ~ waves(BN) x BN (one CTA per SM, tiles of equal cost)

@@ -336,28 +336,40 @@ div_rows_kernel(float *__restrict__ Wn, const float *__restrict__ s, int n_pix) 
 
 }  // namespace
 
+// rows of the partial-statistics arrays: the column sweep uses at most 64 row splits, the fused GEMM epilogue
+// (emc_gemm.cu store_row_and_col_stats) one per 32 rotations
+int normalize_stat_rows(int n_rot) {
+    const int fused = ceil_div(n_rot, 32);
+    return fused > 64 ? fused : 64;
+}
+
 size_t normalize_scratch_floats(int n_rot, int ld_n) {
-    (void)n_rot;
-    return (size_t)(2 * 64 + 2) * (size_t)ld_n;      // split partials (max, sum) + combined (max, 1/sum)
+    return (size_t)(2 * normalize_stat_rows(n_rot) + 2) * (size_t)ld_n;   // partials (max, sum) + combined (max, 1/sum)
 }
 
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
-                            float *s, double *loglik, bool accumulate, float *scratch,
+                            float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
                             cudaStream_t st) {
-    const int col_blocks = ceil_div(n_pat, kColsPerBlock);
-    const int splits = row_splits_for(n_rot, col_blocks);
-    const int rows_per_split = ceil_div(n_rot, splits);
-    const int n_splits = ceil_div(n_rot, rows_per_split);
-    float *part_m = scratch, *part_z = scratch + (size_t)64 * ld_n;
+    const int stat_rows = normalize_stat_rows(n_rot);
+    float *part_m = scratch, *part_z = scratch + (size_t)stat_rows * ld_n;
     if (!accumulate) {
         if (s) EMC_TRY_CUDA(cudaMemsetAsync(s, 0, sizeof(float) * n_rot, st));
         if (loglik) EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
     }
-    colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split,
-                                                                     part_m, part_z);
-    EMC_LAUNCHED();
-    float *col_m = scratch + (size_t)128 * ld_n, *col_iz = col_m + ld_n;
+    int n_splits;
+    if (stats_ready) {
+        n_splits = ceil_div(n_rot, 32);               // written by the log-likelihood GEMM's epilogue
+    } else {
+        const int col_blocks = ceil_div(n_pat, kColsPerBlock);
+        const int splits = row_splits_for(n_rot, col_blocks);
+        const int rows_per_split = ceil_div(n_rot, splits);
+        n_splits = ceil_div(n_rot, rows_per_split);
+        colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split,
+                                                                         part_m, part_z);
+        EMC_LAUNCHED();
+    }
+    float *col_m = scratch + (size_t)2 * stat_rows * ld_n, *col_iz = col_m + ld_n;
     colstats_combine_kernel<<<ceil_div(ld_n, 256), 256, 0, st>>>(part_m, part_z, n_pat, ld_n, n_splits, col_m, col_iz,
                                                                  loglik);
     EMC_LAUNCHED();
