@@ -88,7 +88,7 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
     l.acc = a.take<float2>((size_t)8 * n * n * n);
-    l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n) : 0);
+    l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n, n_pix) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
@@ -172,7 +172,7 @@ emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc
     if (!sizes_ok(model->n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
     float *blocked = nullptr;
     if (ws) {
-        EMC_TRY(check_ws(ws, ws_bytes, round_up(sizeof(float) * expand_scratch_floats(model->n), 1024)));
+        EMC_TRY(check_ws(ws, ws_bytes, round_up(sizeof(float) * expand_scratch_floats(model->n, det->n_pix), 1024)));
         blocked = (float *)ws;
     }
     return launch_expand(model->model, model->n, det->q, det->mask, det->n_pix, rot->quat, rot->n_rot, W, idx,

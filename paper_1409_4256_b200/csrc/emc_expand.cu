@@ -118,55 +118,80 @@ build_blocked_kernel(const float *__restrict__ model, int n, float4 *__restrict_
     blocked[2 * t + 1] = make_float4(v[4], v[5], v[6], v[7]);
 }
 
+// One 32-byte corner block in one request (LDG.256): a divergent gather costs the L1 one tag lookup per lane and
+// instruction, so two 16-byte loads of the same block cost twice as much as this.
+__device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b) {
+    asm volatile("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+                 : "l"(p));
+}
+
+// q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0): one coalesced 16-byte load per sample
+__global__ void __launch_bounds__(256)
+pack_geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix, float4 *__restrict__ qm) {
+    const int p = blockIdx.x * 256 + threadIdx.x;
+    if (p >= n_pix) return;
+    qm[p] = make_float4(q[3 * p], q[3 * p + 1], q[3 * p + 2], (mask && mask[p] == 0) ? 0.f : 1.f);
+}
+
+// The kernel is bound by instruction issue (about 180 warp instructions per 32 samples before this version,
+// ncu r01_v2), not by memory, so it is specialised on the outputs it has to write, reads its geometry as one
+// float4 per pixel and has no divergent control flow: a lane past the end of the detector repeats the last
+// pixel and only its stores are predicated.
+template <bool W_OUT, bool IDX_OUT, bool PLANES>
 __global__ void __launch_bounds__(kThreads)
-expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float *__restrict__ q,
-                      const uint8_t *__restrict__ mask, int n_pix, const float *__restrict__ quat,
-                      float *__restrict__ W, int32_t *__restrict__ idx, __half *__restrict__ planes, int ld_p,
-                      size_t plane_stride, float *__restrict__ S) {
-    __shared__ float rm[9];
+expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, int n_pix,
+                      const float *__restrict__ quat, float *__restrict__ W, int32_t *__restrict__ idx,
+                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S) {
+    __shared__ float rm_s[9];
     __shared__ float red[kThreads / 32];
     const int r = blockIdx.x;
     if (threadIdx.x == 0) {
         RotMat m = rotation_matrix(quat + 4 * (size_t)r);
 #pragma unroll
-        for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
+        for (int i = 0; i < 9; ++i) rm_s[i] = m.m[i];
     }
     __syncthreads();
+    float rm[9];
+#pragma unroll
+    for (int i = 0; i < 9; ++i) rm[i] = rm_s[i];
     const unsigned h = (unsigned)n >> 1;
     const unsigned per_copy = h * h * h;                    // 8 * per_copy <= 2^30 for n <= 1024
     float part = 0.f;
 #pragma unroll
     for (int j = 0; j < kPixPerThread; ++j) {
         const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
-        if (p >= n_pix) continue;
-        const Sample s = locate(rm, q[3 * p], q[3 * p + 1], q[3 * p + 2], n);
-        float w = 0.f;
-        if (s.base >= 0) {
-            const unsigned c = ((s.bx & 1u) << 2) | ((s.by & 1u) << 1) | (s.bz & 1u);
-            const unsigned blk = c * per_copy + (((unsigned)s.bx >> 1) * h + ((unsigned)s.by >> 1)) * h + ((unsigned)s.bz >> 1);
-            const float4 *bp = blocked + 2 * (size_t)blk;
-            const float4 lo4 = __ldg(bp), hi4 = __ldg(bp + 1);
-            const float z0 = 1.f - s.tz, y0 = 1.f - s.ty, x0 = 1.f - s.tx;
-            const float c00 = lo4.x * z0 + lo4.y * s.tz;
-            const float c01 = lo4.z * z0 + lo4.w * s.tz;
-            const float c10 = hi4.x * z0 + hi4.y * s.tz;
-            const float c11 = hi4.z * z0 + hi4.w * s.tz;
-            w = (c00 * y0 + c01 * s.ty) * x0 + (c10 * y0 + c11 * s.ty) * s.tx;
-        }
+        const bool in = p < n_pix;
+        const float4 g = qm[in ? p : n_pix - 1];
+        const Sample s = locate(rm, g.x, g.y, g.z, n);
+        const bool inside = s.base >= 0;
+        // outside samples read block 0 (any valid address) and are zeroed afterwards
+        const unsigned bx = inside ? (unsigned)s.bx : 0u, by = inside ? (unsigned)s.by : 0u, bz = inside ? (unsigned)s.bz : 0u;
+        const unsigned c = ((bx & 1u) << 2) | ((by & 1u) << 1) | (bz & 1u);
+        const unsigned blk = c * per_copy + ((bx >> 1) * h + (by >> 1)) * h + (bz >> 1);
+        float4 lo4, hi4;
+        ldg256(blocked + 2 * (size_t)blk, lo4, hi4);
+        const float z0 = 1.f - s.tz, y0 = 1.f - s.ty, x0 = 1.f - s.tx;
+        const float c00 = lo4.x * z0 + lo4.y * s.tz;
+        const float c01 = lo4.z * z0 + lo4.w * s.tz;
+        const float c10 = hi4.x * z0 + hi4.y * s.tz;
+        const float c11 = hi4.z * z0 + hi4.w * s.tz;
+        float w = (c00 * y0 + c01 * s.ty) * x0 + (c10 * y0 + c11 * s.ty) * s.tx;
+        w = inside ? w : 0.f;
         const size_t o = (size_t)r * n_pix + p;
-        if (W) W[o] = w;
-        if (idx) idx[o] = s.base;
-        const bool use = mask ? (mask[p] != 0) : true;
-        if (planes) {
+        if (W_OUT && in) W[o] = w;
+        if (IDX_OUT && in) idx[o] = s.base;
+        const bool use = in && g.w != 0.f;
+        if (PLANES && in) {
             __half hi, lo;
-            split_logw(w, use && s.base >= 0, hi, lo);
+            split_logw(w, use && inside, hi, lo);
             const size_t po = (size_t)r * ld_p + p;
             planes[po] = hi;
             planes[plane_stride + po] = lo;
         }
-        if (use) part += w;
+        part += use ? w : 0.f;
     }
-    if (S) {
+    if (PLANES) {                                            // S accompanies the planes (log-likelihood operands)
         const float t = block_sum(part, red);
         if (threadIdx.x == 0) atomicAdd(S + r, t);
     }
@@ -200,18 +225,35 @@ logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
 
 }  // namespace
 
-size_t expand_scratch_floats(int n) { return (n & 1) ? 0 : (size_t)8 * n * n * n; }
+static size_t expand_blocked_floats(int n) { return (size_t)8 * n * n * n; }
+// blocked model copies + one float4 of geometry per pixel
+size_t expand_scratch_floats(int n, int n_pix) { return (n & 1) ? 0 : expand_blocked_floats(n) + (size_t)4 * n_pix; }
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
                          int ld_p, float *S, float *blocked, cudaStream_t st) {
     dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+    if (planes && !S) return EMC_ERR_ARG;
     if (blocked && (n & 1) == 0) {
         const size_t blocks = (size_t)n * n * n;              // 8 copies x (n/2)^3 blocks
+        float4 *qm = reinterpret_cast<float4 *>(blocked + expand_blocked_floats(n));
         build_blocked_kernel<<<(unsigned)((blocks + 255) / 256), 256, 0, st>>>(model, n, (float4 *)blocked);
         EMC_LAUNCHED();
-        expand_blocked_kernel<<<grid, kThreads, 0, st>>>((const float4 *)blocked, n, q, mask, n_pix, quat, W, idx,
-                                                         planes, ld_p, (size_t)n_rot * ld_p, S);
+        pack_geometry_kernel<<<ceil_div(n_pix, 256), 256, 0, st>>>(q, mask, n_pix, qm);
+        EMC_LAUNCHED();
+        const float4 *b4 = (const float4 *)blocked;
+        const size_t ps = (size_t)n_rot * ld_p;
+#define EMC_EXPAND_CASE(w_, i_, p_)                                                                                   \
+    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, qm, n_pix, quat, W, idx, planes, ld_p, ps, S)
+        const int sel = (W ? 4 : 0) | (idx ? 2 : 0) | (planes ? 1 : 0);
+        switch (sel) {
+            case 1: EMC_EXPAND_CASE(false, false, true); break;
+            case 2: EMC_EXPAND_CASE(false, true, false); break;
+            case 4: EMC_EXPAND_CASE(true, false, false); break;
+            case 6: EMC_EXPAND_CASE(true, true, false); break;
+            default: return EMC_ERR_ARG;                         // no caller asks for slices and operand planes at once
+        }
+#undef EMC_EXPAND_CASE
         EMC_LAUNCHED();
         return EMC_OK;
     }

@@ -66,8 +66,9 @@ enum PlaneFormat { FMT_F16 = 0, FMT_BF16 = 1 };   // = the UMMA instruction desc
 // ---------------------------------------------------------------- stage launchers (device work)
 // Expand (emc_expand.cu).  Any of W, idx, planes may be null.  planes = [2][R][ld_p] fp16 (hi, lo)
 // of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).
-// `blocked` = scratch of expand_scratch_floats(n) floats for the blocked model copies, or null (plain gathers).
-size_t expand_scratch_floats(int n);
+// `blocked` = scratch of expand_scratch_floats(n, n_pix) floats (blocked model copies + packed geometry; then W / idx
+// or planes, not both), or null (plain gathers).
+size_t expand_scratch_floats(int n, int n_pix);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
                          int ld_p, float *S, float *blocked, cudaStream_t st);

@@ -197,20 +197,38 @@ __device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int
 }
 
 // between the sweeps: per column, combine the split partials into (max, 1/sum) and add up the total
-// log-likelihood  LL = sum_d (m_d + log z_d).
+// log-likelihood  LL = sum_d (m_d + log z_d).  block = 32 columns x 8 row lanes; row lane y merges the
+// partials k = y, y + 8, ... online, then the 8 are merged through shared memory.
 __global__ void __launch_bounds__(256)
 colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_z, int n_pat, int ld_n,
                         int n_splits, float *__restrict__ col_m, float *__restrict__ col_iz,
                         double *__restrict__ loglik) {
-    const int d = blockIdx.x * 256 + threadIdx.x;
+    __shared__ float sm_m[8][32], sm_z[8][32];
+    const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
+    const int d = blockIdx.x * 32 + x;
+    float mt = -INFINITY, zt = 0.f;
+    if (d < n_pat) {
+        for (int k = y; k < n_splits; k += 8) {
+            const float mk = part_m[(size_t)k * ld_n + d], zk = part_z[(size_t)k * ld_n + d];
+            if (zk > 0.f) {
+                if (mk > mt) { zt = zt * expf(mt - mk) + zk; mt = mk; }
+                else zt += zk * expf(mk - mt);
+            }
+        }
+    }
+    sm_m[y][x] = mt;
+    sm_z[y][x] = zt;
+    __syncthreads();
+    if (y != 0) return;
     double ll = 0.0;
     if (d < n_pat) {
-        float mt = -INFINITY, zt = 0.f;
-        for (int k = 0; k < n_splits; ++k) mt = fmaxf(mt, part_m[(size_t)k * ld_n + d]);
-        for (int k = 0; k < n_splits; ++k) {
-            const float zk = part_z[(size_t)k * ld_n + d];
-            if (zk > 0.f) zt += zk * expf(part_m[(size_t)k * ld_n + d] - mt);
-        }
+        mt = -INFINITY;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mt = fmaxf(mt, sm_m[k][x]);
+        zt = 0.f;
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if (sm_z[k][x] > 0.f) zt += sm_z[k][x] * expf(sm_m[k][x] - mt);
         col_m[d] = mt;
         col_iz[d] = 1.f / zt;
         ll = (double)mt + (double)logf(zt);
@@ -221,14 +239,7 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
     if (loglik) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) ll += __shfl_xor_sync(0xffffffffu, ll, o);
-        __shared__ double red[8];
-        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ll;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t = 0.0;
-            for (int w = 0; w < 8; ++w) t += red[w];
-            atomicAdd(loglik, t);
-        }
+        if (x == 0) atomicAdd(loglik, ll);
     }
 }
 
@@ -370,7 +381,7 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
         EMC_LAUNCHED();
     }
     float *col_m = scratch + (size_t)2 * stat_rows * ld_n, *col_iz = col_m + ld_n;
-    colstats_combine_kernel<<<ceil_div(ld_n, 256), 256, 0, st>>>(part_m, part_z, n_pat, ld_n, n_splits, col_m, col_iz,
+    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_z, n_pat, ld_n, n_splits, col_m, col_iz,
                                                                  loglik);
     EMC_LAUNCHED();
     // second sweep: 512-column chunks; enough row splits for about six resident blocks per SM
