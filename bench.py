@@ -165,6 +165,11 @@ def workload_name(cfg):
             + (f", pattern chunks of {cfg.n_pat_chunk}" if cfg.n_pat_chunk < cfg.n_pat else ""))
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two contractions, from the one `ncu --set full`
+# capture of this build summarised in profiles/r01_v3_full_ncu.md (bytes; config:stage)
+NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 804.4e6, "C2:update": 901.1e6}
+
+
 # ------------------------------------------------------------------------------ clocks
 
 class ClockSampler:
@@ -375,15 +380,13 @@ def main():
     for k in ("loglik", "update"):
         stages[k]["frac_of_bf16_sustained"] = stages[k]["issued_tflops"] / peaks["bf16_sustained"]
     dom = "update" if stage_ms["update"] >= stage_ms["loglik"] else "loglik"
-    traffic = None
-    tpath = ROOT / "profiles" / "traffic.json"
-    if tpath.exists():
-        traffic = json.loads(tpath.read_text()).get(f"{cfg.name}:{dom}")
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(f"{cfg.name}:{dom}")
     roofline = dict(bound="tensor", kernel=f"plane_gemm_kernel ({dom}, {stages[dom]['dtype']})",
                     achieved=stages[dom]["issued_tflops"], peak=peaks["bf16_sustained"], unit="TFLOP/s",
                     frac=stages[dom]["issued_tflops"] / peaks["bf16_sustained"], traffic=traffic,
                     peak_source=f"{peaks['source']} bf16 sustained (kernel timed inside a long step)",
                     avg_launch_ms=stage_ms[dom] / max(1, stage_spans[dom]),
+                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v3_full_ncu.md)",
                     note="achieved = 2*planes*R*N*P_eff flops per launch / CUDA-event launch time (issued MMA work of "
                          "the split scheme on unmasked pixels); useful TFLOP/s is in stages")
 
