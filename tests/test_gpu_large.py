@@ -1,0 +1,110 @@
+"""Parity at the geometry of BASELINE.json's large configs (C3: 128^3 / 128x128 / R = 25 000;
+C5 last stage: 256^3 / 256x256 / R = 50 000) on SAMPLED outputs the oracle computes one by one.
+Model, detector, mask and rotation list are the configs' own; only the pattern count is cut
+(make_inputs(..., n_pat=...)) so that the seeded generator finishes in seconds.  What these sizes
+exercise beyond C2: linear indices past 2^31 (R x P = 3.3e9), accumulators that do not fit L2,
+hundreds of K chunks, ragged last pair tiles.  (`-m gpu`)"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def sampled_rows(n_rot, k, seed):
+    """k rotation indices: the first, the last, the ones around 2^31 / n_pix, and random ones."""
+    rng = np.random.default_rng(seed)
+    rows = set(rng.integers(0, n_rot, size=k).tolist()) | {0, 1, n_rot - 2, n_rot - 1}
+    return np.array(sorted(rows), dtype=np.int64)
+
+
+def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
+    inp = inputs_cache(name, n_pat=n_pat)
+    cfg = inp.cfg
+    quat, weight = inp.quat[stage], inp.weight[stage]
+    n_rot, n_pix = quat.shape[0], cfg.n_pix
+    d_q, d_mask, d_quat, d_k = dev(inp.q), dev(inp.mask), dev(quat), dev(inp.counts)
+    rows = sampled_rows(n_rot, n_rows, 7)
+    if n_rot * n_pix > 2 ** 31:                                       # rows on both sides of the 32-bit boundary
+        edge = 2 ** 31 // n_pix
+        rows = np.unique(np.concatenate([rows, [edge - 1, edge, edge + 1]]))
+    t_rows = torch.from_numpy(rows).cuda()
+
+    # ---- stage 1 on sampled rotations: idx bit-exact, W within 1e-5
+    w, idx = emc.emc_expand(dev(inp.model_init), d_q, d_quat)
+    torch.cuda.empty_cache()                                          # expand's own workspace
+    ws = emc.make_workspace(cfg.n, n_pix, n_rot, n_pat)               # one workspace for the other stages
+    w_ref, idx_ref = o.expand(inp.model_init, inp.q, quat[rows])
+    assert np.array_equal(host(idx[t_rows]), idx_ref)
+    w_s = host(w[t_rows])
+    assert np.all(np.abs(w_s - w_ref) <= 1e-5 * np.abs(w_ref) + 1e-9 * np.abs(w_ref).max())
+
+    # ---- stage 2 on the GPU's W (identical to the oracle's within 1e-5, checked above): sampled rows of L
+    big_l = emc.emc_loglik(w, idx, d_q, d_mask, d_k, ws=ws)
+    l_ref, a_ref = o.loglik(w_s, idx_ref, inp.counts, inp.mask)
+    err = np.abs(host(big_l[t_rows]) - l_ref) / a_ref
+    assert err.max() <= 1e-5, f"max |dL|/A = {err.max():.3e}"
+    del w, idx
+    torch.cuda.empty_cache()
+
+    # ---- stage 3 stage-wise on sampled columns (each needs all R rows of the GPU's L)
+    p, s, ll = emc.emc_normalize(big_l, d_quat, dev(weight), ws=ws)
+    cols = np.unique(np.concatenate([np.random.default_rng(8).integers(0, n_pat, size=n_cols), [0, n_pat - 1]]))
+    t_cols = torch.from_numpy(cols).cuda()
+    p_ref, _, _ = o.normalize(host(big_l[:, t_cols]), weight)
+    assert np.abs(host(p[:, t_cols]) - p_ref).max() <= 1e-6
+    colsum = host(p.sum(dim=0, dtype=torch.float64))
+    assert np.abs(colsum - 1).max() <= 1e-4
+    s_ref = host(p.sum(dim=1, dtype=torch.float64))
+    assert np.abs(host(s) - s_ref).max() <= 1e-5 * max(1.0, s_ref.max())
+
+    # ---- stage 4 stage-wise on sampled rows: W'[r,:] = sum_d P[r,d] K[d,:] / s[r] from the GPU's P
+    wn = emc.emc_update(p, s, d_q, d_mask, d_k, ws=ws)
+    p_rows = host(p[t_rows])
+    wn_ref, _ = o.update(p_rows, inp.counts, inp.mask)
+    s_rows = p_rows.astype(np.float64).sum(axis=1)
+    got = host(wn[t_rows])
+    keep = s_rows > 1e-20
+    scale = np.abs(wn_ref[keep]).max()
+    rel = np.abs(got[keep] - wn_ref[keep]) / (np.abs(wn_ref[keep]) + 1e-7 * scale)
+    assert rel.max() <= 2e-5, f"max rel dW' = {rel.max():.3e}"       # s[r] itself is a float32 sum on the GPU
+    # photon conservation over ALL rows: sum_r s[r] W'[r,p] = sum_d K[d,p] on unmasked pixels
+    tot = torch.zeros(n_pix, dtype=torch.float64, device="cuda")
+    for r0 in range(0, n_rot, 2048):
+        tot += (wn[r0:r0 + 2048].double() * s[r0:r0 + 2048].double()[:, None]).sum(dim=0)
+    tot = host(tot)
+    k_tot = inp.counts.astype(np.float64).sum(axis=0)
+    use = inp.mask.astype(bool)
+    assert np.abs(tot[use] - k_tot[use]).max() <= 1e-4 * max(1.0, k_tot[use].max())
+
+    # ---- stage 5 on the first n_compress rotations of the GPU's W' (the oracle scatters them in float64)
+    sub = slice(0, n_compress)
+    sw = (host(s[sub]) > 0).astype(np.float32)
+    m, den = emc.emc_compress(wn[sub].contiguous(), dev(sw), d_q, d_mask, d_quat[sub].contiguous(), cfg.n, want_den=True,
+                              ws=ws)
+    m_ref, _, den_ref = o.compress(host(wn[sub]), inp.q, quat[sub], inp.mask, cfg.n, slice_w=sw)
+    m, den, m_ref = host(m).reshape(-1), host(den), m_ref.reshape(-1)
+    cov = den_ref >= 1e-6 * den_ref.max()
+    assert np.all(np.abs(den[cov] - den_ref[cov]) <= 1e-5 * den_ref[cov])
+    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12)
+    assert np.all(m[den_ref == 0] == 0)
+
+
+def test_c3_geometry_sampled(inputs_cache):
+    run_case(inputs_cache, "C3", n_pat=4096, stage=0, n_rows=24, n_cols=48, n_compress=1500)
+
+
+def test_c5_last_stage_geometry_sampled(inputs_cache):
+    run_case(inputs_cache, "C5", n_pat=1024, stage=4, n_rows=12, n_cols=32, n_compress=400)
