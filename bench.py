@@ -223,6 +223,22 @@ class ClockSampler:
                     reasons=sorted(reasons))
 
 
+# ------------------------------------------------------------------------------ replicas
+
+def whole_job(ms_local, units_per_rank, world, device):
+    """The path does not shard: every rank runs a replica.  Returns (max over ranks of the device
+    time in ms, whole-job rate = units all ranks processed / that time).  The only collective of a run."""
+    ms = float(ms_local)
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, world * units_per_rank / (ms * 1e-3)
+
+
 # ------------------------------------------------------------------------------ our arm
 
 def main():
@@ -297,11 +313,7 @@ def main():
     launches = emc.emc_launch_count() - launches0
     clk = clocks.stop()
     prof = emc.emc_profile_read()
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * args.steps * cfg.n_iter / (ms * 1e-3)
+    ms, value = whole_job(ms, args.steps * cfg.n_iter, world, "cuda")
 
     # ---- end to end through the C ABI with HOST buffers
     h_counts = torch.from_numpy(inp.counts).pin_memory()
@@ -343,11 +355,7 @@ def main():
     ev1.record()
     barrier()
     ms_e2e = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e_value = world * args.steps * cfg.n_iter / (ms_e2e * 1e-3)
+    ms_e2e, e2e_value = whole_job(ms_e2e, args.steps * cfg.n_iter, world, "cuda")
 
     # ---- rooflines from the live per-stage CUDA-event times
     p_eff = int(inp.mask.sum())

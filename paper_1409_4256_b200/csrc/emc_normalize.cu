@@ -208,12 +208,19 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
     const int d = blockIdx.x * 32 + x;
     float mt = -INFINITY, zt = 0.f;
     if (d < n_pat) {
-        for (int k = y; k < n_splits; k += 8) {
-            const float mk = part_m[(size_t)k * ld_n + d], zk = part_z[(size_t)k * ld_n + d];
-            if (zk > 0.f) {
-                if (mk > mt) { zt = zt * expf(mt - mk) + zk; mt = mk; }
-                else zt += zk * expf(mk - mt);
+        for (int k0 = y; k0 < n_splits; k0 += 8 * 4) {               // 4 independent loads in flight
+            float mk[4], zk[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int k = k0 + 8 * u;
+                mk[u] = k < n_splits ? part_m[(size_t)k * ld_n + d] : -INFINITY;
+                zk[u] = k < n_splits ? part_z[(size_t)k * ld_n + d] : 0.f;
             }
+            float mb = fmaxf(fmaxf(mk[0], mk[1]), fmaxf(mk[2], mk[3]));
+            if (mb > mt) { zt *= expf(mt - mb); mt = mb; }             // zt = 0 while mt = -inf: expf(-inf) = 0
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (zk[u] > 0.f) zt += zk[u] * expf(mk[u] - mt);
         }
     }
     sm_m[y][x] = mt;
@@ -245,7 +252,7 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
 
 // sweep 2: write P / planes / s.  grid = (ceil(N/512), row splits); a warp owns one row x 512 columns at a
 // time and prefetches the next row while it works on the current one.
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 3)
 normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
                  int ld_n, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_iz,
                  float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
