@@ -53,10 +53,11 @@ struct GemmArgs {
     const float *rowv;
     int epilogue;
     int vec_ok;          // out rows are 16-byte aligned
+    int tma_out;         // pair kernel: results leave through the output tensor map (needs vec_ok)
     int k_chunk;         // k-blocks per TMEM accumulation chunk
     const float *chunk_scale;   // [num_chunks][M] factor applied to a chunk when it is drained, or null
     uint32_t idesc;
-    // fused column statistics of the log-likelihood epilogue (pair kernel, STATS = true), see store_row_and_col_stats()
+    // fused column statistics of the log-likelihood epilogue (pair kernel, STATS = true), see tile_out()
     float *stat_m, *stat_z;     // [ceil(M/32)][ld_stat]
     int ld_stat;
     const float *weight;        // [M] prior weights w_r or null = uniform
@@ -394,7 +395,10 @@ __device__ __forceinline__ void umma_commit_2sm(uint32_t bar) {
                  ::"r"(bar), "h"((uint16_t)3) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_leader(uint32_t bar) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar & kPeerBitMask) : "memory");
+    // relaxed: what is ordered is this warp's tcgen05.ld before the leader's next tcgen05.mma, and the tcgen05 fences
+    // on both sides do that; a release at cluster scope compiles to a full MEMBAR.GPU, which waits for the tile's
+    // result stores to drain.
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar & kPeerBitMask) : "memory");
 }
 __device__ __forceinline__ void tmem_alloc_2sm(uint32_t dst_smem, uint32_t cols) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
@@ -407,61 +411,105 @@ __device__ __forceinline__ void tmem_dealloc_2sm(uint32_t addr, uint32_t cols) {
 constexpr int PAIR_M = 2 * BLOCK_M;            // rows of a pair tile
 constexpr int kGroupPairM = 4;                 // rasterisation: 4 pair-rows (1024 rows) share each n sweep
 
-constexpr int kStatPitch = 33;                 // floats per row of a warp's 32 x 32 transposition tile
+constexpr int kOutTileBytes = 32 * 128;        // a warp's 32 x 32 fp32 staging tile (one SWIZZLE_128B box)
 template <int NP, int BN, int STAGES, bool STATS>
 struct Cfg2 {
     static constexpr int HB = BN / 2;                                 // B rows held by each CTA
     static constexpr int B_BYTES = HB * BLOCK_K * 2;
     static constexpr int STAGE_BYTES = NP * A_PLANE_BYTES + B_BYTES;  // per CTA
+    static constexpr int OUT_BYTES = kNumEpiWarps * kOutTileBytes;    // after the ring, 1024-byte aligned
     static constexpr int BAR_BYTES = 256;
-    static constexpr int STAT_BYTES = STATS ? kNumEpiWarps * 32 * kStatPitch * 4 : 0;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + STAT_BYTES + 1024;
+    static constexpr int LW_BYTES = STATS ? kNumEpiWarps * 128 : 0;   // log w of a warp's 32 rows
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + OUT_BYTES + BAR_BYTES + LW_BYTES + 1024;
+    static_assert(STAGE_BYTES % 1024 == 0, "the staging tiles must keep the 1024-byte swizzle alignment");
     static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory per CTA");
     static_assert(2 * BN <= 512, "two accumulator stages must fit the 512 TMEM columns");
     static_assert(BN % 64 == 0 && BN <= 256, "UMMA N for M = 256; two epilogue warps per lane quarter");
     static_assert(HB % 8 == 0, "whole swizzle atoms");
 };
 
-// Log-likelihood epilogue of the pair kernel: store + fused first sweep of the normalisation (stage 3).
-// The warp holds 32 rows (rotations) x CW columns (patterns), one row per lane.  Each 32 x 32 block goes
-// through a padded shared-memory tile private to the warp and comes back transposed (lane = column), so that
-//  - L = acc - S[r] leaves as one full 128-byte line per row instead of 32 scattered 16-byte pieces, and
-//  - the per-column max and sum of exp of a = L + log w_r over the 32 rows fall out of the same walk; they are
-//    written as one partial per (32-row block, column) for colstats_combine_kernel.
-// a is formed from the stored fp32 L exactly as normalize_kernel forms it, so the maximum is the maximum of
-// the values the second sweep sees.  Column 32 of the tile (the padding) carries log w of the row, -inf for
-// rows beyond M.
-template <int CW>
-__device__ __forceinline__ void store_row_and_col_stats(const float (&racc)[CW], const GemmArgs &args, int m, int row0,
-                                                        int n_base, float *tile, int lane) {
-    if (row0 >= args.M) return;                                     // warp-uniform: no valid row in this block
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, uint32_t src, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(map), "r"(src), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap *map, uint32_t src, int c0, int c1) {
+    asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(map), "r"(src), "r"(c0), "r"(c1) : "memory");
+}
+
+// Final phase of a tile in the pair kernel.  The warp holds 32 rows x CW columns, one row per lane.  Measured
+// (clock64 around this phase, C2): with per-lane global stores it took 20-33 thousand cycles per tile, more than
+// the two TMEM stages of MMA work that can hide it, because every L1 wavefront queues behind the tensor core's
+// operand reads and the TMA fills; so the phase is built to issue as few wavefronts as possible.  Each 32 x 32
+// block is written once to a 4 KB shared-memory tile in the SWIZZLE_128B pattern (8 conflict-free 16-byte stores
+// per lane) and leaves as ONE asynchronous TMA store (or reduce-add for EPI_ADD), which also clips the ragged
+// edges of the matrix.  The log-likelihood variant (STATS) reads the same tile back transposed (lane = column)
+// for the first sweep of the normalisation: per-column max and sum of exp of a = L + log w_r over the 32 rows,
+// one partial per (32-row block, column), in one online pass.  a is formed from the stored fp32 L exactly as
+// normalize_kernel forms it.  Rows beyond M are staged as -inf (STATS) and never reach memory.
+template <int CW, bool STATS>
+__device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs &args, const CUtensorMap *tmC, int m,
+                                         int row0, int n_base, uint8_t *tile, float *lwbuf, int lane) {
+    if (row0 >= args.M) return;                                     // warp-uniform: nothing of this block exists
     const bool live = m < args.M;
-    const float rv = live ? args.rowv[m] : 0.f;
-    tile[lane * kStatPitch + 32] = live ? (args.weight ? logf(args.weight[m]) : args.log_uniform) : -INFINITY;
-    const int rows = min(32, args.M - row0);
+    const float rv = (live && args.rowv) ? args.rowv[m] : 0.f;
+    // eq. (2.5) divides a whole row by s[r]: one reciprocal per row.  (A division per element ran at 280 cycles
+    // each here: most numerators are subnormal and take the slow path of the IEEE division routine.)
+    const float inv = rv > 0.f ? 1.f / rv : 0.f;
+    const bool inv_ok = !(rv > 0.f) || inv < 3.0e38f;              // s[r] so small that 1/s overflows: divide
+    const uint32_t tile_s = smem_u32(tile);
+    const bool uniform = args.weight == nullptr;
+    if (STATS && !uniform) lwbuf[lane] = live ? logf(args.weight[m]) : 0.f;
     const size_t so = (size_t)(row0 >> 5) * args.ld_stat;
 #pragma unroll
     for (int c = 0; c < CW; c += 32) {
+        if (n_base + c >= args.N) break;                            // warp-uniform
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the tile is free again
+        __syncwarp();
 #pragma unroll
-        for (int j = 0; j < 32; ++j) tile[lane * kStatPitch + j] = racc[c + j] - rv;
-        __syncwarp();
-        const int col = n_base + c + lane;
-        const bool col_ok = col < args.N;
-        float *o = args.out + (size_t)row0 * args.ld_out + col;
-        float mx = -INFINITY;
-#pragma unroll 8
-        for (int i = 0; i < 32; ++i) {
-            const float v = tile[i * kStatPitch + lane];
-            if (col_ok && i < rows) o[(size_t)i * args.ld_out] = v;
-            mx = fmaxf(mx, v + tile[i * kStatPitch + 32]);
+        for (int k = 0; k < 8; ++k) {
+            float f[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float v = racc[c + 4 * k + j];
+                if (args.epilogue == EPI_SUB_ROW) f[j] = v - rv;
+                else if (args.epilogue == EPI_DIV_ROW) f[j] = inv_ok ? v * inv : (rv > 0.f ? v / rv : 0.f);
+                else f[j] = v;
+                if (STATS && !live) f[j] = -INFINITY;
+            }
+            *reinterpret_cast<float4 *>(tile + lane * 128 + ((k ^ (lane & 7)) << 4)) = make_float4(f[0], f[1], f[2], f[3]);
         }
-        float z = 0.f;
-#pragma unroll 8
-        for (int i = 0; i < 32; ++i) z += __expf((tile[i * kStatPitch + lane] + tile[i * kStatPitch + 32]) - mx);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
-        if (col_ok) {
-            args.stat_m[so + col] = mx;
-            args.stat_z[so + col] = z;
+        if (lane == 0) {
+            if (args.epilogue == EPI_ADD) tma_reduce_add_2d(tmC, tile_s, n_base + c, row0);
+            else tma_store_2d(tmC, tile_s, n_base + c, row0);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (STATS) {
+            const int col = n_base + c + lane;
+            const float *colp = reinterpret_cast<const float *>(tile) + (lane & 3);
+            const int chunk = lane >> 2;
+            // online (max, sum) over the 32 rows, four rows per step: one rescale of the running sum per step
+            float mx = -INFINITY, z = 0.f;
+#pragma unroll
+            for (int i0 = 0; i0 < 32; i0 += 4) {
+                float a[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int i = i0 + k;
+                    a[k] = colp[i * 32 + ((chunk ^ (i & 7)) << 2)] + (uniform ? args.log_uniform : lwbuf[i]);
+                }
+                // rows beyond M carry -inf: exp(-inf - mn) = 0; the floor keeps mn finite (no -inf - -inf) even if a
+                // caller passes zero weights
+                const float mn = fmaxf(fmaxf(fmaxf(mx, fmaxf(a[0], a[1])), fmaxf(a[2], a[3])), -3.0e38f);
+                z = z * __expf(mx - mn) + ((__expf(a[0] - mn) + __expf(a[1] - mn)) + (__expf(a[2] - mn) + __expf(a[3] - mn)));
+                mx = mn;
+            }
+            if (col < args.N) {
+                args.stat_m[so + col] = mx;
+                args.stat_z[so + col] = z;
+            }
         }
     }
 }
@@ -480,11 +528,12 @@ __device__ __forceinline__ void pair_tile_coords(int tile, const GemmArgs &a, in
 template <int NP, int BN, int STAGES, bool STATS>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
 plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                       const GemmArgs args) {
+                       const __grid_constant__ CUtensorMap tmC, const GemmArgs args) {
     using C = Cfg2<NP, BN, STAGES, STATS>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + STAGES * C::STAGE_BYTES;
+    const uint32_t out_base = smem_base + STAGES * C::STAGE_BYTES;            // 8 staging tiles of 4 KB
+    const uint32_t bar_base = out_base + C::OUT_BYTES;
     const uint32_t full_bar = bar_base, empty_bar = bar_base + 8 * STAGES;
     const uint32_t tfull_bar = bar_base + 16 * STAGES, tempty_bar = tfull_bar + 16;
     const uint32_t tmem_slot = tempty_bar + 16;
@@ -500,6 +549,7 @@ plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_con
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full_bar + 8 * s, 1);
             mbar_init(empty_bar + 8 * s, 1);
@@ -606,16 +656,18 @@ plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_con
                 if (lane == 0) mbar_arrive_leader(tempty_bar + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
             }
-            if constexpr (STATS) {                 // log-likelihood (EPI_SUB_ROW): transposed store + column statistics
-                float *tile = reinterpret_cast<float *>(smem_raw + (bar_base + C::BAR_BYTES - smem_u32(smem_raw))) +
-                              (warp - 2) * 32 * kStatPitch;
-                store_row_and_col_stats<CW>(racc, args, m, m_blk * PAIR_M + (int)rank * BLOCK_M + quarter * 32,
-                                            n_blk * BN + half * CW, tile, lane);
-            } else if (m < args.M) {
+            if (args.tma_out) {
+                uint8_t *tile = smem_raw + (out_base - smem_u32(smem_raw)) + (warp - 2) * kOutTileBytes;
+                float *lwbuf = reinterpret_cast<float *>(smem_raw + (bar_base + C::BAR_BYTES - smem_u32(smem_raw))) +
+                               (warp - 2) * 32;
+                tile_out<CW, STATS>(racc, args, &tmC, m, m_blk * PAIR_M + (int)rank * BLOCK_M + quarter * 32,
+                                    n_blk * BN + half * CW, tile, lwbuf, lane);
+            } else if (m < args.M) {               // misaligned output: per-lane stores
                 const float rv = args.rowv ? args.rowv[m] : 0.f;
                 store_row<CW>(racc, args, m, n_blk * BN + half * CW, rv);
             }
         }
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // staging tiles read, results written
     }
 
     tc_fence_before();
@@ -688,6 +740,21 @@ emc_status make_map(CUtensorMap *map, const void *base, PlaneFormat fmt, int ran
     return EMC_OK;
 }
 
+// fp32 output [rows][ld] as 32 x 32 boxes in the SWIZZLE_128B pattern (tile_out)
+emc_status make_out_map(CUtensorMap *map, const float *base, int rows, int cols, int ld) {
+    EncodeTiledFn enc;
+    EMC_TRY(get_encode_fn(&enc));
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+    const cuuint32_t box[2] = {32, 32};
+    const cuuint32_t ones[2] = {1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(base), dims, strides, box, ones,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cuda_fail(cudaErrorInvalidValue, "cuTensorMapEncodeTiled (output)");
+    return EMC_OK;
+}
+
 int num_sms() {
     static int sms = 0;
     if (!sms) {
@@ -724,7 +791,7 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
     a.chunk_scale = g.chunk_scale;
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
-    a.stat_m = a.stat_z = nullptr; a.ld_stat = 0; a.weight = nullptr; a.log_uniform = 0.f;
+    a.stat_m = a.stat_z = nullptr; a.ld_stat = 0; a.weight = nullptr; a.log_uniform = 0.f; a.tma_out = 0;
     // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
     // N >> 3 in [17,23); M >> 4 in [24,29)
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
@@ -789,6 +856,10 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
               ((uint32_t)(PAIR_M >> 4) << 24);
     a.stat_m = g.stat_m; a.stat_z = g.stat_z; a.ld_stat = g.ld_stat; a.weight = g.weight;
     a.log_uniform = -logf((float)g.M);
+    a.tma_out = a.vec_ok;
+    if (STATS && !a.tma_out) return EMC_ERR_ARG;             // gemm_fuses_stats() said no
+    CUtensorMap tmC = tmA;                                    // placeholder when the output is not TMA-addressable
+    if (a.tma_out) EMC_TRY(make_out_map(&tmC, g.out, g.M, g.N, g.ld_out));
     auto kern = plane_gemm_pair_kernel<NP, BN, STAGES, STATS>;
     static int clusters = 0;
     if (!clusters) {
@@ -797,7 +868,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     }
     const int tiles = a.num_m_tiles * a.num_n_tiles;
     const int grid = 2 * (tiles < clusters ? tiles : clusters);
-    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, a);     // cluster size is a kernel attribute
+    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, tmC, a);     // cluster size is a kernel attribute
     EMC_LAUNCHED();
     return EMC_OK;
 }
@@ -805,7 +876,9 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
 }  // namespace
 
 bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug) {
-    return g.stat_m && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug;
+    const bool aligned = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);      // the output goes out by TMA
+    return g.stat_m && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug &&
+           aligned;
 }
 
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st) {
@@ -824,7 +897,7 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), pairs) * 192;
         if (g.stat_m)
             return c192 < c256 ? launch_tc_pair<2, 192, 4, true>(g, st) : launch_tc_pair<2, 256, 4, true>(g, st);
-        return c192 < c256 ? launch_tc_pair<2, 192, 5, false>(g, st) : launch_tc_pair<2, 256, 4, false>(g, st);
+        return c192 < c256 ? launch_tc_pair<2, 192, 4, false>(g, st) : launch_tc_pair<2, 256, 4, false>(g, st);
     }
     if (g.n_planes == 2) {
         // tile width by wave quantisation: time ~ waves(BN) x BN (one CTA per SM, tiles of equal cost)
