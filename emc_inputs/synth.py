@@ -55,6 +55,8 @@ CONFIGS = {
     "T0": EmcConfig("T0", 16, 16, (60,), 40, 40, "int32", 2.0, 12, 0.0, 0, 10),
     "T1": EmcConfig("T1", 24, 20, (203,), 157, 157, "uint16", 0.5, 20, 2.0, 2, 11),
     "T2": EmcConfig("T2", 32, 40, (333, 401), 517, 200, "uint16", 0.3, 30, 3.0, 2, 12),
+    # odd everything: grid 17^3 (no blocked layouts), 15 x 15 = 225 pixels (rows of W' not 16-byte aligned), uint8 counts
+    "T3": EmcConfig("T3", 17, 15, (97,), 77, 77, "uint8", 0.8, 10, 1.5, 1, 13),
 }
 
 

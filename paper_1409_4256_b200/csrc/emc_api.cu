@@ -130,12 +130,14 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     if (stats_ready) {
+        const size_t rows = (size_t)normalize_stat_rows(n_rot);
         g.stat_m = l.scratch;
-        g.stat_z = l.scratch + (size_t)normalize_stat_rows(n_rot) * l.ld_n;
+        g.stat_w = l.scratch + rows * l.ld_n;
+        g.stat_z = l.scratch + 2 * rows * l.ld_n;
         g.ld_stat = l.ld_n;
         g.weight = weight;
         *stats_ready = ld_out == l.ld_n && gemm_fuses_stats(g, simt);
-        if (!*stats_ready) g.stat_m = g.stat_z = nullptr;
+        if (!*stats_ready) g.stat_m = g.stat_w = g.stat_z = nullptr;
     }
     return launch_plane_gemm(g, simt, st);
 }

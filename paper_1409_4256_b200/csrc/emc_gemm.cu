@@ -58,7 +58,7 @@ struct GemmArgs {
     const float *chunk_scale;   // [num_chunks][M] factor applied to a chunk when it is drained, or null
     uint32_t idesc;
     // fused column statistics of the log-likelihood epilogue (pair kernel, STATS = true), see tile_out()
-    float *stat_m, *stat_z;     // [ceil(M/32)][ld_stat]
+    float *stat_m, *stat_w, *stat_z;   // [ceil(M/32)][ld_stat]: reference pair (L, log w) and sum
     int ld_stat;
     const float *weight;        // [M] prior weights w_r or null = uniform
     float log_uniform;          // -log(M)
@@ -490,24 +490,51 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
             const int col = n_base + c + lane;
             const float *colp = reinterpret_cast<const float *>(tile) + (lane & 3);
             const int chunk = lane >> 2;
-            // online (max, sum) over the 32 rows, four rows per step: one rescale of the running sum per step
-            float mx = -INFINITY, z = 0.f;
+            // online statistics over the 32 rows, four rows per step, as a reference pair (mL, mw) = (L, log w) of
+            // the row with the largest L + log w and z = sum exp((L - mL) + (log w - mw)): see ColStat in
+            // emc_normalize.cu for why the two differences are taken separately.  Rows beyond M carry L = -inf.
+            float mL = -INFINITY, mw = 0.f, z = 0.f;
+            if (uniform) {
+                // log w is the same for every row: it drops out of the differences, the reference is the largest L
+                mw = args.log_uniform;
 #pragma unroll
-            for (int i0 = 0; i0 < 32; i0 += 4) {
-                float a[4];
+                for (int i0 = 0; i0 < 32; i0 += 4) {
+                    float l4[4];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int i = i0 + k;
-                    a[k] = colp[i * 32 + ((chunk ^ (i & 7)) << 2)] + (uniform ? args.log_uniform : lwbuf[i]);
+                    for (int k = 0; k < 4; ++k) l4[k] = colp[(i0 + k) * 32 + ((chunk ^ ((i0 + k) & 7)) << 2)];
+                    // row 0 of a block exists, so mn is finite from the first step on; exp(-inf - mn) = 0
+                    const float mn = fmaxf(fmaxf(mL, fmaxf(l4[0], l4[1])), fmaxf(l4[2], l4[3]));
+                    z = z * __expf(mL - mn) + ((__expf(l4[0] - mn) + __expf(l4[1] - mn)) + (__expf(l4[2] - mn) + __expf(l4[3] - mn)));
+                    mL = mn;
                 }
-                // rows beyond M carry -inf: exp(-inf - mn) = 0; the floor keeps mn finite (no -inf - -inf) even if a
-                // caller passes zero weights
-                const float mn = fmaxf(fmaxf(fmaxf(mx, fmaxf(a[0], a[1])), fmaxf(a[2], a[3])), -3.0e38f);
-                z = z * __expf(mx - mn) + ((__expf(a[0] - mn) + __expf(a[1] - mn)) + (__expf(a[2] - mn) + __expf(a[3] - mn)));
-                mx = mn;
+            } else {
+#pragma unroll 2
+                for (int i0 = 0; i0 < 32; i0 += 4) {
+                    float l4[4], w4[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int i = i0 + k;
+                        l4[k] = colp[i * 32 + ((chunk ^ (i & 7)) << 2)];
+                        w4[k] = lwbuf[i];
+                    }
+                    float bL = mL, bw = mw, bkey = mL + mw;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const float key = l4[k] + w4[k];
+                        if (key > bkey) { bkey = key; bL = l4[k]; bw = w4[k]; }
+                    }
+                    if (bL == -INFINITY) continue;                      // nothing but -inf so far (zero weights)
+                    float add = 0.f;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) add += __expf((l4[k] - bL) + (w4[k] - bw));
+                    z = z * __expf((mL - bL) + (mw - bw)) + add;
+                    mL = bL;
+                    mw = bw;
+                }
             }
             if (col < args.N) {
-                args.stat_m[so + col] = mx;
+                args.stat_m[so + col] = mL;
+                args.stat_w[so + col] = mw;
                 args.stat_z[so + col] = z;
             }
         }
@@ -791,7 +818,7 @@ emc_status launch_tc(const GemmProblem &g, cudaStream_t st) {
     a.k_chunk = g.k_chunk > 0 ? g.k_chunk : kChunkKBlocks;
     a.chunk_scale = g.chunk_scale;
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
-    a.stat_m = a.stat_z = nullptr; a.ld_stat = 0; a.weight = nullptr; a.log_uniform = 0.f; a.tma_out = 0;
+    a.stat_m = a.stat_w = a.stat_z = nullptr; a.ld_stat = 0; a.weight = nullptr; a.log_uniform = 0.f; a.tma_out = 0;
     // instruction descriptor (kind::f16): D = F32 [4,6); A format [7,10); B format [10,13); both K-major;
     // N >> 3 in [17,23); M >> 4 in [24,29)
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
@@ -854,7 +881,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     a.vec_ok = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
               ((uint32_t)(PAIR_M >> 4) << 24);
-    a.stat_m = g.stat_m; a.stat_z = g.stat_z; a.ld_stat = g.ld_stat; a.weight = g.weight;
+    a.stat_m = g.stat_m; a.stat_w = g.stat_w; a.stat_z = g.stat_z; a.ld_stat = g.ld_stat; a.weight = g.weight;
     a.log_uniform = -logf((float)g.M);
     a.tma_out = a.vec_ok;
     if (STATS && !a.tma_out) return EMC_ERR_ARG;             // gemm_fuses_stats() said no
@@ -877,7 +904,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
 
 bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug) {
     const bool aligned = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);      // the output goes out by TMA
-    return g.stat_m && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug &&
+    return g.stat_m && g.stat_w && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug &&
            aligned;
 }
 

@@ -98,9 +98,10 @@ struct GemmProblem {
     int k_chunk = 0;    // k-blocks (of 64) per TMEM accumulation chunk, 0 = default (8 = 512 elements)
     const float *chunk_scale = nullptr;   // [ceil(K/512)][M] factor applied when a chunk is drained, or null
     // log-likelihood only: fused first sweep of the normalisation.  When stat_m is set (and the CTA-pair kernel
-    // runs, see gemm_fuses_stats()) the epilogue writes per-(32-row block, column) partial max / sum-exp of
-    // a = out + log w_r into stat_m, stat_z [ceil(M/32)][ld_stat]; weight = [M] prior weights or null = 1/M.
-    float *stat_m = nullptr, *stat_z = nullptr;
+    // runs, see gemm_fuses_stats()) the epilogue writes per-(32-row block, column) partial statistics of
+    // a = out + log w_r (reference pair + sum-exp, emc_normalize.cu ColStat) into stat_m, stat_w, stat_z
+    // [ceil(M/32)][ld_stat]; weight = [M] prior weights or null = 1/M.
+    float *stat_m = nullptr, *stat_w = nullptr, *stat_z = nullptr;
     int ld_stat = 0;
     const float *weight = nullptr;
     bool one_cta = false;   // EMC_GEMM_1CTA: the one-CTA kernel instead of CTA pairs (cta_group::2)
@@ -117,7 +118,7 @@ bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug);
 // operand planes of P for the update GEMM: two fp16 planes scaled per (row, 512-column chunk) with the inverse
 // scales in chunk_inv_scale [ceil(ld_n/512)][R], or (bf16x3) three unscaled bf16 planes.
 size_t normalize_scratch_floats(int n_rot, int ld_n);
-int normalize_stat_rows(int n_rot);   // scratch = part_m [rows][ld_n], part_z [rows][ld_n], col_m [ld_n], col_iz [ld_n]
+int normalize_stat_rows(int n_rot);   // scratch = part_m, part_w, part_z [rows][ld_n] each, then col_m, col_w, col_iz [ld_n] each
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,

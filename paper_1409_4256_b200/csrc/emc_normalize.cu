@@ -34,28 +34,51 @@ __device__ __forceinline__ float log_weight(const float *__restrict__ weight, in
     return weight ? logf(weight[r]) : log_uniform;
 }
 
-__device__ __forceinline__ void online(float a, float &m, float &z) {
-    if (a > m) {
-        z = z * expf(m - a) + 1.f;
-        m = a;
+// Column statistics are kept as a REFERENCE PAIR (mL, mw) = (L, log w) of the row with the largest a = L + log w seen
+// so far, and z = sum exp((L - mL) + (log w - mw)).  Subtracting L from L and log w from log w before adding keeps
+// the exponent accurate to its own magnitude; forming a = L + log w first would round it to ulp(|L|), which at
+// |L| of a few thousand moves P by 1e-4 relative (T2 asks 1e-6 absolute).  With uniform weights the second
+// difference is exactly 0.
+struct ColStat {
+    float mL, mw, z;
+};
+__device__ __forceinline__ float rel_exponent(float L, float lw, float mL, float mw) { return (L - mL) + (lw - mw); }
+__device__ __forceinline__ void online(float L, float lw, ColStat &c) {
+    if (L + lw > c.mL + c.mw) {
+        c.z = c.z * expf(rel_exponent(c.mL, c.mw, L, lw)) + 1.f;      // z = 0 while the pair is (-inf, 0): 0 * 0
+        c.mL = L;
+        c.mw = lw;
     } else {
-        z += expf(a - m);
+        c.z += expf(rel_exponent(L, lw, c.mL, c.mw));
+    }
+}
+// merge b into a
+__device__ __forceinline__ void merge(ColStat &a, const ColStat &b) {
+    if (!(b.z > 0.f)) return;
+    if (b.mL + b.mw > a.mL + a.mw) {
+        a.z = a.z * expf(rel_exponent(a.mL, a.mw, b.mL, b.mw)) + b.z;
+        a.mL = b.mL;
+        a.mw = b.mw;
+    } else {
+        a.z += b.z * expf(rel_exponent(b.mL, b.mw, a.mL, a.mw));
     }
 }
 
-// sweep 1: partial (max, sum) of every column over the rows of one split
+// sweep 1: partial statistics of every column over the rows of one split (stage API; inside emc_iterate the
+// log-likelihood GEMM's epilogue writes the same partials, one per 32 rows)
 __global__ void __launch_bounds__(kThreads)
 colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
-                int ld_n, int rows_per_split, float *__restrict__ part_m, float *__restrict__ part_z) {
-    __shared__ float4 sm_m[kWarps][32], sm_z[kWarps][32];
+                int ld_n, int rows_per_split, float *__restrict__ part_m, float *__restrict__ part_w,
+                float *__restrict__ part_z) {
+    __shared__ float sm_m[kWarps][kColsPerBlock], sm_w[kWarps][kColsPerBlock], sm_z[kWarps][kColsPerBlock];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d = blockIdx.x * kColsPerBlock + lane * kVec;
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
     const float log_uniform = -logf((float)n_rot);
-    float m[kVec], z[kVec];
+    ColStat c[kVec];
 #pragma unroll
-    for (int j = 0; j < kVec; ++j) { m[j] = -INFINITY; z[j] = 0.f; }
+    for (int j = 0; j < kVec; ++j) c[j] = ColStat{-INFINITY, 0.f, 0.f};
     if (d < n_pat) {                                   // ld_n is a multiple of 4: the float4 stays inside the row
         for (int r0 = r_lo + warp; r0 < r_hi; r0 += kWarps * kBatch) {
             float4 v[kBatch];
@@ -71,36 +94,32 @@ colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, i
 #pragma unroll
             for (int b = 0; b < kBatch; ++b) {
                 if (r0 + b * kWarps < r_hi) {
-                    online(v[b].x + lw[b], m[0], z[0]);
-                    online(v[b].y + lw[b], m[1], z[1]);
-                    online(v[b].z + lw[b], m[2], z[2]);
-                    online(v[b].w + lw[b], m[3], z[3]);
+                    online(v[b].x, lw[b], c[0]);
+                    online(v[b].y, lw[b], c[1]);
+                    online(v[b].z, lw[b], c[2]);
+                    online(v[b].w, lw[b], c[3]);
                 }
             }
         }
     }
-    sm_m[warp][lane] = make_float4(m[0], m[1], m[2], m[3]);
-    sm_z[warp][lane] = make_float4(z[0], z[1], z[2], z[3]);
+#pragma unroll
+    for (int j = 0; j < kVec; ++j) {
+        sm_m[warp][lane * kVec + j] = c[j].mL;
+        sm_w[warp][lane * kVec + j] = c[j].mw;
+        sm_z[warp][lane * kVec + j] = c[j].z;
+    }
     __syncthreads();
     if (warp == 0 && d < n_pat) {
-        float mt[kVec], zt[kVec];
 #pragma unroll
-        for (int j = 0; j < kVec; ++j) { mt[j] = -INFINITY; zt[j] = 0.f; }
+        for (int j = 0; j < kVec; ++j) {
+            ColStat t = ColStat{-INFINITY, 0.f, 0.f};
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const float4 a = sm_m[w][lane];
-            mt[0] = fmaxf(mt[0], a.x); mt[1] = fmaxf(mt[1], a.y); mt[2] = fmaxf(mt[2], a.z); mt[3] = fmaxf(mt[3], a.w);
+            for (int w = 0; w < kWarps; ++w) merge(t, ColStat{sm_m[w][lane * kVec + j], sm_w[w][lane * kVec + j], sm_z[w][lane * kVec + j]});
+            const size_t o = (size_t)blockIdx.y * ld_n + d + j;
+            part_m[o] = t.mL;
+            part_w[o] = t.mw;
+            part_z[o] = t.z;
         }
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const float4 a = sm_m[w][lane], b = sm_z[w][lane];
-            if (b.x > 0.f) zt[0] += b.x * expf(a.x - mt[0]);
-            if (b.y > 0.f) zt[1] += b.y * expf(a.y - mt[1]);
-            if (b.z > 0.f) zt[2] += b.z * expf(a.z - mt[2]);
-            if (b.w > 0.f) zt[3] += b.w * expf(a.w - mt[3]);
-        }
-        *reinterpret_cast<float4 *>(part_m + (size_t)blockIdx.y * ld_n + d) = make_float4(mt[0], mt[1], mt[2], mt[3]);
-        *reinterpret_cast<float4 *>(part_z + (size_t)blockIdx.y * ld_n + d) = make_float4(zt[0], zt[1], zt[2], zt[3]);
     }
 }
 
@@ -200,47 +219,43 @@ __device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int
 // log-likelihood  LL = sum_d (m_d + log z_d).  block = 32 columns x 8 row lanes; row lane y merges the
 // partials k = y, y + 8, ... online, then the 8 are merged through shared memory.
 __global__ void __launch_bounds__(256)
-colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_z, int n_pat, int ld_n,
-                        int n_splits, float *__restrict__ col_m, float *__restrict__ col_iz,
+colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_w,
+                        const float *__restrict__ part_z, int n_pat, int ld_n, int n_splits,
+                        float *__restrict__ col_m, float *__restrict__ col_w, float *__restrict__ col_iz,
                         double *__restrict__ loglik) {
-    __shared__ float sm_m[8][32], sm_z[8][32];
+    __shared__ float sm_m[8][32], sm_w[8][32], sm_z[8][32];
     const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
     const int d = blockIdx.x * 32 + x;
-    float mt = -INFINITY, zt = 0.f;
+    ColStat t = ColStat{-INFINITY, 0.f, 0.f};
     if (d < n_pat) {
-        for (int k0 = y; k0 < n_splits; k0 += 8 * 4) {               // 4 independent loads in flight
-            float mk[4], zk[4];
+        for (int k0 = y; k0 < n_splits; k0 += 8 * 4) {               // 4 independent partials in flight
+            ColStat c[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int k = k0 + 8 * u;
-                mk[u] = k < n_splits ? part_m[(size_t)k * ld_n + d] : -INFINITY;
-                zk[u] = k < n_splits ? part_z[(size_t)k * ld_n + d] : 0.f;
+                const size_t o = (size_t)k * ld_n + d;
+                c[u] = k < n_splits ? ColStat{part_m[o], part_w[o], part_z[o]} : ColStat{-INFINITY, 0.f, 0.f};
             }
-            float mb = fmaxf(fmaxf(mk[0], mk[1]), fmaxf(mk[2], mk[3]));
-            if (mb > mt) { zt *= expf(mt - mb); mt = mb; }             // zt = 0 while mt = -inf: expf(-inf) = 0
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (zk[u] > 0.f) zt += zk[u] * expf(mk[u] - mt);
+            for (int u = 0; u < 4; ++u) merge(t, c[u]);
         }
     }
-    sm_m[y][x] = mt;
-    sm_z[y][x] = zt;
+    sm_m[y][x] = t.mL;
+    sm_w[y][x] = t.mw;
+    sm_z[y][x] = t.z;
     __syncthreads();
     if (y != 0) return;
     double ll = 0.0;
     if (d < n_pat) {
-        mt = -INFINITY;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) mt = fmaxf(mt, sm_m[k][x]);
-        zt = 0.f;
-#pragma unroll
-        for (int k = 0; k < 8; ++k)
-            if (sm_z[k][x] > 0.f) zt += sm_z[k][x] * expf(sm_m[k][x] - mt);
-        col_m[d] = mt;
-        col_iz[d] = 1.f / zt;
-        ll = (double)mt + (double)logf(zt);
+        for (int k = 1; k < 8; ++k) merge(t, ColStat{sm_m[k][x], sm_w[k][x], sm_z[k][x]});
+        col_m[d] = t.mL;
+        col_w[d] = t.mw;
+        col_iz[d] = 1.f / t.z;
+        ll = ((double)t.mL + (double)t.mw) + (double)logf(t.z);
     } else if (d < ld_n) {
         col_m[d] = 0.f;
+        col_w[d] = 0.f;
         col_iz[d] = 0.f;
     }
     if (loglik) {
@@ -252,24 +267,26 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
 
 // sweep 2: write P / planes / s.  grid = (ceil(N/512), row splits); a warp owns one row x 512 columns at a
 // time and prefetches the next row while it works on the current one.
-__global__ void __launch_bounds__(kThreads, 3)
+// UNIFORM = no weight array: log w is the same for every row and drops out of (L - mL) + (log w - mw).
+template <bool UNIFORM>
+__global__ void __launch_bounds__(kThreads, UNIFORM ? 3 : 2)
 normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
-                 int ld_n, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_iz,
-                 float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                 int ld_n, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_w,
+                 const float *__restrict__ col_iz, float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
                  float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d0 = blockIdx.x * kChunkCols;
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
-    const float log_uniform = -logf((float)n_rot);
-    float4 mt[kGroups], iz[kGroups];
+    float4 mt[kGroups], mw[UNIFORM ? 1 : kGroups], iz[kGroups];
     bool ok[kGroups];
 #pragma unroll
     for (int g = 0; g < kGroups; ++g) {
         const int d = d0 + g * kColsPerBlock + lane * kVec;
-        ok[g] = d < n_pat;                              // col_m / col_iz are defined (0) up to ld_n
+        ok[g] = d < n_pat;                              // col_m / col_w / col_iz are defined (0) up to ld_n
         mt[g] = ok[g] ? *reinterpret_cast<const float4 *>(col_m + d) : make_float4(0.f, 0.f, 0.f, 0.f);
         iz[g] = ok[g] ? *reinterpret_cast<const float4 *>(col_iz + d) : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (!UNIFORM) mw[g] = ok[g] ? *reinterpret_cast<const float4 *>(col_w + d) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
     float4 nxt[kGroups];
     int r = r_lo + warp;
@@ -288,21 +305,23 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
                 if (ok[g])
                     nxt[g] = *reinterpret_cast<const float4 *>(L + (size_t)(r + kWarps) * ld_n + d0 + g * kColsPerBlock + lane * kVec);
         }
-        const float lw = log_weight(weight, r, log_uniform);
+        const float lw = UNIFORM ? 0.f : logf(weight[r]);
         const size_t row_off = (size_t)r * ld_n;
         float p[kGroups][4];
         float sum = 0.f;
 #pragma unroll
         for (int g = 0; g < kGroups; ++g) {
             const int d = d0 + g * kColsPerBlock + lane * kVec;
-            const float a[4] = {v[g].x + lw, v[g].y + lw, v[g].z + lw, v[g].w + lw};
+            const float a[4] = {v[g].x, v[g].y, v[g].z, v[g].w};
             const float m4[4] = {mt[g].x, mt[g].y, mt[g].z, mt[g].w};
             const float z4[4] = {iz[g].x, iz[g].y, iz[g].z, iz[g].w};
+            float w4[4] = {0.f, 0.f, 0.f, 0.f};
+            if (!UNIFORM) { w4[0] = lw - mw[g].x; w4[1] = lw - mw[g].y; w4[2] = lw - mw[g].z; w4[3] = lw - mw[g].w; }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 float pj = 0.f;
                 if (d + j < n_pat) {
-                    pj = expf(a[j] - m4[j]) * z4[j];
+                    pj = expf(UNIFORM ? a[j] - m4[j] : (a[j] - m4[j]) + w4[j]) * z4[j];
                     if (pj < EMC_P_MIN) pj = 0.f;                      // DESIGN.md §3 G20
                 }
                 p[g][j] = pj;
@@ -362,7 +381,7 @@ int normalize_stat_rows(int n_rot) {
 }
 
 size_t normalize_scratch_floats(int n_rot, int ld_n) {
-    return (size_t)(2 * normalize_stat_rows(n_rot) + 2) * (size_t)ld_n;   // partials (max, sum) + combined (max, 1/sum)
+    return (size_t)(3 * normalize_stat_rows(n_rot) + 3) * (size_t)ld_n;   // partials (mL, mw, z) + combined (mL, mw, 1/z)
 }
 
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
@@ -370,7 +389,7 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
                             cudaStream_t st) {
     const int stat_rows = normalize_stat_rows(n_rot);
-    float *part_m = scratch, *part_z = scratch + (size_t)stat_rows * ld_n;
+    float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
     if (!accumulate) {
         if (s) EMC_TRY_CUDA(cudaMemsetAsync(s, 0, sizeof(float) * n_rot, st));
         if (loglik) EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
@@ -384,12 +403,12 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
         const int rows_per_split = ceil_div(n_rot, splits);
         n_splits = ceil_div(n_rot, rows_per_split);
         colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split,
-                                                                         part_m, part_z);
+                                                                         part_m, part_w, part_z);
         EMC_LAUNCHED();
     }
-    float *col_m = scratch + (size_t)2 * stat_rows * ld_n, *col_iz = col_m + ld_n;
-    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_z, n_pat, ld_n, n_splits, col_m, col_iz,
-                                                                 loglik);
+    float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
+    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_splits, col_m,
+                                                                 col_w, col_iz, loglik);
     EMC_LAUNCHED();
     // second sweep: 512-column chunks; enough row splits for about six resident blocks per SM
     const int chunks = ceil_div(n_pat, kChunkCols);
@@ -398,9 +417,13 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     if (splits2 > cap2) splits2 = cap2;
     if (splits2 < 1) splits2 = 1;
     const int rows2 = ceil_div(n_rot, splits2);
-    normalize_kernel<<<dim3(chunks, ceil_div(n_rot, rows2)), kThreads, 0, st>>>(
-        L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_iz, P, planes, bf16x3 ? 1 : 0, plane_stride,
-        chunk_inv_scale, s);
+    const dim3 grid2(chunks, ceil_div(n_rot, rows2));
+    if (weight)
+        normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_w, col_iz, P,
+                                                            planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
+    else
+        normalize_kernel<true><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_w, col_iz, P,
+                                                           planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
     EMC_LAUNCHED();
     return EMC_OK;
 }

@@ -40,7 +40,7 @@ class Case:
         self.d_counts = dev(inp.counts)
 
 
-@pytest.fixture(scope="module", params=["T1", "T2", "C1"])
+@pytest.fixture(scope="module", params=["T1", "T2", "T3", "C1"])
 def case(request, inputs_cache):
     inp = inputs_cache(request.param)
     return Case(inp, stage=len(inp.quat) - 1)
