@@ -166,8 +166,8 @@ def workload_name(cfg):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two contractions, from the one `ncu --set full`
-# capture of this build summarised in profiles/r01_v3_full_ncu.md (bytes; config:stage)
-NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 804.4e6, "C2:update": 901.1e6}
+# capture of this build summarised in profiles/r01_v4_full_ncu.md (bytes; config:stage)
+NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 823.9e6, "C2:update": 899.0e6}
 
 
 # ------------------------------------------------------------------------------ clocks
@@ -394,7 +394,7 @@ def main():
                     frac=stages[dom]["issued_tflops"] / peaks["bf16_sustained"], traffic=traffic,
                     peak_source=f"{peaks['source']} bf16 sustained (kernel timed inside a long step)",
                     avg_launch_ms=stage_ms[dom] / max(1, stage_spans[dom]),
-                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v3_full_ncu.md)",
+                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v4_full_ncu.md)",
                     note="achieved = 2*planes*R*N*P_eff flops per launch / CUDA-event launch time (issued MMA work of "
                          "the split scheme on unmasked pixels); useful TFLOP/s is in stages")
 
