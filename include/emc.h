@@ -178,6 +178,23 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
                        size_t ws_bytes, void *stream);
 
+/* Adaptive EMC, section 3.4 and eq. (3.1): `n_iter` iterations that start on the coarsest
+ * rotation list levels[0] and move on to the next list after an iteration n >= 1 whose total log-likelihood
+ * satisfies  |L^n - L^(n-1)| <= threshold |L^n|  (the paper: threshold = 0.01, and the lists are the
+ * discretisations d, d+1, ... of eq. (2.7)); the last list is kept.  Each iteration is one emc_iterate().
+ *   levels        HOST array of n_levels rotation lists (their quat / weight arrays are device pointers)
+ *   model_out     [n^3] float, out: the model after the last iteration
+ *   model_tmp     [n^3] float scratch (the iterations alternate between the two; neither may alias model->model)
+ *   loglik        [n_iter] device doubles, out
+ *   level_of_iter HOST [n_iter] int32, out: index of the list iteration n ran on
+ *   ws            sized for the largest list.
+ * The criterion is evaluated on the host in float64 from the device's log-likelihood, so this call synchronises
+ * `stream` once per iteration (the paper's master node does the same). */
+EMC_API emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc_rotations *levels,
+                      int n_levels, const emc_patterns *pat, int n_iter, double threshold, int n_pat_chunk,
+                      float *model_out, float *model_tmp, double *loglik, int32_t *level_of_iter,
+                      unsigned flags, void *ws, size_t ws_bytes, void *stream);
+
 /* Synchronises `stream` and reports what only the device saw during calls that used `ws`:
  * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (results are then undefined),
  * EMC_ERR_CUDA if the stream is in error.  Clears the record. */

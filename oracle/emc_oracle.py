@@ -292,3 +292,32 @@ def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=Fal
     om = s.astype(np.float32) if weighted else (s > 0).astype(np.float32)
     new_model, _, den = compress(wn, q, quat, mask, n, slice_w=om)
     return dict(model=new_model, W=w, idx=idx, L=l_all, P=p_all, s=s, Wn=wn, LL=ll, den=den)
+
+
+# ----------------------------------------------------------------------------------------------
+# Adaptive EMC, PAPER.md:205-210 (section 3.4, eq. 3.1)
+# ----------------------------------------------------------------------------------------------
+
+def refine_criterion(ll_prev, ll_cur, threshold=0.01):
+    """Eq. (3.1): the rotational discretisation is refined when |L^n - L^(n-1)| <= 0.01 |L^n|."""
+    return abs(ll_cur - ll_prev) <= threshold * abs(ll_cur)
+
+
+def refine(model, q, mask, levels, counts, n_iter, threshold=0.01, weighted=False):
+    """Adaptive EMC: start on the coarsest rotation list `levels[0]` = (quat, weight) and
+    move to the next list "whenever the current value seems too small to improve the likelihood any further",
+    i.e. after an iteration n >= 1 whose log-likelihood satisfies eq. (3.1) against iteration n - 1 (the paper
+    increases d of eq. (2.7) by one; here the lists are given, DESIGN.md NEXT-1).  The last list is kept.
+    Returns dict(model, LL [n_iter], level [n_iter] = index of the list iteration n ran on)."""
+    level = 0
+    lls, used = [], []
+    cur = np.asarray(model, dtype=np.float32)
+    for n in range(n_iter):
+        quat, weight = levels[level]
+        out = iterate(cur, q, mask, quat, weight, counts, weighted=weighted)
+        cur = out["model"]
+        lls.append(out["LL"])
+        used.append(level)
+        if n >= 1 and level + 1 < len(levels) and refine_criterion(lls[n - 1], lls[n], threshold):
+            level += 1
+    return dict(model=cur, LL=np.array(lls), level=np.array(used, dtype=np.int32))

@@ -30,7 +30,7 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_workspace_bytes", "emc_expand", "emc_loglik", "emc_normalize", "emc_update", "emc_compress",
-           "emc_iterate", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+           "emc_iterate", "emc_refine", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
 class EmcError(RuntimeError):
@@ -87,6 +87,9 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate.restype = ci
     lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                 ci, ci, vp, vp, ci, vp, cu, vp, sz, vp]
+    lib.emc_refine.restype = ci
+    lib.emc_refine.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), ci, POINTER(_Patterns), ci,
+                               c_double, ci, vp, vp, vp, POINTER(ctypes.c_int32), cu, vp, sz, vp]
     lib.emc_check.restype = ci
     lib.emc_check.argtypes = [vp, vp]
     lib.emc_profile_read.restype = ci
@@ -276,6 +279,25 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
                               p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
            "emc_iterate")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
+
+
+def emc_refine(model, q, mask, levels, counts, n_iter, threshold=0.01, n_pat_chunk=0, flags=0, ws=None):
+    """Adaptive EMC (section 3.4, eq. 3.1).  `levels` = [(quat [R,4], weight [R] or None), ...] from coarse to
+    fine.  Returns dict(model, loglik [n_iter] float64 tensor, level = list of the list index of every iteration)."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rots = (_Rotations * len(levels))(*[_rotations(qt, w) for qt, w in levels])
+    pat = _patterns(counts, det.n_pix, bool(flags & EMC_PATTERNS_ON_HOST))
+    chunk = pat.n_pat if (n_pat_chunk == 0 or n_pat_chunk > pat.n_pat) else n_pat_chunk
+    model_out, model_tmp = torch.empty_like(model), torch.empty_like(model)
+    loglik = torch.zeros(n_iter, dtype=torch.float64, device=model.device)
+    level = (ctypes.c_int32 * n_iter)()
+    ws, wp, wb = _ws(ws, n, det.n_pix, max(r.n_rot for r in rots), chunk, flags)
+    _check(load().emc_refine(m, det, rots, len(levels), pat, n_iter, float(threshold), n_pat_chunk,
+                             model_out.data_ptr(), model_tmp.data_ptr(), loglik.data_ptr(), level, flags, wp, wb,
+                             _stream()), "emc_refine")
+    return dict(model=model_out, loglik=loglik, level=list(level), ws=ws)
 
 
 def emc_check(ws):

@@ -4,6 +4,7 @@
 #include <atomic>
 #include <cstdio>
 #include <cstring>
+#include <cmath>
 
 #include "emc_internal.cuh"
 
@@ -319,6 +320,38 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                                     model_out, nullptr, st));
         }
         model_cur = model_out;
+    }
+    return EMC_OK;
+}
+
+emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc_rotations *levels,
+                      int n_levels, const emc_patterns *pat, int n_iter, double threshold, int n_pat_chunk,
+                      float *model_out, float *model_tmp, double *loglik, int32_t *level_of_iter,
+                      unsigned flags, void *ws, size_t ws_bytes, void *stream) {
+    if (!model || !model->model || !levels || n_levels <= 0 || n_iter <= 0 || !model_out || !model_tmp ||
+        model_out == model_tmp || model_out == model->model || model_tmp == model->model || !loglik ||
+        !level_of_iter || !(threshold >= 0.0))
+        return EMC_ERR_ARG;
+    for (int l = 0; l < n_levels; ++l)
+        if (!rot_ok(&levels[l])) return EMC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    float *bufs[2] = {model_out, model_tmp};
+    const float *src = model->model;
+    int level = 0;
+    double prev = 0.0;
+    for (int i = 0; i < n_iter; ++i) {
+        float *dst = bufs[(n_iter - 1 - i) & 1];                    // the last iteration lands in model_out
+        const emc_model cur = {model->n, src};
+        EMC_TRY(emc_iterate(&cur, det, &levels[level], pat, 1, n_pat_chunk, dst, nullptr, 0, loglik + i, flags, ws,
+                            ws_bytes, stream));
+        level_of_iter[i] = level;
+        double ll = 0.0;
+        EMC_TRY_CUDA(cudaMemcpyAsync(&ll, loglik + i, sizeof(double), cudaMemcpyDeviceToHost, st));
+        EMC_TRY_CUDA(cudaStreamSynchronize(st));
+        // eq. (3.1)
+        if (i >= 1 && level + 1 < n_levels && fabs(ll - prev) <= threshold * fabs(ll)) ++level;
+        prev = ll;
+        src = dst;
     }
     return EMC_OK;
 }
