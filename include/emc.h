@@ -168,7 +168,9 @@ EMC_API emc_status emc_compress(const float *Wnew, const float *slice_w, const e
  * Patterns are processed in chunks of n_pat_chunk (0 = all at once): stages 2-3 per chunk, s[r]
  * and the update numerators summed over chunks, divided after the last (DESIGN.md §3 G9).
  *   pat->counts may be a PINNED HOST pointer when flags has EMC_PATTERNS_ON_HOST: each chunk is
- *   then copied to the device inside the call.
+ *   then copied to the device inside the call, on a library-owned side stream into two staging
+ *   buffers of the workspace, so that the copy of one chunk overlaps the work on the previous one
+ *   (one thread at a time; use one stream per workspace).
  *   model_out [n^3] float, out (may not alias model->model).
  *   P_out     [R][ld_n] float of the LAST iteration, out, or NULL (ld_n >= N; needs one chunk).
  *   loglik    [n_iter] device doubles, out: total log-likelihood of each iteration. */

@@ -50,6 +50,27 @@ struct Span {
     }
 };
 
+// ---- host-resident patterns (EMC_PATTERNS_ON_HOST): chunks cross PCIe on a side stream into two staging buffers, so
+// the copy of chunk j + 1 overlaps pack + GEMMs of chunk j.  Created on first use; one thread at a time.
+struct Copier {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, entry = nullptr;
+    bool ok = false;
+};
+Copier g_copy;
+
+emc_status copier_init() {
+    if (g_copy.ok) return EMC_OK;
+    EMC_TRY_CUDA(cudaStreamCreateWithFlags(&g_copy.stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.ready[i], cudaEventDisableTiming));
+        EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.freed[i], cudaEventDisableTiming));
+    }
+    EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.entry, cudaEventDisableTiming));
+    g_copy.ok = true;
+    return EMC_OK;
+}
+
 size_t count_size(emc_count_type t) { return t == EMC_I32 ? 4 : (t == EMC_U16 ? 2 : 1); }
 
 // One layout serves every entry point; a call uses the parts it needs.
@@ -67,7 +88,7 @@ struct Layout {
     float2 *acc;              // [8 G]         8 staggered grids of 64-byte (num, den) corner blocks
     float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
-    void *stage;              // one chunk of raw counts (patterns on host)
+    void *stage;              // two chunks of raw counts (patterns on host, double-buffered)
     int ld_p, ld_n;
     size_t total;
 };
@@ -165,7 +186,7 @@ extern "C" {
 
 size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags) {
     if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return 0;
-    const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? (size_t)n_pat_chunk * n_pix * 4 : 0;
+    const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? 2 * round_up((size_t)n_pat_chunk * n_pix * 4, 1024) : 0;
     return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage).total;
 }
 
@@ -255,7 +276,8 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     const int n_chunks = ceil_div(n_pat, chunk);
     const bool on_host = (flags & EMC_PATTERNS_ON_HOST) != 0;
     const size_t csz = count_size(pat->type);
-    const size_t stage_bytes = on_host ? (size_t)chunk * n_pix * 4 : 0;
+    const size_t stage_one = round_up((size_t)chunk * n_pix * 4, 1024);          // one staging buffer (4 B per count at most)
+    const size_t stage_bytes = on_host ? 2 * stage_one : 0;
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes).total));
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
@@ -265,6 +287,25 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
 
     EMC_TRY(reset_header(l, st));
+    // pack jobs in order: every (iteration, chunk) when there are several chunks, else the one resident chunk once
+    const int n_jobs = n_chunks > 1 ? n_iter * n_chunks : 1;
+    auto issue_copy = [&](int j) -> emc_status {              // host -> staging buffer j & 1, on the side stream
+        const int c = j % n_chunks, d0 = c * chunk;
+        const int nc = n_pat - d0 < chunk ? n_pat - d0 : chunk;
+        const int b = j & 1;
+        if (j >= 2) EMC_TRY_CUDA(cudaStreamWaitEvent(g_copy.stream, g_copy.freed[b], 0));   // pack j - 2 has read it
+        EMC_TRY_CUDA(cudaMemcpyAsync((uint8_t *)l.stage + b * stage_one, (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz,
+                                     (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, g_copy.stream));
+        EMC_TRY_CUDA(cudaEventRecord(g_copy.ready[b], g_copy.stream));
+        return EMC_OK;
+    };
+    if (on_host) {
+        EMC_TRY(copier_init());
+        EMC_TRY_CUDA(cudaEventRecord(g_copy.entry, st));      // earlier work on `st` may still read the staging buffers
+        EMC_TRY_CUDA(cudaStreamWaitEvent(g_copy.stream, g_copy.entry, 0));
+        EMC_TRY(issue_copy(0));
+    }
+    int job = 0;
     const float *model_cur = model->model;
     for (int it = 0; it < n_iter; ++it) {
         // stage 1: Expand, with logW planes and S fused in
@@ -283,10 +324,14 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                 Span sp(prof, EMC_STAGE_PACK, st);
                 const uint8_t *src = (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz;
                 if (on_host) {
-                    EMC_TRY_CUDA(cudaMemcpyAsync(l.stage, src, (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, st));
-                    src = (const uint8_t *)l.stage;
+                    const int b = job & 1;
+                    if (job + 1 < n_jobs) EMC_TRY(issue_copy(job + 1));      // overlaps this chunk's pack and GEMMs
+                    EMC_TRY_CUDA(cudaStreamWaitEvent(st, g_copy.ready[b], 0));
+                    src = (const uint8_t *)l.stage + b * stage_one;
                 }
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, bf16x3, l.ld_n, l.hdr, st));
+                if (on_host) EMC_TRY_CUDA(cudaEventRecord(g_copy.freed[job & 1], st));
+                ++job;
             }
             // stage 2: L = logW K^T - S  (+ the column max / sum-exp partials of stage 3 from the same epilogue)
             bool stats_ready = false;

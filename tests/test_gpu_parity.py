@@ -165,6 +165,12 @@ def test_iterate_chunked_matches_single_chunk(inputs_cache):
     h = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, n_pat_chunk=200,
                         flags=emc.EMC_PATTERNS_ON_HOST)
     assert np.abs(host(h["model"]) - mb).max() <= 1e-5 * np.abs(mb).max()
+    # two iterations x three chunks through the two staging buffers = the same as device-resident patterns
+    b2 = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=2, n_pat_chunk=200)
+    h2 = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, n_iter=2, n_pat_chunk=200,
+                         flags=emc.EMC_PATTERNS_ON_HOST)
+    assert np.abs(host(h2["model"]) - host(b2["model"])).max() <= 1e-5 * np.abs(host(b2["model"])).max()
+    assert np.allclose(host(h2["loglik"]), host(b2["loglik"]), rtol=1e-6)   # fp32 atomics order the second iteration
 
 
 def test_iterate_multi_iteration_matches_repeated_calls(inputs_cache):
