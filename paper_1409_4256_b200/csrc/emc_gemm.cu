@@ -154,6 +154,9 @@ __device__ __forceinline__ void tile_coords(int tile, const GemmArgs &a, int &m_
 template <int CW>
 __device__ __forceinline__ void store_row(const float (&racc)[CW], const GemmArgs &args, int m, int n_base, float rv) {
     float *orow = args.out + (size_t)m * args.ld_out;
+    // one reciprocal per row (subnormal numerators make a per-element division take its slow path, see tile_out)
+    const float inv = rv > 0.f ? 1.f / rv : 0.f;
+    const bool inv_ok = !(rv > 0.f) || inv < 3.0e38f;
 #pragma unroll
     for (int c = 0; c < CW; c += 4) {
         const int n0 = n_base + c;
@@ -164,7 +167,7 @@ __device__ __forceinline__ void store_row(const float (&racc)[CW], const GemmArg
             for (int j = 0; j < 4; ++j) f[j] -= rv;
         } else if (args.epilogue == EPI_DIV_ROW) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) f[j] = rv > 0.f ? f[j] / rv : 0.f;
+            for (int j = 0; j < 4; ++j) f[j] = inv_ok ? f[j] * inv : (rv > 0.f ? f[j] / rv : 0.f);
         }
         float *o = orow + n0;
         if (args.vec_ok && n0 + 4 <= args.N) {
