@@ -321,3 +321,76 @@ def refine(model, q, mask, levels, counts, n_iter, threshold=0.01, weighted=Fals
         if n >= 1 and level + 1 < len(levels) and refine_criterion(lls[n - 1], lls[n], threshold):
             level += 1
     return dict(model=cur, LL=np.array(lls), level=np.array(used, dtype=np.int32))
+
+
+# ----------------------------------------------------------------------------------------------
+# The paper's own likelihood: Gaussian with a fluence per (rotation, frame), eqs. (2.2), (2.3),
+# (2.5), (2.6), (2.11), PAPER.md:70-89, 124-130  (NEXT-3, readings GA1-GA7)
+# ----------------------------------------------------------------------------------------------
+
+def fluence(w, counts, mask):
+    """phi[r,d] = sum_i K[d,i]^2 / sum_i W[r,i] K[d,i] over unmasked pixels   (eq. 2.6).
+    Where the denominator is 0 (a frame without photons on the slice's support) phi is +inf: K/phi = 0 (GA3).
+    Returns float64 [R,N]."""
+    use = _use(mask, np.asarray(w).shape[1])
+    wd = np.asarray(w, dtype=np.float32).astype(np.float64)[:, use]
+    k = np.asarray(counts)[:, use].astype(np.float64)
+    num = (k * k).sum(axis=1)                                    # [N]
+    den = wd @ k.T                                               # [R,N]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return np.where(den > 0, num[None, :] / den, np.inf)
+
+
+def gaussian_loglik(w, counts, mask, phi, sigma, chunk=8):
+    """Q[r,d] = sum_i -(K[d,i]/phi[r,d] - W[r,i])^2 / (2 sigma^2) over unmasked pixels, evaluated term by term as
+    eqs. (2.2)-(2.3) print it.  Also returns the scale the tolerance refers to,
+    A[r,d] = sum_i ((K/phi)^2 + W^2) / (2 sigma^2).  Returns (Q, A) float64 [R,N]."""
+    use = _use(mask, np.asarray(w).shape[1])
+    wd = np.asarray(w, dtype=np.float32).astype(np.float64)[:, use]
+    k = np.asarray(counts)[:, use].astype(np.float64)
+    n_rot, n_pat = wd.shape[0], k.shape[0]
+    q = np.empty((n_rot, n_pat))
+    a = np.empty((n_rot, n_pat))
+    inv = 1.0 / (2.0 * float(sigma) ** 2)
+    for r0 in range(0, n_rot, chunk):
+        r1 = min(n_rot, r0 + chunk)
+        scaled = k[None, :, :] / phi[r0:r1, :, None]             # [r,N,Pu]; K / inf = 0
+        diff = scaled - wd[r0:r1, None, :]
+        q[r0:r1] = -(diff * diff).sum(axis=2) * inv
+        a[r0:r1] = ((scaled * scaled).sum(axis=2) + (wd[r0:r1] ** 2).sum(axis=1)[:, None]) * inv
+    return q, a
+
+
+def update_gaussian(p, counts, mask, phi):
+    """W'[r,i] = sum_d P[r,d] K[d,i] / phi[r,d]  /  sum_d P[r,d]   (eq. 2.5 with the index typo read as P_jk, G10;
+    numerator = eq. 2.11).  Masked pixels and rows with s[r] = 0 give 0.  Returns (W' float32 [R,P], s float64)."""
+    pd = np.asarray(p).astype(np.float64)
+    k = np.asarray(counts)
+    use = _use(mask, k.shape[1])
+    s = pd.sum(axis=1)
+    with np.errstate(divide="ignore"):
+        num = (pd / phi) @ np.where(use[None, :], k, 0).astype(np.float64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        wn = np.where(s[:, None] > 0, num / s[:, None], 0.0)
+    wn[:, ~use] = 0.0
+    return wn.astype(np.float32), s
+
+
+def iterate_gaussian(model, q, mask, quat, weight, counts, sigma, weighted=True):
+    """One EMC iteration with the paper's Gaussian model: expand (2.9) -> fluence (2.6) from the expanded slices
+    -> E-step (2.2)-(2.4) -> M-step (2.5)/(2.11) with the same fluence -> compress (2.12) (or (2.10) with
+    weighted=False).  GA1: the fluence is recomputed from the current slices in every iteration and used in the E-
+    and M-step of that iteration.  Stage boundaries carry float32 (W, Q, P, W').
+    Returns dict(model, W, idx, phi, L, A, P, s, Wn, LL, den)."""
+    counts = np.asarray(counts)
+    n = np.asarray(model).shape[0]
+    w, idx = expand(model, q, quat)
+    phi = fluence(w, counts, mask)
+    big_q, big_a = gaussian_loglik(w, counts, mask, phi, sigma)
+    l32 = big_q.astype(np.float32)
+    p, _, ll = normalize(l32, weight)
+    p32 = p.astype(np.float32)
+    wn, s = update_gaussian(p32, counts, mask, phi)
+    om = s.astype(np.float32) if weighted else (s > 0).astype(np.float32)
+    new_model, _, den = compress(wn, q, quat, mask, n, slice_w=om)
+    return dict(model=new_model, W=w, idx=idx, phi=phi, L=l32, A=big_a, P=p32, s=s, Wn=wn, LL=ll, den=den)
