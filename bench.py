@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--bf16x3", action="store_true", help="opt-in: P as three unscaled bf16 planes in the update (3 MMAs per k-step)")
     ap.add_argument("--weighted", action="store_true", help="Compress by eq. (2.12) instead of eq. (2.10)")
+    ap.add_argument("--gaussian-sigma", type=float, default=0.0,
+                    help="> 0: time the paper's Gaussian likelihood with fluence (emc_iterate_gaussian, DESIGN.md section 11) "
+                         "instead of the Poisson path; not the BASELINE.json metric, no cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -285,6 +288,12 @@ def main():
         """all iterations of the config, device-resident inputs"""
         src, k, it0 = d_model0, 0, 0
         for quat, wgt, n_it, _, _ in plan:
+            if args.gaussian_sigma > 0:
+                out = emc.emc_iterate_gaussian(src, d_q, d_mask, quat, wgt, d_counts, args.gaussian_sigma, n_iter=n_it,
+                                               flags=f | emc.EMC_COMPRESS_WEIGHTED, ws=ws)
+                d_ll[it0:it0 + n_it] = out["loglik"]
+                src, it0 = out["model"], it0 + n_it
+                continue
             emc.emc_iterate(src, d_q, d_mask, quat, wgt, d_counts, n_iter=n_it, n_pat_chunk=chunk, flags=f, ws=ws,
                             model_out=bufs[k], loglik=d_ll[it0:it0 + n_it])
             src, k, it0 = bufs[k], 1 - k, it0 + n_it
@@ -314,6 +323,19 @@ def main():
     clk = clocks.stop()
     prof = emc.emc_profile_read()
     ms, value = whole_job(ms, args.steps * cfg.n_iter, world, "cuda")
+
+    if args.gaussian_sigma > 0:                  # a side measurement: device-resident only, Poisson-path JSON keys kept
+        prof_g = {k: v[0] / (args.steps * cfg.n_iter) for k, v in prof.items()}
+        if rank == 0:
+            print(json.dumps(dict(metric="emc_gaussian_iterations_per_s", value=value, unit=UNIT, n_gpus=world,
+                                  steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms / args.steps,
+                                  sigma=args.gaussian_sigma, config=dict(workload=workload_name(cfg)), clocks=clk,
+                                  stage_ms_per_iteration=prof_g, gpu_launches=int(launches),
+                                  loglik_per_iteration=[float(x) for x in d_ll.cpu().tolist()])))
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
 
     # ---- end to end through the C ABI with HOST buffers
     h_counts = torch.from_numpy(inp.counts).pin_memory()

@@ -180,6 +180,21 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
                        size_t ws_bytes, void *stream);
 
+/* Algorithm 1 with the paper's own likelihood: Gaussian around the slice with a fluence per (rotation, frame),
+ * eqs. (2.2), (2.3), (2.5)/(2.11), (2.6), PAPER.md:70-89, 124-130 (NEXT-3, readings GA1-GA7):
+ *   phi[r,d]  = sum_p K[d,p]^2 / sum_p W[r,p] K[d,p]                     (2.6), from the slices of this iteration
+ *   Q[r,d]    = -sum_p (K[d,p] / phi[r,d] - W[r,p])^2 / (2 sigma^2)      (2.2)-(2.3)
+ *   P         = the same normalisation over rotations as emc_normalize, with Q in the place of L
+ *   Wnew[r,p] = sum_d P[r,d] K[d,p] / phi[r,d]  /  sum_d P[r,d]          (2.5)
+ * over unmasked pixels, then Compress by eq. (2.12) with EMC_COMPRESS_WEIGHTED (what the paper runs) or (2.10).
+ * With phi of (2.6), Q collapses to (B^2 / A_d - C_r) / (2 sigma^2), B = sum_p W K (one plane GEMM), A_d = sum_p K^2,
+ * C_r = sum_p W^2; float32 evaluation of that form carries an absolute error of about 1e-7 C_r / (2 sigma^2).
+ * One pattern chunk, device-resident or host-resident patterns; slices must stay below 65504 (fp16 operand planes).
+ * Arguments as emc_iterate; sigma > 0 in the units of the model. */
+EMC_API emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                                const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
+                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream);
+
 /* Adaptive EMC, section 3.4 and eq. (3.1): `n_iter` iterations that start on the coarsest
  * rotation list levels[0] and move on to the next list after an iteration n >= 1 whose total log-likelihood
  * satisfies  |L^n - L^(n-1)| <= threshold |L^n|  (the paper: threshold = 0.01, and the lists are the

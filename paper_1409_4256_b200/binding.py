@@ -30,7 +30,7 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_workspace_bytes", "emc_expand", "emc_loglik", "emc_normalize", "emc_update", "emc_compress",
-           "emc_iterate", "emc_refine", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+           "emc_iterate", "emc_iterate_gaussian", "emc_refine", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
 class EmcError(RuntimeError):
@@ -87,6 +87,9 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate.restype = ci
     lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                 ci, ci, vp, vp, ci, vp, cu, vp, sz, vp]
+    lib.emc_iterate_gaussian.restype = ci
+    lib.emc_iterate_gaussian.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
+                                         ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp]
     lib.emc_refine.restype = ci
     lib.emc_refine.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), ci, POINTER(_Patterns), ci,
                                c_double, ci, vp, vp, vp, POINTER(ctypes.c_int32), cu, vp, sz, vp]
@@ -278,6 +281,25 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
     _check(load().emc_iterate(m, det, rot, pat, n_iter, n_pat_chunk, _dev(model_out, torch.float32, "model_out"),
                               p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
            "emc_iterate")
+    return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
+
+
+def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None):
+    """Algorithm 1 with the paper's Gaussian likelihood and fluence (eqs. 2.2-2.6).  Returns dict(model, loglik, P)."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rot = _rotations(quat, weight)
+    pat = _patterns(counts, det.n_pix, bool(flags & EMC_PATTERNS_ON_HOST))
+    dev = model.device
+    model_out = torch.empty_like(model)
+    loglik = torch.zeros(n_iter, dtype=torch.float64, device=dev)
+    ld = ld_for(pat.n_pat)
+    p = torch.empty((rot.n_rot, ld), dtype=torch.float32, device=dev) if want_p else None
+    ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, pat.n_pat, flags)
+    _check(load().emc_iterate_gaussian(m, det, rot, pat, n_iter, float(sigma), model_out.data_ptr(),
+                                       p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
+           "emc_iterate_gaussian")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
 
 

@@ -88,6 +88,7 @@ struct Layout {
     float2 *acc;              // [8 G]         8 staggered grids of 64-byte (num, den) corner blocks
     float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
+    float *Asq;               // [ld_n]        sum_p K^2 per pattern (Gaussian model)
     void *stage;              // two chunks of raw counts (patterns on host, double-buffered)
     int ld_p, ld_n;
     size_t total;
@@ -112,6 +113,7 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.acc = a.take<float2>((size_t)8 * n * n * n);
     l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n, n_pix) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
+    l.Asq = a.take<float>((size_t)l.ld_n);
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
     return l;
@@ -142,13 +144,14 @@ emc_status reset_header(const Layout &l, cudaStream_t st) {
 // kernel that runs supports it (weight = prior weights or null)
 emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
                            unsigned flags, cudaStream_t st, const float *weight = nullptr,
-                           bool *stats_ready = nullptr) {
+                           bool *stats_ready = nullptr, const GaussTerms *gauss = nullptr) {
     GemmProblem g;
     g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
     g.M = n_rot; g.N = n_pat; g.K = n_pix;
     g.lda = l.ld_p; g.ldb = l.ld_p; g.plane_stride = (size_t)n_rot * l.ld_p;
     g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
-    g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = EPI_SUB_ROW;
+    g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = gauss ? EPI_GAUSS : EPI_SUB_ROW;
+    if (gauss) { g.gauss_a = gauss->a_col; g.inv2s2 = gauss->inv2s2; }
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     if (stats_ready) {
@@ -263,10 +266,12 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
                            rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);
 }
 
-emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
-                       const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
-                       float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
-                       size_t ws_bytes, void *stream) {
+// Algorithm 1 for both likelihood models; sigma > 0 selects the paper's Gaussian model (section 11 of DESIGN.md)
+static emc_status iterate_impl(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                               const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
+                               float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
+                               size_t ws_bytes, void *stream, float sigma) {
+    const bool gauss = sigma > 0.f;
     if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_iter <= 0 || !model_out ||
         model_out == model->model || !loglik || n_pat_chunk < 0)
         return EMC_ERR_ARG;
@@ -281,6 +286,9 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes).total));
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
+    if (gauss && (n_chunks != 1 || (flags & (EMC_UPDATE_BF16X3 | EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
+    const GaussTerms gterms = {l.S, l.Asq, gauss ? 1.f / (2.f * sigma * sigma) : 0.f};
+    const GaussTerms *gt = gauss ? &gterms : nullptr;
     cudaStream_t st = (cudaStream_t)stream;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
     const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
@@ -313,7 +321,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
             Span sp(prof, EMC_STAGE_EXPAND, st);
             EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
             EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                                  l.planesL, l.ld_p, l.S, l.blocked, st));
+                                  l.planesL, l.ld_p, l.S, l.blocked, st, gauss));
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
@@ -331,13 +339,17 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                 }
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, bf16x3, l.ld_n, l.hdr, st));
                 if (on_host) EMC_TRY_CUDA(cudaEventRecord(g_copy.freed[job & 1], st));
+                if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
+                    EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * l.ld_n, st));
+                    EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, l.Asq, st));
+                }
                 ++job;
             }
             // stage 2: L = logW K^T - S  (+ the column max / sum-exp partials of stage 3 from the same epilogue)
             bool stats_ready = false;
             {
                 Span sp(prof, EMC_STAGE_LOGLIK, st);
-                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st, rot->weight, &stats_ready));
+                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st, rot->weight, &stats_ready, gt));
             }
             // stage 3: responsibilities of this chunk; s and LL add up over chunks
             float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
@@ -345,7 +357,7 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                 Span sp(prof, EMC_STAGE_NORMALIZE, st);
                 EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, bf16x3,
                                          (size_t)n_rot * l.ld_n, l.pscale, l.s, loglik + it, true, l.scratch, stats_ready,
-                                         st));
+                                         st, gt));
             }
             // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
             const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
@@ -367,6 +379,22 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
         model_cur = model_out;
     }
     return EMC_OK;
+}
+
+emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                       const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
+                       float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
+                       size_t ws_bytes, void *stream) {
+    return iterate_impl(model, det, rot, pat, n_iter, n_pat_chunk, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes,
+                        stream, 0.f);
+}
+
+emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                                const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
+                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream) {
+    if (!(sigma > 0.f)) return EMC_ERR_ARG;
+    return iterate_impl(model, det, rot, pat, n_iter, 0, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes, stream,
+                        sigma);
 }
 
 emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc_rotations *levels,

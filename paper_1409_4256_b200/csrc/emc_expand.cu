@@ -32,8 +32,9 @@ __device__ __forceinline__ float block_sum(float v, float *red) {
 }
 
 // logW -> two fp16 planes: hi = fp16(lw), lo = fp16(lw - hi); 22 significand bits in all.
-__device__ __forceinline__ void split_logw(float w, bool live, __half &hi, __half &lo) {
-    float lw = live ? logf(fmaxf(w, 1e-30f)) : 0.f;
+// gauss (the paper's Gaussian model): the operand is W itself, not log W
+__device__ __forceinline__ void split_logw(float w, bool live, __half &hi, __half &lo, int gauss = 0) {
+    float lw = live ? (gauss ? w : logf(fmaxf(w, 1e-30f))) : 0.f;
     hi = __float2half_rn(lw);
     lo = __float2half_rn(lw - __half2float(hi));
 }
@@ -43,7 +44,7 @@ __global__ void __launch_bounds__(kThreads)
 expand_kernel(const float *__restrict__ model, int n, const float *__restrict__ q,
               const uint8_t *__restrict__ mask, int n_pix, const float *__restrict__ quat,
               float *__restrict__ W, int32_t *__restrict__ idx, __half *__restrict__ planes, int ld_p,
-              size_t plane_stride, float *__restrict__ S) {
+              size_t plane_stride, float *__restrict__ S, int gauss) {
     __shared__ float rm[9];
     __shared__ float red[kThreads / 32];
     const int r = blockIdx.x;
@@ -76,12 +77,12 @@ expand_kernel(const float *__restrict__ model, int n, const float *__restrict__ 
         const bool use = mask ? (mask[p] != 0) : true;
         if (planes) {
             __half hi, lo;
-            split_logw(w, use && s.base >= 0, hi, lo);
+            split_logw(w, use && s.base >= 0, hi, lo, gauss);
             const size_t po = (size_t)r * ld_p + p;
             planes[po] = hi;
             planes[plane_stride + po] = lo;
         }
-        if (use) part += w;
+        if (use) part += gauss ? w * w : w;
     }
     if (S) {
         const float t = block_sum(part, red);
@@ -142,7 +143,7 @@ template <bool W_OUT, bool IDX_OUT, bool PLANES>
 __global__ void __launch_bounds__(kThreads)
 expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, int n_pix,
                       const float *__restrict__ quat, float *__restrict__ W, int32_t *__restrict__ idx,
-                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S) {
+                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S, int gauss) {
     __shared__ float rm_s[9];
     __shared__ float red[kThreads / 32];
     const int r = blockIdx.x;
@@ -184,12 +185,12 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
         const bool use = in && g.w != 0.f;
         if (PLANES && in) {
             __half hi, lo;
-            split_logw(w, use && inside, hi, lo);
+            split_logw(w, use && inside, hi, lo, gauss);
             const size_t po = (size_t)r * ld_p + p;
             planes[po] = hi;
             planes[plane_stride + po] = lo;
         }
-        part += use ? w : 0.f;
+        part += use ? (gauss ? w * w : w) : 0.f;
     }
     if (PLANES) {                                            // S accompanies the planes (log-likelihood operands)
         const float t = block_sum(part, red);
@@ -231,8 +232,9 @@ size_t expand_scratch_floats(int n, int n_pix) { return (n & 1) ? 0 : expand_blo
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, cudaStream_t st) {
+                         int ld_p, float *S, float *blocked, cudaStream_t st, bool gauss) {
     dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+    const int g = gauss ? 1 : 0;
     if (planes && !S) return EMC_ERR_ARG;
     if (blocked && (n & 1) == 0) {
         const size_t blocks = (size_t)n * n * n;              // 8 copies x (n/2)^3 blocks
@@ -244,7 +246,7 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         const float4 *b4 = (const float4 *)blocked;
         const size_t ps = (size_t)n_rot * ld_p;
 #define EMC_EXPAND_CASE(w_, i_, p_)                                                                                   \
-    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, qm, n_pix, quat, W, idx, planes, ld_p, ps, S)
+    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, qm, n_pix, quat, W, idx, planes, ld_p, ps, S, g)
         const int sel = (W ? 4 : 0) | (idx ? 2 : 0) | (planes ? 1 : 0);
         switch (sel) {
             case 1: EMC_EXPAND_CASE(false, false, true); break;
@@ -258,7 +260,7 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         return EMC_OK;
     }
     expand_kernel<<<grid, kThreads, 0, st>>>(model, n, q, mask, n_pix, quat, W, idx, planes, ld_p,
-                                             (size_t)n_rot * ld_p, S);
+                                             (size_t)n_rot * ld_p, S, g);
     EMC_LAUNCHED();
     return EMC_OK;
 }

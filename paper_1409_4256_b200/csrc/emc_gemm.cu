@@ -64,6 +64,16 @@ struct GemmArgs {
     float log_uniform;          // -log(M)
 };
 
+// Gaussian model (EPI_GAUSS, STATS = 2): out = B = acc; the statistics are taken of Q = (B^2 / A_d - C_r) / (2 sigma^2).
+// A kernel parameter of its own so that the other instantiations keep their exact parameter block and code.
+struct GaussParams {
+    const float *a;             // [N] A_d = sum_p K^2
+    float inv2s2;               // 1 / (2 sigma^2)
+};
+struct NoGauss {};
+template <int STATS> struct GaussOf { typedef NoGauss type; };
+template <> struct GaussOf<2> { typedef GaussParams type; };
+
 // ------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return (uint32_t)__cvta_generic_to_shared(p);
@@ -415,7 +425,7 @@ constexpr int PAIR_M = 2 * BLOCK_M;            // rows of a pair tile
 constexpr int kGroupPairM = 4;                 // rasterisation: 4 pair-rows (1024 rows) share each n sweep
 
 constexpr int kOutTileBytes = 32 * 128;        // a warp's 32 x 32 fp32 staging tile (one SWIZZLE_128B box)
-template <int NP, int BN, int STAGES, bool STATS>
+template <int NP, int BN, int STAGES, int STATS>
 struct Cfg2 {
     static constexpr int HB = BN / 2;                                 // B rows held by each CTA
     static constexpr int B_BYTES = HB * BLOCK_K * 2;
@@ -450,9 +460,10 @@ __device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap *map, uint32
 // for the first sweep of the normalisation: per-column max and sum of exp of a = L + log w_r over the 32 rows,
 // one partial per (32-row block, column), in one online pass.  a is formed from the stored fp32 L exactly as
 // normalize_kernel forms it.  Rows beyond M are staged as -inf (STATS) and never reach memory.
-template <int CW, bool STATS>
+template <int CW, int STATS>   // STATS: 0 = store only, 1 = + column statistics of L, 2 = + those of the Gaussian Q
 __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs &args, const CUtensorMap *tmC, int m,
-                                         int row0, int n_base, uint8_t *tile, float *lwbuf, int lane) {
+                                         int row0, int n_base, uint8_t *tile, float *lwbuf, int lane,
+                                         const typename GaussOf<STATS>::type &gp) {
     if (row0 >= args.M) return;                                     // warp-uniform: nothing of this block exists
     const bool live = m < args.M;
     const float rv = (live && args.rowv) ? args.rowv[m] : 0.f;
@@ -461,8 +472,16 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
     const float inv = rv > 0.f ? 1.f / rv : 0.f;
     const bool inv_ok = !(rv > 0.f) || inv < 3.0e38f;              // s[r] so small that 1/s overflows: divide
     const uint32_t tile_s = smem_u32(tile);
-    const bool uniform = args.weight == nullptr;
-    if (STATS && !uniform) lwbuf[lane] = live ? logf(args.weight[m]) : 0.f;
+    // Gaussian model: Q = B^2 g_d + (-C_r / (2 sigma^2)), g_d = 1 / (2 sigma^2 A_d): the row term joins log w_r as the
+    // row's "log weight", the element term B^2 g_d plays the role of L in the reference-pair statistics
+    constexpr bool gauss = STATS == 2;
+    const bool uniform = args.weight == nullptr && !gauss;
+    if constexpr (STATS == 1) {
+        if (!uniform) lwbuf[lane] = live ? logf(args.weight[m]) : 0.f;
+    } else if constexpr (STATS == 2) {
+        const float lw = args.weight ? logf(live ? args.weight[m] : 1.f) : args.log_uniform;
+        lwbuf[lane] = live ? gauss_row_term(lw, rv, gp.inv2s2) : -INFINITY;
+    }
     const size_t so = (size_t)(row0 >> 5) * args.ld_stat;
 #pragma unroll
     for (int c = 0; c < CW; c += 32) {
@@ -478,7 +497,7 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
                 if (args.epilogue == EPI_SUB_ROW) f[j] = v - rv;
                 else if (args.epilogue == EPI_DIV_ROW) f[j] = inv_ok ? v * inv : (rv > 0.f ? v / rv : 0.f);
                 else f[j] = v;
-                if (STATS && !live) f[j] = -INFINITY;
+                if (STATS && !live) f[j] = gauss ? 0.f : -INFINITY;
             }
             *reinterpret_cast<float4 *>(tile + lane * 128 + ((k ^ (lane & 7)) << 4)) = make_float4(f[0], f[1], f[2], f[3]);
         }
@@ -493,6 +512,10 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
             const int col = n_base + c + lane;
             const float *colp = reinterpret_cast<const float *>(tile) + (lane & 3);
             const int chunk = lane >> 2;
+            float g_col = 0.f;
+            if constexpr (gauss) {
+                if (col < args.N) g_col = gauss_col_factor(gp.a[col], gp.inv2s2);
+            }
             // online statistics over the 32 rows, four rows per step, as a reference pair (mL, mw) = (L, log w) of
             // the row with the largest L + log w and z = sum exp((L - mL) + (log w - mw)): see ColStat in
             // emc_normalize.cu for why the two differences are taken separately.  Rows beyond M carry L = -inf.
@@ -518,6 +541,7 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
                     for (int k = 0; k < 4; ++k) {
                         const int i = i0 + k;
                         l4[k] = colp[i * 32 + ((chunk ^ (i & 7)) << 2)];
+                        if constexpr (gauss) l4[k] = gauss_elem_term(l4[k], g_col);
                         w4[k] = lwbuf[i];
                     }
                     float bL = mL, bw = mw, bkey = mL + mw;
@@ -555,10 +579,11 @@ __device__ __forceinline__ void pair_tile_coords(int tile, const GemmArgs &a, in
 }
 
 // args.num_m_tiles counts PAIR tiles (256 rows)
-template <int NP, int BN, int STAGES, bool STATS>
+template <int NP, int BN, int STAGES, int STATS>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
 plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                       const __grid_constant__ CUtensorMap tmC, const GemmArgs args) {
+                       const __grid_constant__ CUtensorMap tmC, const GemmArgs args,
+                       const typename GaussOf<STATS>::type gp) {
     using C = Cfg2<NP, BN, STAGES, STATS>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -691,7 +716,7 @@ plane_gemm_pair_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_con
                 float *lwbuf = reinterpret_cast<float *>(smem_raw + (bar_base + C::BAR_BYTES - smem_u32(smem_raw))) +
                                (warp - 2) * 32;
                 tile_out<CW, STATS>(racc, args, &tmC, m, m_blk * PAIR_M + (int)rank * BLOCK_M + quarter * 32,
-                                    n_blk * BN + half * CW, tile, lwbuf, lane);
+                                    n_blk * BN + half * CW, tile, lwbuf, lane, gp);
             } else if (m < args.M) {               // misaligned output: per-lane stores
                 const float rv = args.rowv ? args.rowv[m] : 0.f;
                 store_row<CW>(racc, args, m, n_blk * BN + half * CW, rv);
@@ -857,7 +882,7 @@ int max_pair_clusters(const void *kern, int smem_bytes) {
     return n;
 }
 
-template <int NP, int BN, int STAGES, bool STATS>
+template <int NP, int BN, int STAGES, int STATS>
 emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     using C = Cfg2<NP, BN, STAGES, STATS>;
     CUtensorMap tmA, tmB;
@@ -898,7 +923,9 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     }
     const int tiles = a.num_m_tiles * a.num_n_tiles;
     const int grid = 2 * (tiles < clusters ? tiles : clusters);
-    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, tmC, a);     // cluster size is a kernel attribute
+    typename GaussOf<STATS>::type gp;
+    if constexpr (STATS == 2) { gp.a = g.gauss_a; gp.inv2s2 = g.inv2s2; }
+    kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, tmC, a, gp);     // cluster size is a kernel attribute
     EMC_LAUNCHED();
     return EMC_OK;
 }
@@ -907,7 +934,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
 
 bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug) {
     const bool aligned = (g.ld_out % 4 == 0) && (((uintptr_t)g.out & 15) == 0);      // the output goes out by TMA
-    return g.stat_m && g.stat_w && g.stat_z && g.rowv && g.epilogue == EPI_SUB_ROW && g.n_planes == 2 && !g.one_cta && !simt_debug &&
+    return g.stat_m && g.stat_w && g.stat_z && g.rowv && (g.epilogue == EPI_SUB_ROW || g.epilogue == EPI_GAUSS) && g.n_planes == 2 && !g.one_cta && !simt_debug &&
            aligned;
 }
 
@@ -920,14 +947,18 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         EMC_LAUNCHED();
         return EMC_OK;
     }
+    if (g.epilogue == EPI_GAUSS && !(g.stat_m && g.gauss_a && g.n_planes == 2 && !g.one_cta && !simt_debug))
+        return EMC_ERR_UNSUPPORTED;                              // the Gaussian statistics exist in the pair kernel only
     if (g.n_planes == 2 && !g.one_cta) {
         // CTA pairs; tile width by wave quantisation: time ~ waves(BN) x BN (one pair per TPC, tiles of equal cost)
         const int mt = ceil_div(g.M, PAIR_M), pairs = num_sms() / 2;
         const long c256 = (long)ceil_div(mt * ceil_div(g.N, 256), pairs) * 256;
         const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), pairs) * 192;
+        if (g.stat_m && g.epilogue == EPI_GAUSS)
+            return c192 < c256 ? launch_tc_pair<2, 192, 4, 2>(g, st) : launch_tc_pair<2, 256, 4, 2>(g, st);
         if (g.stat_m)
-            return c192 < c256 ? launch_tc_pair<2, 192, 4, true>(g, st) : launch_tc_pair<2, 256, 4, true>(g, st);
-        return c192 < c256 ? launch_tc_pair<2, 192, 4, false>(g, st) : launch_tc_pair<2, 256, 4, false>(g, st);
+            return c192 < c256 ? launch_tc_pair<2, 192, 4, 1>(g, st) : launch_tc_pair<2, 256, 4, 1>(g, st);
+        return c192 < c256 ? launch_tc_pair<2, 192, 4, 0>(g, st) : launch_tc_pair<2, 256, 4, 0>(g, st);
     }
     if (g.n_planes == 2) {
         // tile width by wave quantisation: time ~ waves(BN) x BN (one CTA per SM, tiles of equal cost)

@@ -65,13 +65,14 @@ enum PlaneFormat { FMT_F16 = 0, FMT_BF16 = 1 };   // = the UMMA instruction desc
 
 // ---------------------------------------------------------------- stage launchers (device work)
 // Expand (emc_expand.cu).  Any of W, idx, planes may be null.  planes = [2][R][ld_p] fp16 (hi, lo)
-// of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).
+// of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).  gauss: the planes
+// hold W itself and S[r] += sum_{p:mask} W^2 (the operands of the paper's Gaussian model).
 // `blocked` = scratch of expand_scratch_floats(n, n_pix) floats (blocked model copies + packed geometry; then W / idx
 // or planes, not both), or null (plain gathers).
 size_t expand_scratch_floats(int n, int n_pix);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, cudaStream_t st);
+                         int ld_p, float *S, float *blocked, cudaStream_t st, bool gauss = false);
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
@@ -81,6 +82,9 @@ emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
                        const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
                        WsHeader *hdr, cudaStream_t st);
+
+// A[d] = sum_p Kc[d][p]^2 (fluence numerators of the Gaussian model, eq. 2.6)
+emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float *Asq, cudaStream_t st);
 
 // Plane GEMM on tcgen05 (emc_gemm.cu):  acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
 struct GemmProblem {
@@ -104,25 +108,47 @@ struct GemmProblem {
     float *stat_m = nullptr, *stat_w = nullptr, *stat_z = nullptr;
     int ld_stat = 0;
     const float *weight = nullptr;
+    const float *gauss_a = nullptr;   // EPI_GAUSS: [N] A_d = sum_p K[d,p]^2
+    float inv2s2 = 0.f;               // EPI_GAUSS: 1 / (2 sigma^2)
     bool one_cta = false;   // EMC_GEMM_1CTA: the one-CTA kernel instead of CTA pairs (cta_group::2)
 };
 enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-likelihood)
        EPI_STORE = 1,       // out = acc                                (raw update numerator)
        EPI_ADD = 2,         // out += acc                               (numerator over chunks)
-       EPI_DIV_ROW = 3 };   // out = rowv[m] > 0 ? acc / rowv[m] : 0    (eq. 2.5)
+       EPI_DIV_ROW = 3,     // out = rowv[m] > 0 ? acc / rowv[m] : 0    (eq. 2.5)
+       EPI_GAUSS = 4 };     // out = acc = B; rowv = C, gauss_a = A: statistics of Q = (B^2/A - C) / (2 sigma^2)
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st);
 // true if launch_plane_gemm(g, simt_debug, .) fills g.stat_m / g.stat_z
 bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug);
 
+// Gaussian model (eqs. 2.2, 2.3, 2.6): with phi = A_d / B_rd,  Q_rd = (B_rd^2 / A_d - C_r) / (2 sigma^2)
+//   = B^2 g_d + (-C_r / (2 sigma^2)),  g_d = 1 / (2 sigma^2 A_d)  (0 for a frame without photons).
+// The GEMM epilogue (statistics) and normalize_kernel (second sweep) must form the two terms BIT-IDENTICALLY, hence
+// explicit single-rounding intrinsics that the compiler cannot contract differently in the two kernels.
+#ifdef __CUDACC__
+__device__ __forceinline__ float gauss_col_factor(float a_col, float inv2s2) {
+    return a_col > 0.f ? __fdiv_rn(inv2s2, a_col) : 0.f;
+}
+__device__ __forceinline__ float gauss_elem_term(float b, float g_col) { return __fmul_rn(__fmul_rn(b, b), g_col); }
+__device__ __forceinline__ float gauss_row_term(float log_w, float c_row, float inv2s2) {
+    return __fsub_rn(log_w, __fmul_rn(c_row, inv2s2));
+}
+#endif
+
 // Normalise (emc_normalize.cu).  scratch = normalize_scratch_floats() floats.  `planes` (optional) receives the
 // operand planes of P for the update GEMM: two fp16 planes scaled per (row, 512-column chunk) with the inverse
 // scales in chunk_inv_scale [ceil(ld_n/512)][R], or (bf16x3) three unscaled bf16 planes.
+// Gaussian model: L holds B = W K^T; c_row [R] = sum_p W^2, a_col [N] = sum_p K^2, inv2s2 = 1 / (2 sigma^2)
+struct GaussTerms {
+    const float *c_row, *a_col;
+    float inv2s2;
+};
 size_t normalize_scratch_floats(int n_rot, int ld_n);
 int normalize_stat_rows(int n_rot);   // scratch = part_m, part_w, part_z [rows][ld_n] each, then col_m, col_w, col_iz [ld_n] each
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st);
+                            cudaStream_t st, const GaussTerms *gauss = nullptr);
 // operand planes of a given P (stage API of emc_update).
 emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);

@@ -339,6 +339,64 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
     }
 }
 
+// Second sweep for the paper's Gaussian model (NEXT-3): the "L" buffer holds B[r,d] = sum_p W K.
+//   Q = B^2 g_d + (log w_r - C_r / (2 sigma^2))   (same two terms, bit for bit, as the GEMM's statistics),
+//   P = exp((B^2 g_d - mL_d) + (lw'_r - mw_d)) / z_d,   update operand = P / phi = P B / A_d   (eq. 2.11).
+// Same thread layout as normalize_kernel; column data is re-read per row (L1-resident) to keep registers free.
+__global__ void __launch_bounds__(kThreads, 2)
+normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ weight, const float *__restrict__ c_row,
+                       const float *__restrict__ a_col, float inv2s2, int n_rot, int n_pat, int ld_n, int rows_per_split,
+                       const float *__restrict__ col_m, const float *__restrict__ col_w, const float *__restrict__ col_iz,
+                       float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                       float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int d0 = blockIdx.x * kChunkCols;
+    const int r_lo = blockIdx.y * rows_per_split;
+    const int r_hi = min(n_rot, r_lo + rows_per_split);
+    const float log_uniform = -logf((float)n_rot);
+    for (int r = r_lo + warp; r < r_hi; r += kWarps) {
+        const float lw = gauss_row_term(weight ? logf(weight[r]) : log_uniform, c_row[r], inv2s2);
+        const size_t row_off = (size_t)r * ld_n;
+        float p[kGroups][4], q[kGroups][4];
+        float sum = 0.f;
+#pragma unroll
+        for (int g = 0; g < kGroups; ++g) {
+            const int d = d0 + g * kColsPerBlock + lane * kVec;
+            const bool ok = d < n_pat;                      // ld_n is a multiple of 4: whole float4s
+            const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 b4 = ok ? *reinterpret_cast<const float4 *>(B + row_off + d) : z4;
+            const float4 m4 = ok ? *reinterpret_cast<const float4 *>(col_m + d) : z4;
+            const float4 w4 = ok ? *reinterpret_cast<const float4 *>(col_w + d) : z4;
+            const float4 i4 = ok ? *reinterpret_cast<const float4 *>(col_iz + d) : z4;
+            const float4 a4 = ok ? *reinterpret_cast<const float4 *>(a_col + d) : z4;
+            const float bb[4] = {b4.x, b4.y, b4.z, b4.w}, mm[4] = {m4.x, m4.y, m4.z, m4.w};
+            const float ww[4] = {w4.x, w4.y, w4.z, w4.w}, ii[4] = {i4.x, i4.y, i4.z, i4.w};
+            const float aa[4] = {a4.x, a4.y, a4.z, a4.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float pj = 0.f, qj = 0.f;
+                if (d + j < n_pat) {
+                    const float e = gauss_elem_term(bb[j], gauss_col_factor(aa[j], inv2s2));
+                    pj = expf((e - mm[j]) + (lw - ww[j])) * ii[j];
+                    if (pj < EMC_P_MIN) pj = 0.f;                      // DESIGN.md §3 G20
+                    qj = aa[j] > 0.f ? pj * (bb[j] / aa[j]) : 0.f;     // P / phi, phi = A / B (GA3: no photons -> 0)
+                }
+                p[g][j] = pj;
+                q[g][j] = qj;
+                sum += pj;
+            }
+            if (P && ok) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
+        }
+        if (planes)
+            write_planes(q, d0, lane, ld_n, row_off, planes, bf16x3, plane_stride,
+                         chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
+        if (s) {
+            sum = warp_sum(sum);
+            if (lane == 0) atomicAdd(s + r, sum);
+        }
+    }
+}
+
 // operand planes of a given P (stage API of emc_update).  grid = (ceil(N/512), ceil(R/8)); warp per row.
 __global__ void __launch_bounds__(kThreads)
 p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, void *__restrict__ planes, int ld_pl,
@@ -387,7 +445,8 @@ size_t normalize_scratch_floats(int n_rot, int ld_n) {
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st) {
+                            cudaStream_t st, const GaussTerms *gauss) {
+    if (gauss && !stats_ready) return EMC_ERR_UNSUPPORTED;       // the Gaussian model's statistics come from the GEMM
     const int stat_rows = normalize_stat_rows(n_rot);
     float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
     if (!accumulate) {
@@ -418,7 +477,11 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     if (splits2 < 1) splits2 = 1;
     const int rows2 = ceil_div(n_rot, splits2);
     const dim3 grid2(chunks, ceil_div(n_rot, rows2));
-    if (weight)
+    if (gauss)
+        normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->a_col, gauss->inv2s2, n_rot, n_pat,
+                                                           ld_n, rows2, col_m, col_w, col_iz, P, planes, bf16x3 ? 1 : 0,
+                                                           plane_stride, chunk_inv_scale, s);
+    else if (weight)
         normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_w, col_iz, P,
                                                             planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
     else

@@ -54,7 +54,36 @@ pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *_
     if ((threadIdx.x & 31) == 0 && vmax > (kt_bf16 ? 256 : EMC_MAX_COUNT)) atomicMax(&hdr->max_count, vmax);
 }
 
+// A[d] = sum_{p: mask} K[d,p]^2 from the packed counts (masked pixels are already 0): the numerator of the
+// fluence, eq. (2.6).  One warp per pattern; counts <= 2048 are exact in float and so are the squares.
+__global__ void __launch_bounds__(256)
+rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, float *__restrict__ Asq) {
+    const int d = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (d >= n_pat) return;
+    const __half *row = Kc + (size_t)d * ld_p;
+    float t = 0.f;
+    for (int p = lane * 8; p < n_pix; p += 256) {              // ld_p is a multiple of 64: 16-byte loads stay in the row
+        const uint4 v = *reinterpret_cast<const uint4 *>(row + p);
+        const __half2 *h = reinterpret_cast<const __half2 *>(&v);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float2 f = __half22float2(h[j]);
+            if (p + 2 * j < n_pix) t += f.x * f.x;
+            if (p + 2 * j + 1 < n_pix) t += f.y * f.y;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) Asq[d] = t;
+}
+
 }  // namespace
+
+emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float *Asq, cudaStream_t st) {
+    rowsq_kernel<<<ceil_div(n_pat, 8), 256, 0, st>>>(Kc, n_pat, n_pix, ld_p, Asq);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
 
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
                        const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,

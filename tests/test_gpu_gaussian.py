@@ -1,0 +1,63 @@
+"""Parity of emc_iterate_gaussian (the paper's Gaussian likelihood with fluence, eqs. 2.2-2.6; DESIGN.md section 11
+NEXT-3) with the oracle, which evaluates eq. (2.2) term by term in float64.  (`-m gpu`)
+
+Tolerances: Q is not exposed by the C ABI (the kernels carry B = sum_p W K), so the E-step is checked through
+P: |dP| <= 1e-6 + 2 P_ref max_r |dQ| with |dQ| <= 1e-5 A[r,d], A = sum_p ((K/phi)^2 + W^2) / (2 sigma^2) (the scale
+of the float32 terms Q is the difference of; same form as T1/T2 of the Poisson path); LL relative 1e-5 of the scale
+sum_d max_r A; model' as in the Poisson end-to-end test."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+@pytest.mark.parametrize("name,sigma", [("T1", 20.0), ("T1", 5.0), ("T2", 10.0), ("C1", 30.0)])
+@pytest.mark.parametrize("weighted", [True, False], ids=["eq2.12", "eq2.10"])
+def test_iterate_gaussian_matches_oracle(inputs_cache, name, sigma, weighted):
+    inp = inputs_cache(name)
+    stage = len(inp.quat) - 1
+    quat, weight = inp.quat[stage], inp.weight[stage]
+    if name == "T2":                                         # non-uniform prior weights
+        rng = np.random.default_rng(3)
+        weight = rng.uniform(0.5, 1.5, size=weight.shape).astype(np.float32)
+        weight /= weight.sum()
+    ref = o.iterate_gaussian(inp.model_init, inp.q, inp.mask, quat, weight, inp.counts, sigma, weighted=weighted)
+    flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
+    out = emc.emc_iterate_gaussian(dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(quat), dev(weight),
+                                   dev(inp.counts), sigma, flags=flags, want_p=True)
+    emc.emc_check(out["ws"])
+    p = out["P"].cpu().numpy()
+    dq = 1e-5 * ref["A"].max(axis=0)                         # per column
+    bound = 1e-6 + 2.0 * ref["P"] * dq[None, :]
+    assert np.all(np.abs(p - ref["P"]) <= bound), f"max dP {np.abs(p - ref['P']).max():.3e}"
+    assert np.abs(p.sum(axis=0) - 1).max() <= 1e-5
+    ll = float(out["loglik"].cpu()[0])
+    assert abs(ll - ref["LL"]) <= dq.sum(), (ll, ref["LL"])
+    m, m_ref = out["model"].cpu().numpy().reshape(-1), ref["model"].reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    rel = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-6 * np.abs(m_ref).max())
+    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2, f"model rel: median {np.median(rel):.2e} max {rel.max():.2e}"
+
+
+def test_gaussian_multi_iteration_and_arguments(inputs_cache):
+    inp = inputs_cache("T1")
+    args = (dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]), dev(inp.counts))
+    a = emc.emc_iterate_gaussian(*args, 10.0, n_iter=2)
+    m = args[0]
+    lls = []
+    for _ in range(2):
+        out = emc.emc_iterate_gaussian(m, *args[1:], 10.0)
+        m = out["model"]
+        lls.append(float(out["loglik"].cpu()[0]))
+    assert np.allclose(a["loglik"].cpu().numpy(), lls, rtol=1e-6)
+    with pytest.raises(emc.EmcError):
+        emc.emc_iterate_gaussian(*args, 0.0)
