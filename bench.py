@@ -101,8 +101,8 @@ def oracle_sample(inp, stage, n_rot_s, n_pat_s):
 
 def sample_sizes(cfg):
     """Bounded sample: about 10-30 s of oracle work on a few host cores."""
-    budget = 4.0e11                                         # multiply-adds of the three float64 matmuls
-    n_rot_s = min(max(cfg.n_rot), 2048)
+    budget = 1.2e12                                         # multiply-adds of the three float64 matmuls
+    n_rot_s = min(max(cfg.n_rot), 6144)
     n_pat_s = int(max(64, min(cfg.n_pat, budget / (3.0 * n_rot_s * cfg.n_pix))))
     return n_rot_s, n_pat_s
 
