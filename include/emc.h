@@ -57,8 +57,9 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
 #define EMC_MAX_COUNT 2048
 
 /* Responsibilities below 2^-100 are stored as 0 (DESIGN.md §3 G20): float32 P keeps full relative
- * precision only down to there once it is split into three bf16 planes, and a rotation whose whole
- * row lies below it has no data behind it (s[r] = 0: W'[r,:] = 0, slice skipped by Compress, G17). */
+ * precision only down to there once it is split into 16-bit operand planes for the update contraction,
+ * and a rotation whose whole row lies below it has no data behind it (s[r] = 0: W'[r,:] = 0, slice
+ * skipped by Compress, G17). */
 #define EMC_P_MIN 7.888609052210118e-31f
 
 /* flags */

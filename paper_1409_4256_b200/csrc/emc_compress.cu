@@ -5,10 +5,13 @@
 //
 // with the same trilinear weights f and the same pinned sample geometry as Expand.
 //
-// Measured on B200 (DESIGN.md §7 "Compress"): a global reduction costs the SM about 1.3 cycles per lane when the
-// lanes of a warp hit unrelated sectors and 0.8 when they are contiguous; 16 bytes per lane is the widest there
-// is.  So the design (a) moves a sample's 8 corners x (num, den) = 64 bytes in four 16-byte
-// red.global.add.v4.f32, and (b) makes those 64 bytes CONTIGUOUS and lets four adjacent lanes issue them in
+// Measured on B200 (DESIGN.md §7 "Compress"): what bounds the scatter is the chip's rate of fp32 reductions into
+// L2, which depends on how the bytes are grouped: 64 bytes per sample as four unrelated 16-byte reductions cost
+// 347 us per 2e7 samples, as ONE contiguous 64-byte group issued by four adjacent lanes 224 us (and a
+// cp.reduce.async.bulk of the same 64 bytes, or any mix of the two, the same 225 us); shared-memory atomics are
+// slower than all of them.  So the design (a) moves a sample's 8 corners x (num, den) = 64 bytes in four 16-byte
+// red.global.add.v4.f32 (16 bytes per lane is the widest reduction there is), and (b) makes those 64 bytes
+// CONTIGUOUS and lets four adjacent lanes issue them in
 // one instruction: the accumulator is not a voxel grid but 8 staggered grids of 2x2x2 blocks, one per parity
 // (b_x&1, b_y&1, b_z&1) of the base corner; grid c holds, for every base of that parity, one aligned 64-byte
 // block {num, den} x corner (4 dx + 2 dy + dz), blocks ordered [b_x/2][b_y/2][b_z/2].  After computing its

@@ -11,13 +11,19 @@
 //
 //        acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
 //
-// Kernel: persistent, one CTA per SM, warp-specialised.
+// Kernels: persistent, warp-specialised.
 //   warp 0 lane 0 : TMA producer  (cp.async.bulk.tensor -> 128B-swizzled smem ring, mbarrier tx)
-//   warp 1 lane 0 : MMA issuer    (tcgen05.mma.cta_group::1.kind::f16, 128 x BN x 16, fp32 in TMEM)
-//   warps 2..9    : epilogue      (tcgen05.ld 32x32b -> fp32 register accumulators -> fused row op -> global)
+//   warp 1 lane 0 : MMA issuer    (tcgen05.mma.kind::f16, fp32 accumulators in TMEM)
+//   warps 2..9    : epilogue      (tcgen05.ld 32x32b -> fp32 register accumulators -> fused row op -> out)
 // TMEM holds two accumulator stages of BN columns; the K loop alternates between them in chunks
 // of 512 elements so that the long sums are carried in round-to-nearest fp32 registers (tcgen05
 // accumulation truncates), and the drain of chunk i overlaps the MMAs of chunk i+1.
+//   plane_gemm_pair_kernel : the product path.  One CTA PAIR per 256 x BN tile (cta_group::2), results leave
+//                            through swizzled staging tiles and TMA stores, the log-likelihood variant also writes
+//                            the normalisation's column statistics (tile_out).
+//   plane_gemm_kernel      : one CTA per 128 x BN tile (cta_group::1), per-lane stores; EMC_GEMM_1CTA, a
+//                            comparison / bisecting aid.
+//   simt_plane_gemm_kernel : plain CUDA cores; EMC_DEBUG_SIMT.
 #include "emc_internal.cuh"
 
 namespace emc {

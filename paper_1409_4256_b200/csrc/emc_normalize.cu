@@ -4,10 +4,13 @@
 //
 //   a[r,d] = L[r,d] + log w_r;   m_d = max_r a;   P[r,d] = exp(a - m_d) / sum_r exp(a - m_d)
 //
-// Two sweeps over L (column-wise reductions on a row-major matrix): (1) per-column online
-// (max, sum) in warp-shuffle-free lane-per-column form, split over row ranges for parallelism;
-// (2) write P, its operand planes for the update GEMM, s[r] = sum_d P[r,d] and the total
-// log-likelihood.  HBM-bound: 8 algorithmic bytes per (r,d).
+// Two sweeps (column-wise reductions on a row-major matrix):
+// (1) per-column statistics (ColStat below) as partials over row ranges.  Inside emc_iterate they come from the
+//     log-likelihood GEMM's epilogue, one partial per 32 rotations, and L is never read for them; the stage API
+//     emc_normalize, which is handed an arbitrary L, uses colstats_kernel.  colstats_combine_kernel merges the
+//     partials per column and adds up the total log-likelihood.
+// (2) normalize_kernel reads L once and writes P, its operand planes for the update GEMM and s[r] = sum_d P[r,d].
+// HBM-bound: 8 algorithmic bytes per (r,d).
 #include "emc_internal.cuh"
 
 namespace emc {
