@@ -295,11 +295,24 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
 
     EMC_TRY(reset_header(l, st));
-    // pack jobs in order: every (iteration, chunk) when there are several chunks, else the one resident chunk once
-    const int n_jobs = n_chunks > 1 ? n_iter * n_chunks : 1;
+    // Host-resident patterns in ONE resident chunk: the first iteration is run on sub-ranges of the chunk, so that the
+    // copy of sub-range j + 1 crosses PCIe while sub-range j is packed (into its place in the full-size operands)
+    // and goes through stages 2-4; later iterations use the resident operands in one piece.  Same arithmetic as
+    // pattern chunks (G9).  Sub-ranges are multiples of 512 patterns (the update's K chunk and scale granularity).
+    const bool pipelined = on_host && n_chunks == 1 && !gauss && n_pat >= 4096;
+    const int sub = pipelined ? (int)round_up((size_t)ceil_div(n_pat, 4), 512) : chunk;
+    const int n_sub = pipelined ? ceil_div(n_pat, sub) : 1;
+    // pack jobs in order: every (iteration, chunk) when there are several chunks, else the resident chunk once
+    // (in n_sub pieces when pipelined)
+    const int n_jobs = n_chunks > 1 ? n_iter * n_chunks : n_sub;
+    auto job_range = [&](int j, int &d0, int &nc) {
+        const int step = pipelined ? sub : chunk;
+        d0 = (pipelined ? j : j % n_chunks) * step;
+        nc = n_pat - d0 < step ? n_pat - d0 : step;
+    };
     auto issue_copy = [&](int j) -> emc_status {              // host -> staging buffer j & 1, on the side stream
-        const int c = j % n_chunks, d0 = c * chunk;
-        const int nc = n_pat - d0 < chunk ? n_pat - d0 : chunk;
+        int d0, nc;
+        job_range(j, d0, nc);
         const int b = j & 1;
         if (j >= 2) EMC_TRY_CUDA(cudaStreamWaitEvent(g_copy.stream, g_copy.freed[b], 0));   // pack j - 2 has read it
         EMC_TRY_CUDA(cudaMemcpyAsync((uint8_t *)l.stage + b * stage_one, (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz,
@@ -325,19 +338,33 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
-        for (int c = 0; c < n_chunks; ++c) {
-            const int d0 = c * chunk;
-            const int nc = n_pat - d0 < chunk ? n_pat - d0 : chunk;
+        // the parts of this iteration: pattern chunks (each in the per-chunk buffers), or, in the pipelined first
+        // iteration, sub-ranges of the one resident chunk (each at its offset in the full-size buffers)
+        const bool sub_ranges = pipelined && it == 0;
+        const int n_parts = sub_ranges ? n_sub : n_chunks;
+        for (int c = 0; c < n_parts; ++c) {
+            const int step = sub_ranges ? sub : chunk;
+            const int d0 = c * step;
+            const int nc = n_pat - d0 < step ? n_pat - d0 : step;
+            Layout v = l;                               // view of the buffers this part works in
+            if (sub_ranges) {
+                v.Kc = l.Kc + (size_t)d0 * l.ld_p;
+                v.KT = (uint16_t *)l.KT + d0;
+                v.L = l.L + d0;
+                v.planesP = (uint16_t *)l.planesP + d0;
+                v.pscale = l.pscale + (size_t)(d0 / 512) * n_rot;
+                v.scratch = l.scratch + d0;
+            }
             if (n_chunks > 1 || it == 0) {          // one resident chunk is packed once for all iterations
                 Span sp(prof, EMC_STAGE_PACK, st);
                 const uint8_t *src = (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz;
                 if (on_host) {
                     const int b = job & 1;
-                    if (job + 1 < n_jobs) EMC_TRY(issue_copy(job + 1));      // overlaps this chunk's pack and GEMMs
+                    if (job + 1 < n_jobs) EMC_TRY(issue_copy(job + 1));      // overlaps this part's pack and GEMMs
                     EMC_TRY_CUDA(cudaStreamWaitEvent(st, g_copy.ready[b], 0));
                     src = (const uint8_t *)l.stage + b * stage_one;
                 }
-                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, l.Kc, l.ld_p, l.KT, bf16x3, l.ld_n, l.hdr, st));
+                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, bf16x3, l.ld_n, l.hdr, st));
                 if (on_host) EMC_TRY_CUDA(cudaEventRecord(g_copy.freed[job & 1], st));
                 if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
                     EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * l.ld_n, st));
@@ -349,24 +376,24 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
             bool stats_ready = false;
             {
                 Span sp(prof, EMC_STAGE_LOGLIK, st);
-                EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, nc, l.L, l.ld_n, flags, st, rot->weight, &stats_ready, gt));
+                EMC_TRY(run_loglik_gemm(v, n_rot, n_pix, nc, v.L, l.ld_n, flags, st, rot->weight, &stats_ready, gt));
             }
-            // stage 3: responsibilities of this chunk; s and LL add up over chunks
-            float *p_dst = (P_out && it == n_iter - 1) ? P_out : nullptr;
+            // stage 3: responsibilities of this part; s and LL add up over parts
+            float *p_dst = (P_out && it == n_iter - 1) ? P_out + (sub_ranges ? d0 : 0) : nullptr;
             {
                 Span sp(prof, EMC_STAGE_NORMALIZE, st);
-                EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_dst, l.planesP, bf16x3,
-                                         (size_t)n_rot * l.ld_n, l.pscale, l.s, loglik + it, true, l.scratch, stats_ready,
-                                         st, gt));
+                EMC_TRY(launch_normalize(v.L, rot->weight, n_rot, nc, l.ld_n, p_dst, v.planesP, bf16x3,
+                                         (size_t)n_rot * l.ld_n, v.pscale, l.s, loglik + it, true, v.scratch, stats_ready,
+                                         st, gt, l.ld_n - (sub_ranges ? d0 : 0)));
             }
-            // stage 4: update numerators (divided by s[r] in the epilogue when there is one chunk)
-            const int epi = n_chunks == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
+            // stage 4: update numerators (divided by s[r] in the epilogue when there is one part)
+            const int epi = n_parts == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
             {
                 Span sp(prof, EMC_STAGE_UPDATE, st);
-                EMC_TRY(run_update_gemm(l, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, flags, st));
+                EMC_TRY(run_update_gemm(v, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, flags, st));
             }
         }
-        if (n_chunks > 1) {
+        if (n_parts > 1) {
             Span sp(prof, EMC_STAGE_UPDATE, st);
             EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
         }

@@ -148,7 +148,9 @@ int normalize_stat_rows(int n_rot);   // scratch = part_m, part_w, part_z [rows]
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss = nullptr);
+                            cudaStream_t st, const GaussTerms *gauss = nullptr, int n_store = 0);
+// n_store: columns of a row the call may write (planes padding, column arrays); 0 = ld_n.  Smaller when L, planes and
+// scratch are views that start inside a row (emc_api.cu, pipelined first iteration).
 // operand planes of a given P (stage API of emc_update).
 emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);

@@ -223,7 +223,7 @@ __device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int
 // partials k = y, y + 8, ... online, then the 8 are merged through shared memory.
 __global__ void __launch_bounds__(256)
 colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_w,
-                        const float *__restrict__ part_z, int n_pat, int ld_n, int n_splits,
+                        const float *__restrict__ part_z, int n_pat, int ld_n, int n_store, int n_splits,
                         float *__restrict__ col_m, float *__restrict__ col_w, float *__restrict__ col_iz,
                         double *__restrict__ loglik) {
     __shared__ float sm_m[8][32], sm_w[8][32], sm_z[8][32];
@@ -256,7 +256,7 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
         col_w[d] = t.mw;
         col_iz[d] = 1.f / t.z;
         ll = ((double)t.mL + (double)t.mw) + (double)logf(t.z);
-    } else if (d < ld_n) {
+    } else if (d < n_store) {
         col_m[d] = 0.f;
         col_w[d] = 0.f;
         col_iz[d] = 0.f;
@@ -274,7 +274,7 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
 template <bool UNIFORM>
 __global__ void __launch_bounds__(kThreads, UNIFORM ? 3 : 2)
 normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
-                 int ld_n, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_w,
+                 int ld_n, int n_store, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_w,
                  const float *__restrict__ col_iz, float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
                  float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -333,7 +333,7 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
             if (P && ok[g]) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
         }
         if (planes)
-            write_planes(p, d0, lane, ld_n, row_off, planes, bf16x3, plane_stride,
+            write_planes(p, d0, lane, n_store, row_off, planes, bf16x3, plane_stride,
                          chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
         if (s) {
             sum = warp_sum(sum);
@@ -348,7 +348,8 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
 // Same thread layout as normalize_kernel; column data is re-read per row (L1-resident) to keep registers free.
 __global__ void __launch_bounds__(kThreads, 2)
 normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ weight, const float *__restrict__ c_row,
-                       const float *__restrict__ a_col, float inv2s2, int n_rot, int n_pat, int ld_n, int rows_per_split,
+                       const float *__restrict__ a_col, float inv2s2, int n_rot, int n_pat, int ld_n, int n_store,
+                       int rows_per_split,
                        const float *__restrict__ col_m, const float *__restrict__ col_w, const float *__restrict__ col_iz,
                        float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
                        float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
@@ -391,7 +392,7 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
             if (P && ok) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
         }
         if (planes)
-            write_planes(q, d0, lane, ld_n, row_off, planes, bf16x3, plane_stride,
+            write_planes(q, d0, lane, n_store, row_off, planes, bf16x3, plane_stride,
                          chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
         if (s) {
             sum = warp_sum(sum);
@@ -448,7 +449,8 @@ size_t normalize_scratch_floats(int n_rot, int ld_n) {
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss) {
+                            cudaStream_t st, const GaussTerms *gauss, int n_store) {
+    if (n_store <= 0 || n_store > ld_n) n_store = ld_n;          // columns of a row this call may write
     if (gauss && !stats_ready) return EMC_ERR_UNSUPPORTED;       // the Gaussian model's statistics come from the GEMM
     const int stat_rows = normalize_stat_rows(n_rot);
     float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
@@ -469,7 +471,7 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
         EMC_LAUNCHED();
     }
     float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
-    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_splits, col_m,
+    colstats_combine_kernel<<<ceil_div(n_store, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_store, n_splits, col_m,
                                                                  col_w, col_iz, loglik);
     EMC_LAUNCHED();
     // second sweep: 512-column chunks; enough row splits for about six resident blocks per SM
@@ -482,13 +484,13 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     const dim3 grid2(chunks, ceil_div(n_rot, rows2));
     if (gauss)
         normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->a_col, gauss->inv2s2, n_rot, n_pat,
-                                                           ld_n, rows2, col_m, col_w, col_iz, P, planes, bf16x3 ? 1 : 0,
+                                                           ld_n, n_store, rows2, col_m, col_w, col_iz, P, planes, bf16x3 ? 1 : 0,
                                                            plane_stride, chunk_inv_scale, s);
     else if (weight)
-        normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_w, col_iz, P,
+        normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, n_store, rows2, col_m, col_w, col_iz, P,
                                                             planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
     else
-        normalize_kernel<true><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows2, col_m, col_w, col_iz, P,
+        normalize_kernel<true><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, n_store, rows2, col_m, col_w, col_iz, P,
                                                            planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
     EMC_LAUNCHED();
     return EMC_OK;

@@ -215,3 +215,24 @@ def test_degenerate_sizes(inputs_cache):
     r = o.iterate(inp.model_init, inp.q, inp.mask, c.quat[:1], np.ones(1, np.float32), inp.counts[:1])
     cov = r["den"] > 0
     assert np.allclose(host(out["model"]).reshape(-1)[cov], r["model"].reshape(-1)[cov], rtol=1e-4, atol=1e-7)
+
+
+def test_host_patterns_pipelined_first_iteration(inputs_cache):
+    """N >= 4096 host-resident patterns in one chunk: the first iteration runs on four sub-ranges (ragged last one)
+    while the copies are in flight; results = the device-resident run up to summation order."""
+    inp = inputs_cache("T1", n_pat=4200)
+    c = Case(inp)
+    pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
+    for n_iter in (1, 2):
+        a = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=n_iter, want_p=True)
+        h = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, n_iter=n_iter, want_p=True,
+                            flags=emc.EMC_PATTERNS_ON_HOST)
+        emc.emc_check(h["ws"])
+        ma, mh = host(a["model"]), host(h["model"])
+        assert np.abs(ma - mh).max() <= 1e-5 * np.abs(ma).max()
+        assert np.allclose(host(a["loglik"]), host(h["loglik"]), rtol=1e-6)
+        assert np.abs(host(a["P"]) - host(h["P"])).max() <= (1e-6 if n_iter == 1 else 1e-4)
+    ref = o.iterate(inp.model_init, inp.q, inp.mask, c.quat, c.weight, inp.counts)
+    h1 = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, want_p=True,
+                         flags=emc.EMC_PATTERNS_ON_HOST)
+    assert abs(float(host(h1["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"])
