@@ -474,9 +474,10 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     colstats_combine_kernel<<<ceil_div(n_store, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_store, n_splits, col_m,
                                                                  col_w, col_iz, loglik);
     EMC_LAUNCHED();
-    // second sweep: 512-column chunks; enough row splits for about six resident blocks per SM
+    // second sweep: 512-column chunks; row splits so that the grid is at most 6 x 148 blocks = whole waves of the 2 or 3
+    // blocks per SM the kernels run at (one block more is a wave more: a quarter of the time at C2)
     const int chunks = ceil_div(n_pat, kChunkCols);
-    int splits2 = ceil_div(6 * 148, chunks);
+    int splits2 = (6 * 148) / chunks;
     const int cap2 = ceil_div(n_rot, 4 * kWarps);
     if (splits2 > cap2) splits2 = cap2;
     if (splits2 < 1) splits2 = 1;
