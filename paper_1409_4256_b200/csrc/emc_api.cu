@@ -89,6 +89,7 @@ struct Layout {
     float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
     float *Asq;               // [ld_n]        sum_p K^2 per pattern (Gaussian model)
+    uint32_t *active;         // [R/32 + 1]    slices den was accumulated for (+ the device flag), Compress
     void *stage;              // two chunks of raw counts (patterns on host, double-buffered)
     int ld_p, ld_n;
     size_t total;
@@ -110,10 +111,11 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.pscale = a.take<float>((size_t)ceil_div(l.ld_n, 512) * R);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
-    l.acc = a.take<float2>((size_t)8 * n * n * n);
+    l.acc = a.take<float2>(compress_scratch_float2(n, n_pix));
     l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n, n_pix) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.Asq = a.take<float>((size_t)l.ld_n);
+    l.active = a.take<uint32_t>((size_t)ceil_div(n_rot, 32) + 1);
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
     return l;
@@ -260,7 +262,7 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
                         unsigned flags, void *ws, size_t ws_bytes, void *stream) {
     if (!Wnew || !det_ok(det) || !rot_ok(rot) || !model_out) return EMC_ERR_ARG;
     if (!sizes_ok(n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
-    const size_t need = round_up(sizeof(float2) * (size_t)8 * n * n * n, 1024);
+    const size_t need = round_up(sizeof(float2) * compress_scratch_float2(n, det->n_pix), 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
     return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, det->q, det->mask, det->n_pix,
                            rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);
@@ -400,8 +402,9 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         // stage 5: Compress
         {
             Span sp(prof, EMC_STAGE_COMPRESS, st);
+            const DenCache cache = {l.active, (int *)(l.active + ceil_div(n_rot, 32)), it == 0};
             EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
-                                    model_out, nullptr, st));
+                                    model_out, nullptr, st, &cache));
         }
         model_cur = model_out;
     }

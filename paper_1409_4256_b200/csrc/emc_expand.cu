@@ -228,6 +228,12 @@ logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
 
 static size_t expand_blocked_floats(int n) { return (size_t)8 * n * n * n; }
 // blocked model copies + one float4 of geometry per pixel
+emc_status launch_pack_geometry(const float *q, const uint8_t *mask, int n_pix, float4 *qm, cudaStream_t st) {
+    pack_geometry_kernel<<<ceil_div(n_pix, 256), 256, 0, st>>>(q, mask, n_pix, qm);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
 size_t expand_scratch_floats(int n, int n_pix) { return (n & 1) ? 0 : expand_blocked_floats(n) + (size_t)4 * n_pix; }
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,

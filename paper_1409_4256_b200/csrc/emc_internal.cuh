@@ -73,6 +73,8 @@ size_t expand_scratch_floats(int n, int n_pix);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
                          int ld_p, float *S, float *blocked, cudaStream_t st, bool gauss = false);
+// q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0)
+emc_status launch_pack_geometry(const float *q, const uint8_t *mask, int n_pix, float4 *qm, cudaStream_t st);
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
@@ -157,9 +159,19 @@ emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
 
-// Compress (emc_compress.cu).  acc = [8 G] float2 of scratch (8 staggered grids of corner blocks), zeroed inside.
+// Compress (emc_compress.cu).  acc = compress_scratch_float2(n, n_pix) float2 of scratch (8 staggered grids of corner
+// blocks + packed geometry), zeroed inside.
+size_t compress_scratch_float2(int n, int n_pix);
+// cache (optional, eq. 2.10 with slice_w only): den survives in `acc` from one call to the next and is reused while the
+// set {r: slice_w[r] > 0} stays the one in cache->active; force = accumulate it afresh (first iteration, new list).
+struct DenCache {
+    uint32_t *active;   // [ceil(R/32)] bit mask of the slices den was accumulated for
+    int *changed;       // device flag, scratch
+    bool force;
+};
 emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const float *q,
                            const uint8_t *mask, int n_pix, const float *quat, int n_rot, int n,
-                           float2 *acc, float *model_out, float *den_out, cudaStream_t st);
+                           float2 *acc, float *model_out, float *den_out, cudaStream_t st,
+                           const DenCache *cache = nullptr);
 
 }  // namespace emc
