@@ -169,8 +169,8 @@ def workload_name(cfg):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two contractions, from the one `ncu --set full`
-# capture of this build summarised in profiles/r01_v4_full_ncu.md (bytes; config:stage)
-NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 823.9e6, "C2:update": 899.0e6}
+# capture of this build summarised in profiles/r01_v5_full_ncu.md (bytes; config:stage)
+NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 827.5e6, "C2:update": 898.9e6}
 
 
 # ------------------------------------------------------------------------------ clocks
@@ -423,7 +423,7 @@ def main():
                                                                       % (ms * 1e-3) if sustained else
                                                                       "burst (timed region of %.0f ms, no power cap seen)" % ms),
                     avg_launch_ms=stage_ms[dom] / max(1, stage_spans[dom]),
-                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v4_full_ncu.md)",
+                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v5_full_ncu.md)",
                     note="achieved = 2*planes*R*N*P_eff flops per launch / CUDA-event launch time (issued MMA work of "
                          "the split scheme on unmasked pixels); useful TFLOP/s is in stages.  fp16 and bf16 share one "
                          "tensor rate; the count operand is >90 % zeros, which lowers switching power, so under the "
