@@ -1,0 +1,101 @@
+"""Degenerate and ragged cases of the whole iteration against the oracle (`-m gpu`): one rotation, one pattern,
+patterns without photons, a constant model (north_star's invariant: responsibilities equal the prior), a detector
+that is almost entirely masked, sizes below every tile, and rotation weights that are far from uniform."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from emc_inputs import CONFIGS, make_inputs
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def run_both(model, q, mask, quat, weight, counts, weighted=False):
+    ref = o.iterate(model, q, mask, quat, weight, counts, weighted=weighted)
+    _, ref["A"] = o.loglik(ref["W"], ref["idx"], counts, mask)
+    out = emc.emc_iterate(dev(model), dev(q), dev(mask), dev(quat), dev(weight), dev(counts), want_p=True,
+                          flags=emc.EMC_COMPRESS_WEIGHTED if weighted else 0)
+    emc.emc_check(out["ws"])
+    return ref, out
+
+
+def check(ref, out):
+    p = host(out["P"])
+    # end to end: |dP| <= 1e-6 + 2 P max_r |dL| with |dL| <= 2e-5 A (T2)
+    bound = 1e-6 + 2.0 * ref["P"] * (2e-5 * ref["A"].max(axis=0))[None, :]
+    assert np.all(np.abs(p - ref["P"]) <= bound), f"max dP {np.abs(p - ref['P']).max():.3e}"
+    assert abs(float(host(out["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"]) + 1e-6
+    m, m_ref = host(out["model"]).reshape(-1), ref["model"].reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    rel = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-6 * np.abs(m_ref).max())
+    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2
+    assert np.all(m[ref["den"] == 0] == 0)
+
+
+@pytest.fixture(scope="module")
+def t0():
+    return make_inputs("T0")
+
+
+def test_single_rotation(t0):
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0][:1], np.ones(1, np.float32), t0.counts)
+    assert np.all(host(out["P"]) == 1.0)                       # one rotation takes all the responsibility
+    check(ref, out)
+
+
+def test_single_pattern_and_empty_patterns(t0):
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], t0.weight[0], t0.counts[:1])
+    check(ref, out)
+    k = t0.counts.copy()
+    k[3] = 0                                                    # no photon at all: L = -S[r]
+    k[7, t0.mask.astype(bool)] = 0                              # photons only in masked pixels: the same
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], t0.weight[0], k)
+    check(ref, out)
+    p = host(out["P"])
+    assert np.abs(p[:, 3] - p[:, 7]).max() <= 1e-7
+
+
+def test_constant_model_gives_the_prior(t0):
+    rng = np.random.default_rng(2)
+    w = rng.uniform(0.2, 2.0, size=t0.weight[0].shape).astype(np.float32)
+    w /= w.sum()
+    model = np.full_like(t0.model_init, 0.37)
+    ref, out = run_both(model, t0.q, t0.mask, t0.quat[0], w, t0.counts)
+    p = host(out["P"])
+    assert np.abs(p - w[:, None]).max() <= 1e-6                 # every slice is the same: P[r,d] = w_r
+    check(ref, out)
+
+
+def test_almost_fully_masked_detector(t0):
+    mask = np.zeros_like(t0.mask)
+    mask[[5, 77, 200]] = 1
+    ref, out = run_both(t0.model_init, t0.q, mask, t0.quat[0], t0.weight[0], t0.counts, weighted=True)
+    check(ref, out)
+
+
+def test_sizes_below_every_tile():
+    cfg = dataclasses.replace(CONFIGS["T0"], name="T0s", n=8, n_det=6, n_rot=(3,), n_pat=5, n_pat_chunk=5)
+    inp = make_inputs(cfg)
+    ref, out = run_both(inp.model_init, inp.q, inp.mask, inp.quat[0], inp.weight[0], inp.counts)
+    check(ref, out)
+
+
+def test_extreme_prior_weights(t0):
+    w = np.full(t0.weight[0].shape, 1e-12, dtype=np.float32)
+    w[11] = 1.0
+    w /= w.sum()
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], w, t0.counts)
+    check(ref, out)
