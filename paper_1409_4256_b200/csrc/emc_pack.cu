@@ -54,6 +54,52 @@ pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *_
     if ((threadIdx.x & 31) == 0 && vmax > (kt_bf16 ? 256 : EMC_MAX_COUNT)) atomicMax(&hdr->max_count, vmax);
 }
 
+// uint16 counts with an even number of pixels (the configs' case): the same 64 x 64 tile, but every global access is
+// 4 bytes per lane (two adjacent pixels in, half2 out; two adjacent patterns per half2 on the transposed side), which
+// halves the instruction count of the 2-byte version above (it ran at 50 % issue, 22 % DRAM).
+__global__ void __launch_bounds__(256)
+pack_u16x2_kernel(const uint16_t *__restrict__ counts, int n_pat, int n_pix, const uint8_t *__restrict__ mask,
+                  __half *__restrict__ Kc, int ld_p, __half *__restrict__ KT, int ld_n, WsHeader *__restrict__ hdr) {
+    __shared__ float tile[kTile][kTile + 1];
+    const int p0 = blockIdx.x * kTile, d0 = blockIdx.y * kTile;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // 32 lanes x 2 pixels, 8 rows at a time
+    const int p = p0 + 2 * tx;
+    bool use0 = false, use1 = false;
+    if (p < n_pix) {                                           // n_pix even: p + 1 < n_pix too
+        use0 = mask ? mask[p] != 0 : true;
+        use1 = mask ? mask[p + 1] != 0 : true;
+    }
+    int vmax = 0;
+#pragma unroll
+    for (int j = ty; j < kTile; j += 8) {
+        const int d = d0 + j;
+        float v0 = 0.f, v1 = 0.f;
+        if (d < n_pat && p < n_pix) {
+            const uint32_t two = *reinterpret_cast<const uint32_t *>(counts + (size_t)d * n_pix + p);
+            const int c0 = (int)(two & 0xffffu), c1 = (int)(two >> 16);
+            if (use0) { vmax = max(vmax, c0); v0 = (float)c0; }
+            if (use1) { vmax = max(vmax, c1); v1 = (float)c1; }
+            if (Kc) *reinterpret_cast<__half2 *>(Kc + (size_t)d * ld_p + p) = __floats2half2_rn(v0, v1);
+        }
+        tile[j][2 * tx] = v0;
+        tile[j][2 * tx + 1] = v1;
+    }
+    __syncthreads();
+    if (KT) {
+        const int d = d0 + 2 * tx;
+#pragma unroll
+        for (int j = ty; j < kTile; j += 8) {
+            const int pp = p0 + j;
+            if (pp < n_pix && d < n_pat)                       // ld_n is even: the half2 stays inside the row
+                *reinterpret_cast<__half2 *>(KT + (size_t)pp * ld_n + d) =
+                    __floats2half2_rn(tile[2 * tx][j], d + 1 < n_pat ? tile[2 * tx + 1][j] : 0.f);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+    if ((threadIdx.x & 31) == 0 && vmax > EMC_MAX_COUNT) atomicMax(&hdr->max_count, vmax);
+}
+
 // A[d] = sum_{p: mask} K[d,p]^2 from the packed counts (masked pixels are already 0): the numerator of the
 // fluence, eq. (2.6).  One warp per pattern; counts <= 2048 are exact in float and so are the squares.
 __global__ void __launch_bounds__(256)
@@ -96,6 +142,11 @@ emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n
                                                        ld_p, KT, fb, ld_n, hdr);
             break;
         case EMC_U16:
+            if (!kt_bf16 && (n_pix & 1) == 0 && (((uintptr_t)counts) & 3) == 0) {
+                pack_u16x2_kernel<<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc, ld_p, (__half *)KT,
+                                                        ld_n, hdr);
+                break;
+            }
             pack_kernel<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc,
                                                         ld_p, KT, fb, ld_n, hdr);
             break;
