@@ -47,17 +47,17 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
 // active_check_kernel decides that on the device and the scatter kernel branches on its flag, so no host
 // synchronisation is needed (probe: 153 us against 224 us per 2e7 samples).
 
-// grid = ceil(R / (32 * 256)).  bits[r / 32] = mask of slices with s[r] > 0; *changed = 1 if it differs from the stored
-// mask (or force), else left as the caller zeroed it.
+// One thread per rotation, one warp per word: bits[r / 32] = mask of slices with s[r] > 0; *changed = 1 if it differs
+// from the stored mask (or force), else left as the caller zeroed it.
 __global__ void __launch_bounds__(256)
 active_check_kernel(const float *__restrict__ s, int n_rot, uint32_t *__restrict__ bits, int *__restrict__ changed,
                     int force) {
-    const int w = blockIdx.x * 256 + threadIdx.x;
-    if (w * 32 >= n_rot) return;
-    uint32_t m = 0;
-    for (int i = 0; i < 32 && w * 32 + i < n_rot; ++i) m |= (s[w * 32 + i] > 0.f ? 1u : 0u) << i;
-    if (force || bits[w] != m) *changed = 1;
-    bits[w] = m;
+    const int r = blockIdx.x * 256 + threadIdx.x;
+    const uint32_t m = __ballot_sync(0xffffffffu, r < n_rot && s[r] > 0.f);
+    if ((threadIdx.x & 31) == 0 && r < n_rot) {
+        if (force || bits[r >> 5] != m) *changed = 1;
+        bits[r >> 5] = m;
+    }
 }
 
 // zero the accumulators: everything if *changed, else only the num halves of the blocks
@@ -236,7 +236,7 @@ emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighte
         if (cache && slice_w && !weighted) {
             // den is reused while the set of skipped slices stays the one it was accumulated for (decided on the device)
             EMC_TRY_CUDA(cudaMemsetAsync(cache->changed, 0, sizeof(int), st));
-            active_check_kernel<<<ceil_div(ceil_div(n_rot, 32), 256), 256, 0, st>>>(slice_w, n_rot, cache->active,
+            active_check_kernel<<<ceil_div(n_rot, 256), 256, 0, st>>>(slice_w, n_rot, cache->active,
                                                                                  cache->changed, cache->force ? 1 : 0);
             EMC_LAUNCHED();
             compress_clear_kernel<<<(unsigned)((4 * g + 255) / 256), 256, 0, st>>>(acc4, g, cache->changed);   // g blocks of 64 B
