@@ -88,7 +88,7 @@ struct Layout {
     float2 *acc;              // [8 G]         8 staggered grids of 64-byte (num, den) corner blocks
     float *blocked;           // [8 G]         blocked staggered model copies (Expand)
     float *scratch;           // normalise partials
-    float *Asq;               // [ld_n]        sum_p K^2 per pattern (Gaussian model)
+    float *Asq;               // [2][ld_n]     1 / (2 sigma^2 A_d) and 1 / A_d, A_d = sum_p K^2 (Gaussian model)
     uint32_t *active;         // [R/32 + 1]    slices den was accumulated for (+ the device flag), Compress
     void *stage;              // two chunks of raw counts (patterns on host, double-buffered)
     int ld_p, ld_n;
@@ -114,7 +114,7 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.acc = a.take<float2>(compress_scratch_float2(n, n_pix));
     l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n, n_pix) : 0);
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
-    l.Asq = a.take<float>((size_t)l.ld_n);
+    l.Asq = a.take<float>((size_t)2 * l.ld_n);
     l.active = a.take<uint32_t>((size_t)ceil_div(n_rot, 32) + 1);
     l.stage = a.take<uint8_t>(stage_bytes);
     l.total = a.off;
@@ -153,7 +153,7 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     g.lda = l.ld_p; g.ldb = l.ld_p; g.plane_stride = (size_t)n_rot * l.ld_p;
     g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
     g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = gauss ? EPI_GAUSS : EPI_SUB_ROW;
-    if (gauss) { g.gauss_a = gauss->a_col; g.inv2s2 = gauss->inv2s2; }
+    if (gauss) { g.gauss_g = gauss->g_col; g.inv2s2 = gauss->inv2s2; }
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     if (stats_ready) {
@@ -289,7 +289,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
     if (gauss && (n_chunks != 1 || (flags & (EMC_UPDATE_BF16X3 | EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
-    const GaussTerms gterms = {l.S, l.Asq, gauss ? 1.f / (2.f * sigma * sigma) : 0.f};
+    const GaussTerms gterms = {l.S, l.Asq, l.Asq + l.ld_n, gauss ? 1.f / (2.f * sigma * sigma) : 0.f};
     const GaussTerms *gt = gauss ? &gterms : nullptr;
     cudaStream_t st = (cudaStream_t)stream;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
@@ -369,8 +369,8 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, bf16x3, l.ld_n, l.hdr, st));
                 if (on_host) EMC_TRY_CUDA(cudaEventRecord(g_copy.freed[job & 1], st));
                 if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
-                    EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * l.ld_n, st));
-                    EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, l.Asq, st));
+                    EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * 2 * l.ld_n, st));
+                    EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, gterms.inv2s2, l.Asq, l.Asq + l.ld_n, st));
                 }
                 ++job;
             }

@@ -73,7 +73,7 @@ struct GemmArgs {
 // Gaussian model (EPI_GAUSS, STATS = 2): out = B = acc; the statistics are taken of Q = (B^2 / A_d - C_r) / (2 sigma^2).
 // A kernel parameter of its own so that the other instantiations keep their exact parameter block and code.
 struct GaussParams {
-    const float *a;             // [N] A_d = sum_p K^2
+    const float *g;             // [N] g_d = 1 / (2 sigma^2 A_d), 0 where A_d = 0
     float inv2s2;               // 1 / (2 sigma^2)
 };
 struct NoGauss {};
@@ -520,7 +520,7 @@ __device__ __forceinline__ void tile_out(const float (&racc)[CW], const GemmArgs
             const int chunk = lane >> 2;
             float g_col = 0.f;
             if constexpr (gauss) {
-                if (col < args.N) g_col = gauss_col_factor(gp.a[col], gp.inv2s2);
+                if (col < args.N) g_col = gp.g[col];
             }
             // online statistics over the 32 rows, four rows per step, as a reference pair (mL, mw) = (L, log w) of
             // the row with the largest L + log w and z = sum exp((L - mL) + (log w - mw)): see ColStat in
@@ -930,7 +930,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     const int tiles = a.num_m_tiles * a.num_n_tiles;
     const int grid = 2 * (tiles < clusters ? tiles : clusters);
     typename GaussOf<STATS>::type gp;
-    if constexpr (STATS == 2) { gp.a = g.gauss_a; gp.inv2s2 = g.inv2s2; }
+    if constexpr (STATS == 2) { gp.g = g.gauss_g; gp.inv2s2 = g.inv2s2; }
     kern<<<grid, kGemmThreads, C::SMEM_BYTES, st>>>(tmA, tmB, tmC, a, gp);     // cluster size is a kernel attribute
     EMC_LAUNCHED();
     return EMC_OK;
@@ -953,7 +953,7 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         EMC_LAUNCHED();
         return EMC_OK;
     }
-    if (g.epilogue == EPI_GAUSS && !(g.stat_m && g.gauss_a && g.n_planes == 2 && !g.one_cta && !simt_debug))
+    if (g.epilogue == EPI_GAUSS && !(g.stat_m && g.gauss_g && g.n_planes == 2 && !g.one_cta && !simt_debug))
         return EMC_ERR_UNSUPPORTED;                              // the Gaussian statistics exist in the pair kernel only
     if (g.n_planes == 2 && !g.one_cta) {
         // CTA pairs; tile width by wave quantisation: time ~ waves(BN) x BN (one pair per TPC, tiles of equal cost)

@@ -85,8 +85,10 @@ emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n
                        const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
                        WsHeader *hdr, cudaStream_t st);
 
-// A[d] = sum_p Kc[d][p]^2 (fluence numerators of the Gaussian model, eq. 2.6)
-emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float *Asq, cudaStream_t st);
+// A[d] = sum_p Kc[d][p]^2 (fluence numerators of the Gaussian model, eq. 2.6) as g_col[d] = 1 / (2 sigma^2 A_d) and
+// ia_col[d] = 1 / A_d (both 0 where A_d = 0)
+emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float inv2s2, float *g_col, float *ia_col,
+                        cudaStream_t st);
 
 // Plane GEMM on tcgen05 (emc_gemm.cu):  acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
 struct GemmProblem {
@@ -110,7 +112,7 @@ struct GemmProblem {
     float *stat_m = nullptr, *stat_w = nullptr, *stat_z = nullptr;
     int ld_stat = 0;
     const float *weight = nullptr;
-    const float *gauss_a = nullptr;   // EPI_GAUSS: [N] A_d = sum_p K[d,p]^2
+    const float *gauss_g = nullptr;   // EPI_GAUSS: [N] g_d = 1 / (2 sigma^2 A_d)
     float inv2s2 = 0.f;               // EPI_GAUSS: 1 / (2 sigma^2)
     bool one_cta = false;   // EMC_GEMM_1CTA: the one-CTA kernel instead of CTA pairs (cta_group::2)
 };
@@ -118,7 +120,7 @@ enum { EPI_SUB_ROW = 0,     // out = acc - rowv[m]                      (log-lik
        EPI_STORE = 1,       // out = acc                                (raw update numerator)
        EPI_ADD = 2,         // out += acc                               (numerator over chunks)
        EPI_DIV_ROW = 3,     // out = rowv[m] > 0 ? acc / rowv[m] : 0    (eq. 2.5)
-       EPI_GAUSS = 4 };     // out = acc = B; rowv = C, gauss_a = A: statistics of Q = (B^2/A - C) / (2 sigma^2)
+       EPI_GAUSS = 4 };     // out = acc = B; rowv = C, gauss_g = g: statistics of Q = (B^2/A - C) / (2 sigma^2)
 emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t st);
 // true if launch_plane_gemm(g, simt_debug, .) fills g.stat_m / g.stat_z
 bool gemm_fuses_stats(const GemmProblem &g, bool simt_debug);
@@ -140,9 +142,9 @@ __device__ __forceinline__ float gauss_row_term(float log_w, float c_row, float 
 // Normalise (emc_normalize.cu).  scratch = normalize_scratch_floats() floats.  `planes` (optional) receives the
 // operand planes of P for the update GEMM: two fp16 planes scaled per (row, 512-column chunk) with the inverse
 // scales in chunk_inv_scale [ceil(ld_n/512)][R], or (bf16x3) three unscaled bf16 planes.
-// Gaussian model: L holds B = W K^T; c_row [R] = sum_p W^2, a_col [N] = sum_p K^2, inv2s2 = 1 / (2 sigma^2)
+// Gaussian model: L holds B = W K^T; c_row [R] = sum_p W^2, A_d = sum_p K^2 enters as two column factors, inv2s2 = 1 / (2 sigma^2)
 struct GaussTerms {
-    const float *c_row, *a_col;
+    const float *c_row, *g_col, *ia_col;   // g_col = 1 / (2 sigma^2 A_d), ia_col = 1 / A_d
     float inv2s2;
 };
 size_t normalize_scratch_floats(int n_rot, int ld_n);

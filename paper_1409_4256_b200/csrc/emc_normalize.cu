@@ -348,7 +348,7 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
 // Same thread layout as normalize_kernel; column data is re-read per row (L1-resident) to keep registers free.
 __global__ void __launch_bounds__(kThreads, 2)
 normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ weight, const float *__restrict__ c_row,
-                       const float *__restrict__ a_col, float inv2s2, int n_rot, int n_pat, int ld_n, int n_store,
+                       const float *__restrict__ g_col, const float *__restrict__ ia_col, float inv2s2, int n_rot, int n_pat, int ld_n, int n_store,
                        int rows_per_split,
                        const float *__restrict__ col_m, const float *__restrict__ col_w, const float *__restrict__ col_iz,
                        float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
@@ -372,18 +372,19 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
             const float4 m4 = ok ? *reinterpret_cast<const float4 *>(col_m + d) : z4;
             const float4 w4 = ok ? *reinterpret_cast<const float4 *>(col_w + d) : z4;
             const float4 i4 = ok ? *reinterpret_cast<const float4 *>(col_iz + d) : z4;
-            const float4 a4 = ok ? *reinterpret_cast<const float4 *>(a_col + d) : z4;
+            const float4 a4 = ok ? *reinterpret_cast<const float4 *>(ia_col + d) : z4;
+            const float4 g4 = ok ? *reinterpret_cast<const float4 *>(g_col + d) : z4;
             const float bb[4] = {b4.x, b4.y, b4.z, b4.w}, mm[4] = {m4.x, m4.y, m4.z, m4.w};
             const float ww[4] = {w4.x, w4.y, w4.z, w4.w}, ii[4] = {i4.x, i4.y, i4.z, i4.w};
-            const float aa[4] = {a4.x, a4.y, a4.z, a4.w};
+            const float aa[4] = {a4.x, a4.y, a4.z, a4.w}, gg[4] = {g4.x, g4.y, g4.z, g4.w};
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 float pj = 0.f, qj = 0.f;
                 if (d + j < n_pat) {
-                    const float e = gauss_elem_term(bb[j], gauss_col_factor(aa[j], inv2s2));
+                    const float e = gauss_elem_term(bb[j], gg[j]);
                     pj = expf((e - mm[j]) + (lw - ww[j])) * ii[j];
                     if (pj < EMC_P_MIN) pj = 0.f;                      // DESIGN.md §3 G20
-                    qj = aa[j] > 0.f ? pj * (bb[j] / aa[j]) : 0.f;     // P / phi, phi = A / B (GA3: no photons -> 0)
+                    qj = pj * (bb[j] * aa[j]);                         // P / phi = P B / A (GA3: 1/A = 0 without photons)
                 }
                 p[g][j] = pj;
                 q[g][j] = qj;
@@ -484,7 +485,7 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     const int rows2 = ceil_div(n_rot, splits2);
     const dim3 grid2(chunks, ceil_div(n_rot, rows2));
     if (gauss)
-        normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->a_col, gauss->inv2s2, n_rot, n_pat,
+        normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->g_col, gauss->ia_col, gauss->inv2s2, n_rot, n_pat,
                                                            ld_n, n_store, rows2, col_m, col_w, col_iz, P, planes, bf16x3 ? 1 : 0,
                                                            plane_stride, chunk_inv_scale, s);
     else if (weight)

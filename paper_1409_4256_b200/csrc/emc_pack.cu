@@ -101,9 +101,10 @@ pack_u16x2_kernel(const uint16_t *__restrict__ counts, int n_pat, int n_pix, con
 }
 
 // A[d] = sum_{p: mask} K[d,p]^2 from the packed counts (masked pixels are already 0): the numerator of the
-// fluence, eq. (2.6).  One warp per pattern; counts <= 2048 are exact in float and so are the squares.
+// fluence, eq. (2.6); stored as the two factors the Gaussian model's kernels use per column.  One warp per pattern; counts <= 2048 are exact in float and so are the squares.
 __global__ void __launch_bounds__(256)
-rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, float *__restrict__ Asq) {
+rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, float inv2s2, float *__restrict__ g_col,
+             float *__restrict__ ia_col) {
     const int d = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (d >= n_pat) return;
     const __half *row = Kc + (size_t)d * ld_p;
@@ -120,13 +121,17 @@ rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, floa
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    if (lane == 0) Asq[d] = t;
+    if (lane == 0) {                                          // the two per-column factors every (r, d) needs
+        g_col[d] = gauss_col_factor(t, inv2s2);               // 1 / (2 sigma^2 A_d), 0 for a frame without photons
+        ia_col[d] = t > 0.f ? 1.f / t : 0.f;                  // 1 / A_d
+    }
 }
 
 }  // namespace
 
-emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float *Asq, cudaStream_t st) {
-    rowsq_kernel<<<ceil_div(n_pat, 8), 256, 0, st>>>(Kc, n_pat, n_pix, ld_p, Asq);
+emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float inv2s2, float *g_col, float *ia_col,
+                        cudaStream_t st) {
+    rowsq_kernel<<<ceil_div(n_pat, 8), 256, 0, st>>>(Kc, n_pat, n_pix, ld_p, inv2s2, g_col, ia_col);
     EMC_LAUNCHED();
     return EMC_OK;
 }
