@@ -358,7 +358,36 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
     const float log_uniform = -logf((float)n_rot);
-    for (int r = r_lo + warp; r < r_hi; r += kWarps) {
+    // the column statistics stay in registers for the whole row range; the two Gaussian column factors are re-read per
+    // row (L1-resident); the next row of B is fetched while the current one is worked on
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 cm[kGroups], cw[kGroups], ci[kGroups], nxt[kGroups];
+    bool okg[kGroups];
+#pragma unroll
+    for (int g = 0; g < kGroups; ++g) {
+        const int d = d0 + g * kColsPerBlock + lane * kVec;
+        okg[g] = d < n_pat;                             // ld_n is a multiple of 4: whole float4s
+        cm[g] = okg[g] ? *reinterpret_cast<const float4 *>(col_m + d) : z4;
+        cw[g] = okg[g] ? *reinterpret_cast<const float4 *>(col_w + d) : z4;
+        ci[g] = okg[g] ? *reinterpret_cast<const float4 *>(col_iz + d) : z4;
+        nxt[g] = z4;
+    }
+    int r = r_lo + warp;
+    if (r < r_hi) {
+#pragma unroll
+        for (int g = 0; g < kGroups; ++g)
+            if (okg[g]) nxt[g] = *reinterpret_cast<const float4 *>(B + (size_t)r * ld_n + d0 + g * kColsPerBlock + lane * kVec);
+    }
+    for (; r < r_hi; r += kWarps) {
+        float4 cur[kGroups];
+#pragma unroll
+        for (int g = 0; g < kGroups; ++g) cur[g] = nxt[g];
+        if (r + kWarps < r_hi) {
+#pragma unroll
+            for (int g = 0; g < kGroups; ++g)
+                if (okg[g])
+                    nxt[g] = *reinterpret_cast<const float4 *>(B + (size_t)(r + kWarps) * ld_n + d0 + g * kColsPerBlock + lane * kVec);
+        }
         const float lw = gauss_row_term(weight ? logf(weight[r]) : log_uniform, c_row[r], inv2s2);
         const size_t row_off = (size_t)r * ld_n;
         float p[kGroups][4], q[kGroups][4];
@@ -366,14 +395,10 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
 #pragma unroll
         for (int g = 0; g < kGroups; ++g) {
             const int d = d0 + g * kColsPerBlock + lane * kVec;
-            const bool ok = d < n_pat;                      // ld_n is a multiple of 4: whole float4s
-            const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            const float4 b4 = ok ? *reinterpret_cast<const float4 *>(B + row_off + d) : z4;
-            const float4 m4 = ok ? *reinterpret_cast<const float4 *>(col_m + d) : z4;
-            const float4 w4 = ok ? *reinterpret_cast<const float4 *>(col_w + d) : z4;
-            const float4 i4 = ok ? *reinterpret_cast<const float4 *>(col_iz + d) : z4;
-            const float4 a4 = ok ? *reinterpret_cast<const float4 *>(ia_col + d) : z4;
-            const float4 g4 = ok ? *reinterpret_cast<const float4 *>(g_col + d) : z4;
+            const bool ok = okg[g];
+            const float4 b4 = cur[g], m4 = cm[g], w4 = cw[g], i4 = ci[g];
+            const float4 a4 = ok ? __ldg(reinterpret_cast<const float4 *>(ia_col + d)) : z4;
+            const float4 g4 = ok ? __ldg(reinterpret_cast<const float4 *>(g_col + d)) : z4;
             const float bb[4] = {b4.x, b4.y, b4.z, b4.w}, mm[4] = {m4.x, m4.y, m4.z, m4.w};
             const float ww[4] = {w4.x, w4.y, w4.z, w4.w}, ii[4] = {i4.x, i4.y, i4.z, i4.w};
             const float aa[4] = {a4.x, a4.y, a4.z, a4.w}, gg[4] = {g4.x, g4.y, g4.z, g4.w};
