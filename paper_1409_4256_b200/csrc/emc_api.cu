@@ -154,6 +154,10 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     g.a_fmt = FMT_F16; g.b_fmt = FMT_F16;
     g.out = L; g.ld_out = ld_out; g.rowv = l.S; g.epilogue = gauss ? EPI_GAUSS : EPI_SUB_ROW;
     if (gauss) { g.gauss_g = gauss->g_col; g.inv2s2 = gauss->inv2s2; }
+    // accumulation chunks of 1024 pixels for the Poisson log-likelihood (no per-chunk scales here): the tensor core gets
+    // twice the run-ahead over the end-of-tile phase and half the drains; measured on C2: max |dL|/A 7.6e-7 (4.6e-7 at
+    // 512), signed mean +2.6e-7, tolerance 1e-5.  The Gaussian B keeps 512: its error is amplified by cancellation.
+    if (!gauss) g.k_chunk = 16;
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     if (stats_ready) {
