@@ -170,7 +170,7 @@ def workload_name(cfg):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the two contractions, from the one `ncu --set full`
 # capture of this build summarised in profiles/r01_v5_full_ncu.md (bytes; config:stage)
-NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 822.4e6, "C2:update": 898.9e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 824.5e6, "C2:update": 899.1e6}
 
 
 # ------------------------------------------------------------------------------ clocks
