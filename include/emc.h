@@ -171,7 +171,11 @@ EMC_API emc_status emc_compress(const float *Wnew, const float *slice_w, const e
  *   pat->counts may be a PINNED HOST pointer when flags has EMC_PATTERNS_ON_HOST: each chunk is
  *   then copied to the device inside the call, on a library-owned side stream into two staging
  *   buffers of the workspace, so that the copy of one chunk overlaps the work on the previous one
- *   (one thread at a time; use one stream per workspace).
+ *   (one thread at a time; use one stream per workspace).  With a single resident chunk of at least 4096
+ *   patterns the first iteration runs on four sub-ranges of the chunk while the copies are in flight (the
+ *   same arithmetic as pattern chunks).
+ *   With eq. (2.10) the denominators of Compress are accumulated in the first iteration and reused by the later
+ *   ones for as long as the set of skipped slices (s[r] = 0) stays the same; this is decided on the device.
  *   model_out [n^3] float, out (may not alias model->model).
  *   P_out     [R][ld_n] float of the LAST iteration, out, or NULL (ld_n >= N; needs one chunk).
  *   loglik    [n_iter] device doubles, out: total log-likelihood of each iteration. */
