@@ -61,3 +61,7 @@ def test_gaussian_multi_iteration_and_arguments(inputs_cache):
     assert np.allclose(a["loglik"].cpu().numpy(), lls, rtol=1e-6)
     with pytest.raises(emc.EmcError):
         emc.emc_iterate_gaussian(*args, 0.0)
+    # host-resident patterns go through the staging buffers
+    pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
+    h = emc.emc_iterate_gaussian(*args[:5], pinned, 10.0, n_iter=2, flags=emc.EMC_PATTERNS_ON_HOST)
+    assert np.allclose(h["loglik"].cpu().numpy(), lls, rtol=1e-6)
