@@ -4,6 +4,8 @@ Model, detector, mask and rotation list are the configs' own; only the pattern c
 (make_inputs(..., n_pat=...)) so that the seeded generator finishes in seconds.  What these sizes
 exercise beyond C2: linear indices past 2^31 (R x P = 3.3e9), accumulators that do not fit L2,
 hundreds of K chunks, ragged last pair tiles.  (`-m gpu`)"""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -11,6 +13,9 @@ import torch
 from oracle import emc_oracle as o
 
 pytestmark = pytest.mark.gpu
+
+# EMC_TEST_LARGE=1 runs the same checks at the configs' FULL pattern counts (minutes of input generation)
+FULL = os.environ.get("EMC_TEST_LARGE") == "1"
 
 emc = pytest.importorskip("paper_1409_4256_b200")
 
@@ -103,8 +108,8 @@ def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
 
 
 def test_c3_geometry_sampled(inputs_cache):
-    run_case(inputs_cache, "C3", n_pat=4096, stage=0, n_rows=24, n_cols=48, n_compress=1500)
+    run_case(inputs_cache, "C3", n_pat=50000 if FULL else 4096, stage=0, n_rows=24, n_cols=48, n_compress=1500)
 
 
 def test_c5_last_stage_geometry_sampled(inputs_cache):
-    run_case(inputs_cache, "C5", n_pat=1024, stage=4, n_rows=12, n_cols=32, n_compress=400)
+    run_case(inputs_cache, "C5", n_pat=20000 if FULL else 1024, stage=4, n_rows=12, n_cols=32, n_compress=400)
