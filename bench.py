@@ -1,20 +1,24 @@
 #!/usr/bin/env python
 """bench.py -- EMC iterations/s of the CUDA hot path on synthetic data shaped like the paper's.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
 
+Default workload: BASELINE.json configs[2] = C3 (128^3 model, 128x128 detector, R = 25 000, N = 50 000), the
+config BASELINE.json calls "tensor-core-bound likelihood and update" and the largest one-iteration config
+that is resident on one GPU (BASELINE.json's metric names no config); C1, C2, C4, C5 by --config.
 A "step" is one pass of the whole hot path over the config's workload: every EMC iteration the
-config names (C2: three, C5: five with a growing rotation list), each iteration = Expand ->
+config names (C3: one, C2: three, C5: five with a growing rotation list), each iteration = Expand ->
 log-likelihood -> normalise -> update -> Compress, through the C ABI (emc_iterate).
 
 Prints ONE JSON line (rank 0).  `value` = iterations/s with all inputs resident in HBM; `e2e` = the
 same through the C-ABI call with HOST buffers (pinned counts streamed by the library, model and
 geometry copied in, model and log-likelihood copied out inside the timed region); `roofline` is
 for the dominant kernel, timed live with CUDA events recorded by the library on the launching
-stream (EMC_PROFILE_STAGES); `cpu_baseline` is the CPU oracle timed on this box's host cores on a
-bounded sample (N = 1 only).  With --gpus N > 1 (torchrun) the path does not shard (north_star:
-one GPU, no collectives): every rank runs an independent replica, scaling = "weak".
-`--impl reference` times the oracle itself (rank 0 only).
+stream (EMC_PROFILE_STAGES); `comparator` is cuBLAS (torch.matmul, fp16) on the same operands, timed
+beside it; `cpu_baseline` is the CPU oracle timed on this box's host cores on a bounded sample
+(N = 1 only).  With --gpus N > 1 (torchrun) the path does not shard (north_star: one GPU, no
+collectives): every rank runs an independent replica, scaling = "weak".
+`--impl reference` times the oracle itself (rank 0 only): every step is one bounded sample.
 """
 from __future__ import annotations
 
@@ -35,21 +39,25 @@ import numpy as np  # noqa: E402
 
 METRIC = "emc_iterations_per_s"
 UNIT = "iterations/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels, from the committed `ncu --set full`
+# captures (profiles/*.md name the commands); keyed "<config>:<stage>"
+TRAFFIC_FILE = ROOT / "profiles" / "ncu_dram_bytes_per_launch.json"
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=12)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C2", help="C1..C5 (BASELINE.json configs[0..4]); default C2 = configs[1]")
+    ap.add_argument("--config", default="C3", help="C1..C5 (BASELINE.json configs[0..4]); default C3 = configs[2]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--bf16x3", action="store_true", help="opt-in: P as three unscaled bf16 planes in the update (3 MMAs per k-step)")
     ap.add_argument("--weighted", action="store_true", help="Compress by eq. (2.12) instead of eq. (2.10)")
+    ap.add_argument("--null-weights", action="store_true", help="pass weight = NULL (1/R) instead of the explicit equal weights")
     ap.add_argument("--gaussian-sigma", type=float, default=0.0,
                     help="> 0: time the paper's Gaussian likelihood with fluence (emc_iterate_gaussian, DESIGN.md section 11) "
                          "instead of the Poisson path; not the BASELINE.json metric, no cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-comparator", action="store_true", help="skip the cuBLAS fp16 GEMM on the same operands")
     return ap.parse_args()
 
 
@@ -73,7 +81,7 @@ def oracle_sample(inp, stage, n_rot_s, n_pat_s):
     cfg = inp.cfg
     quat, wgt = inp.quat[stage], inp.weight[stage]
     n_rot, n_pat = len(quat), cfg.n_pat
-    rs, ns = min(n_rot, n_rot_s), min(n_pat, n_pat_s)
+    rs, ns = min(n_rot, n_rot_s), min(n_pat, n_pat_s, inp.counts.shape[0])
     qs = quat[:rs]
     ws = (wgt[:rs] / wgt[:rs].sum()).astype(np.float32)
     ks = inp.counts[:ns]
@@ -99,11 +107,12 @@ def oracle_sample(inp, stage, n_rot_s, n_pat_s):
     return full, dict(times=t, sample_seconds=sum(t.values()), n_rot_sample=rs, n_pat_sample=ns)
 
 
-def sample_sizes(cfg):
-    """Bounded sample: about 10-30 s of oracle work on a few host cores."""
-    budget = 1.2e12                                         # multiply-adds of the three float64 matmuls
-    n_rot_s = min(max(cfg.n_rot), 6144)
-    n_pat_s = int(max(64, min(cfg.n_pat, budget / (3.0 * n_rot_s * cfg.n_pix))))
+def sample_sizes(cfg, scale=1.0):
+    """Bounded sample of the workload: at most 2e7 (rotation, pixel) samples for Expand / Compress (C2's whole count)
+    and 1.2e12 multiply-adds for the float64 matmuls of stages 2 and 4: 10-30 s of oracle work on 8-16 host cores
+    (`scale` shrinks both for the reference arm, which repeats the sample every step)."""
+    n_rot_s = int(min(max(cfg.n_rot), max(256, scale * 2.0e7 / cfg.n_pix)))
+    n_pat_s = int(max(64, min(cfg.n_pat, scale * 1.2e12 / (3.0 * n_rot_s * cfg.n_pix))))
     return n_rot_s, n_pat_s
 
 
@@ -117,9 +126,9 @@ def host_threads():
         return 1
 
 
-def cpu_baseline(inp):
+def cpu_baseline(inp, scale=1.0):
     cfg = inp.cfg
-    n_rot_s, n_pat_s = sample_sizes(cfg)
+    n_rot_s, n_pat_s = sample_sizes(cfg, scale)
     total, parts = 0.0, []
     for stage in range(cfg.n_iter):
         if stage > 0 and cfg.n_rot[stage] == cfg.n_rot[stage - 1]:
@@ -137,27 +146,38 @@ def cpu_baseline(inp):
 
 
 def run_reference(args):
+    """The oracle as it stands on the host cores: every step times one bounded sample of the workload (steps and
+    ms_per_step describe exactly that); `value` extrapolates the mean step to the full workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from emc_inputs import CONFIGS, make_inputs
 
     cfg = CONFIGS[args.config]
-    n_rot_s, n_pat_s = sample_sizes(cfg)
+    scale = 0.3
+    _, n_pat_s = sample_sizes(cfg, scale)
     inp = make_inputs(cfg, n_pat=min(cfg.n_pat, max(n_pat_s, 512)))
     inp.cfg = cfg                                           # extrapolate to the full pattern count
-    times = []
-    for i in range(args.warmup + args.steps):
+    warm = max(args.warmup, 1)
+    times, values = [], []
+    base = None
+    for i in range(warm + args.steps):
         t0 = time.perf_counter()
-        base = cpu_baseline(inp)
-        if i >= args.warmup:
+        base = cpu_baseline(inp, scale)
+        if i >= warm:
             times.append(time.perf_counter() - t0)
-    line = dict(impl="reference", metric=METRIC, value=base["value"], unit=UNIT, n_gpus=args.gpus, steps=args.steps,
-                warmup=args.warmup, ms_per_step=1e3 * cfg.n_iter / base["value"], higher_is_better=True,
+            values.append(base["value"])
+    value = statistics.mean(values)
+    base = dict(base, value=value)
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=warm, ms_per_step=1e3 * statistics.mean(times), higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=workload_name(cfg), note="CPU oracle on a bounded sample, extrapolated"),
-                cpu_baseline=base, sample_wall_s=statistics.mean(times),
-                e2e=dict(value=base["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+                config=dict(workload=workload_name(cfg),
+                            note="every step times the CPU oracle on one bounded sample (cpu_baseline.sample); ms_per_step is "
+                                 "the wall time of such a step, value the extrapolation to the full workload",
+                            ms_per_full_step_extrapolated=1e3 * cfg.n_iter / value),
+                cpu_baseline=base,
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
 
 
@@ -166,11 +186,6 @@ def workload_name(cfg):
     return (f"{cfg.name}: model {cfg.n}^3 fp32, detector {cfg.n_det}x{cfg.n_det}, R={r}, N={cfg.n_pat} "
             f"{cfg.count_dtype} patterns at {cfg.mean_photons} photons/pixel, {cfg.n_iter} iteration(s)"
             + (f", pattern chunks of {cfg.n_pat_chunk}" if cfg.n_pat_chunk < cfg.n_pat else ""))
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the two contractions, from the one `ncu --set full`
-# capture of this build summarised in profiles/r01_v5_full_ncu.md (bytes; config:stage)
-NCU_DRAM_BYTES_PER_LAUNCH = {"C2:loglik": 824.5e6, "C2:update": 899.1e6}
 
 
 # ------------------------------------------------------------------------------ clocks
@@ -192,15 +207,15 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", sel, f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "10"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            time.sleep(0.3)                                 # let the sampler start before the timed region does
         except Exception:
             pass
 
     def stop(self):
         if self.proc is None:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
-        time.sleep(0.15)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
@@ -222,7 +237,10 @@ class ClockSampler:
         os.unlink(self.path)
         if not sm:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
-        return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), power_w_max=max(power), samples=len(sm),
+        # "under load": the samples in the upper half of the power range (the sampler also sees the idle edges)
+        lo, hi = min(power), max(power)
+        load = [c for c, w in zip(sm, power) if w >= lo + 0.5 * (hi - lo)] or sm
+        return dict(sm_mhz=statistics.median(load), sm_max_mhz=max(smax), power_w_max=max(power), samples=len(sm),
                     reasons=sorted(reasons))
 
 
@@ -242,6 +260,40 @@ def whole_job(ms_local, units_per_rank, world, device):
     return ms, world * units_per_rank / (ms * 1e-3)
 
 
+# ------------------------------------------------------------------------------ cuBLAS on the same operands
+
+def cublas_comparator(emc, torch, d_model0, d_q, d_mask, quat, d_counts, n_rep=4):
+    """The log-likelihood contraction's operands handed to cuBLAS: hi plane of log W (fp16, [R, P], masked pixels 0)
+    times the count matrix (fp16, [N, P]) -> [R, N], torch.matmul, CUDA events.  ONE plane: the kernel issues two
+    such products per launch, so its ISSUED rate is what compares with this number.  The count operand is mostly
+    zeros, which lowers the tensor cores' switching power; a dense random GEMM (MEASURED_PEAKS.json) does not have
+    that advantage, this one does."""
+    w, _ = emc.emc_expand(d_model0, d_q, quat, want_idx=False)
+    a = torch.log(torch.clamp(w, min=1e-30))
+    del w
+    a *= d_mask.to(torch.float32)[None, :]
+    a = a.to(torch.float16)
+    b = torch.empty(d_counts.shape, dtype=torch.float16, device="cuda")
+    for d0 in range(0, d_counts.shape[0], 8192):           # in slices: no int32 copy of the whole matrix
+        b[d0:d0 + 8192] = (d_counts[d0:d0 + 8192].to(torch.int32) * d_mask.to(torch.int32)[None, :]).to(torch.float16)
+    torch.cuda.synchronize()
+    c = None
+    for _ in range(2):
+        c = torch.matmul(a, b.t())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_rep):
+        c = torch.matmul(a, b.t())
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / n_rep
+    flops = 2.0 * a.shape[0] * b.shape[0] * a.shape[1]
+    del a, b, c
+    torch.cuda.empty_cache()
+    return dict(what="torch.matmul (cuBLAS) fp16 [R,P] x [N,P]^T on the hi plane of log W and the count matrix of this "
+                     "workload, all P pixels, fp16 output", ms=ms, tflops=flops / (ms * 1e-3) / 1e12, reps=n_rep)
+
+
 # ------------------------------------------------------------------------------ our arm
 
 def main():
@@ -249,11 +301,15 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
 
+    from emc_inputs import CONFIGS, make_inputs
+
+    cfg = CONFIGS[args.config]
+    inp = make_inputs(cfg)                                   # every rank: an independent replica
+
     import torch
     import torch.distributed as dist
 
     import paper_1409_4256_b200 as emc
-    from emc_inputs import CONFIGS, make_inputs
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -263,9 +319,8 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg = CONFIGS[args.config]
-    inp = make_inputs(cfg)                                   # every rank: an independent replica
     peaks = measured_peaks()
+    warmup = max(args.warmup, 3)
 
     dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
     d_model0, d_q, d_mask, d_counts = dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.counts)
@@ -275,12 +330,13 @@ def main():
         if plan and cfg.n_rot[s] == cfg.n_rot[s - 1]:
             plan[-1][2] += 1
         else:
-            plan.append([dev(inp.quat[s]), dev(inp.weight[s]), 1, inp.quat[s], inp.weight[s]])
-    flags = (emc.EMC_UPDATE_BF16X3 if args.bf16x3 else 0) | (emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0)
+            plan.append([dev(inp.quat[s]), None if args.null_weights else dev(inp.weight[s]), 1, inp.quat[s], inp.weight[s]])
+    flags = emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0
     chunk = cfg.n_pat_chunk if cfg.n_pat_chunk < cfg.n_pat else 0
     ws_bytes = max(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, r, cfg.n_pat_chunk, emc.EMC_PATTERNS_ON_HOST)
                    for r in cfg.n_rot)
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    ctx = emc.EmcContext()                                   # copy stream + timing events, created outside the hot path
     d_ll = torch.zeros(cfg.n_iter, dtype=torch.float64, device="cuda")
     bufs = [torch.empty_like(d_model0), torch.empty_like(d_model0)]
 
@@ -290,12 +346,12 @@ def main():
         for quat, wgt, n_it, _, _ in plan:
             if args.gaussian_sigma > 0:
                 out = emc.emc_iterate_gaussian(src, d_q, d_mask, quat, wgt, d_counts, args.gaussian_sigma, n_iter=n_it,
-                                               flags=f | emc.EMC_COMPRESS_WEIGHTED, ws=ws)
+                                               flags=f | emc.EMC_COMPRESS_WEIGHTED, ws=ws, ctx=ctx)
                 d_ll[it0:it0 + n_it] = out["loglik"]
                 src, it0 = out["model"], it0 + n_it
                 continue
             emc.emc_iterate(src, d_q, d_mask, quat, wgt, d_counts, n_iter=n_it, n_pat_chunk=chunk, flags=f, ws=ws,
-                            model_out=bufs[k], loglik=d_ll[it0:it0 + n_it])
+                            model_out=bufs[k], loglik=d_ll[it0:it0 + n_it], ctx=ctx)
             src, k, it0 = bufs[k], 1 - k, it0 + n_it
         return src
 
@@ -304,10 +360,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(warmup):
         step(flags)
     emc.emc_check(ws)
-    emc.emc_profile_read()
+    emc.emc_profile_read(ctx)
 
     clocks = ClockSampler(local)
     launches0 = emc.emc_launch_count()
@@ -321,14 +377,14 @@ def main():
     ms = ev0.elapsed_time(ev1)
     launches = emc.emc_launch_count() - launches0
     clk = clocks.stop()
-    prof = emc.emc_profile_read()
+    prof = emc.emc_profile_read(ctx)
     ms, value = whole_job(ms, args.steps * cfg.n_iter, world, "cuda")
 
     if args.gaussian_sigma > 0:                  # a side measurement: device-resident only, Poisson-path JSON keys kept
         prof_g = {k: v[0] / (args.steps * cfg.n_iter) for k, v in prof.items()}
         if rank == 0:
             print(json.dumps(dict(metric="emc_gaussian_iterations_per_s", value=value, unit=UNIT, n_gpus=world,
-                                  steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms / args.steps,
+                                  steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,
                                   sigma=args.gaussian_sigma, config=dict(workload=workload_name(cfg)), clocks=clk,
                                   stage_ms_per_iteration=prof_g, gpu_launches=int(launches),
                                   loglik_per_iteration=[float(x) for x in d_ll.cpu().tolist()])))
@@ -346,7 +402,7 @@ def main():
     h_out = torch.empty_like(h_model).pin_memory()
     h_ll = torch.empty(cfg.n_iter, dtype=torch.float64).pin_memory()
     e_model, e_q, e_mask = torch.empty_like(d_model0), torch.empty_like(d_q), torch.empty_like(d_mask)
-    e_rot = [(torch.empty_like(q), torch.empty_like(w)) for q, w, _, _, _ in plan]
+    e_rot = [(torch.empty_like(q), torch.empty(len(w), dtype=torch.float32, device="cuda")) for q, _, _, _, w in plan]
     h2d = (h_counts.numel() * h_counts.element_size() * (cfg.n_iter if chunk else len(plan))
            + h_model.numel() * 4 + h_q.numel() * 4 + h_mask.numel()
            + sum(q.numel() * 4 + w.numel() * 4 for q, w in h_rot))
@@ -362,7 +418,7 @@ def main():
             dw.copy_(hw, non_blocking=True)
             emc.emc_iterate(src, e_q, e_mask, dq, dw, h_counts, n_iter=n_it, n_pat_chunk=chunk,
                             flags=flags | emc.EMC_PATTERNS_ON_HOST, ws=ws, model_out=bufs[k],
-                            loglik=d_ll[it0:it0 + n_it])
+                            loglik=d_ll[it0:it0 + n_it], ctx=ctx)
             src, k, it0 = bufs[k], 1 - k, it0 + n_it
         h_out.copy_(src, non_blocking=True)
         h_ll.copy_(d_ll, non_blocking=True)
@@ -381,7 +437,6 @@ def main():
 
     # ---- rooflines from the live per-stage CUDA-event times
     p_eff = int(inp.mask.sum())
-    n_planes_p = 3 if args.bf16x3 else 2
     rn = sum(r * cfg.n_pat for r in cfg.n_rot) * args.steps            # (rotation, pattern) pairs processed
     rp = sum(cfg.n_rot) * args.steps
     g = cfg.n ** 3
@@ -396,8 +451,7 @@ def main():
                        issued_tflops=tf(2 * useful, stage_ms["loglik"]), planes=2, dtype="fp16x2"),
         "update": dict(ms=stage_ms["update"], launches=stage_spans["update"], bound="tensor",
                        useful_tflops=tf(useful, stage_ms["update"]),
-                       issued_tflops=tf(n_planes_p * useful, stage_ms["update"]), planes=n_planes_p,
-                       dtype="bf16x3" if args.bf16x3 else "fp16x2 chunk-scaled"),
+                       issued_tflops=tf(2 * useful, stage_ms["update"]), planes=2, dtype="fp16x2 chunk-scaled"),
         "expand": dict(ms=stage_ms["expand"], bound="hbm",
                        gbs=gbs(rp * cfg.n_pix * 4.0 + 4.0 * g * stage_spans["expand"], stage_ms["expand"])),
         "normalize": dict(ms=stage_ms["normalize"], bound="hbm", gbs=gbs(8.0 * rn, stage_ms["normalize"])),
@@ -407,35 +461,45 @@ def main():
     }
     for k in ("expand", "normalize", "compress"):
         stages[k]["frac_of_hbm"] = stages[k]["gbs"] / peaks["hbm"]
-    for k in ("loglik", "update"):
-        stages[k]["frac_of_bf16_sustained"] = stages[k]["issued_tflops"] / peaks["bf16_sustained"]
-        stages[k]["frac_of_bf16_burst"] = stages[k]["issued_tflops"] / peaks["bf16_burst"]
-    dom = "update" if stage_ms["update"] >= stage_ms["loglik"] else "loglik"
-    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(f"{cfg.name}:{dom}")
-    # which measured cuBLAS figure: the burst one while the timed region is too short for the power cap to bite (the
-    # whole region well under a second, no sw_power_cap seen), else the sustained one
-    sustained = ms >= 1000.0 or "sw_power_cap" in (clk.get("reasons") or [])
+    # which measured cuBLAS figure: the sustained one when the kernel is timed inside a long step (a timed region of a
+    # second or more, where the 1 kW power cap decides the clock), the burst one for a short region
+    sustained = ms >= 1000.0
     peak = peaks["bf16_sustained"] if sustained else peaks["bf16_burst"]
+    for k in ("loglik", "update"):
+        stages[k]["useful_frac_of_peak"] = stages[k]["useful_tflops"] / peak
+        stages[k]["issued_frac_of_peak"] = stages[k]["issued_tflops"] / peak
+    dom = "update" if stage_ms["update"] >= stage_ms["loglik"] else "loglik"
+    traffic, traffic_src = None, None
+    if TRAFFIC_FILE.exists():
+        rec = json.loads(TRAFFIC_FILE.read_text()).get(f"{cfg.name}:{dom}")
+        if rec:
+            traffic, traffic_src = rec["bytes"], rec["source"]
+    # tensor-core peak the chip has at the clock it held during this run (148 SMs x 8192 dense fp16 flops per clock)
+    clock_peak = 148 * 8192 * clk["sm_mhz"] * 1e6 / 1e12 if clk.get("sm_mhz") else None
     roofline = dict(bound="tensor", kernel=f"plane_gemm_pair_kernel ({dom}, {stages[dom]['dtype']})",
-                    achieved=stages[dom]["issued_tflops"], peak=peak, unit="TFLOP/s",
-                    frac=stages[dom]["issued_tflops"] / peak, traffic=traffic,
-                    peak_source=f"{peaks['source']} cuBLAS bf16 " + ("sustained (timed region of %.1f s under the power cap)"
-                                                                      % (ms * 1e-3) if sustained else
-                                                                      "burst (timed region of %.0f ms, no power cap seen)" % ms),
+                    achieved=stages[dom]["useful_tflops"], peak=peak, unit="TFLOP/s",
+                    frac=stages[dom]["useful_tflops"] / peak, traffic=traffic,
+                    issued=stages[dom]["issued_tflops"], issued_frac=stages[dom]["issued_tflops"] / peak,
+                    issued_frac_of_clock_peak=(stages[dom]["issued_tflops"] / clock_peak) if clock_peak else None,
+                    clock_peak_tflops=clock_peak,
+                    peak_source=f"{peaks['source']} cuBLAS bf16 " + ("sustained (timed region of %.2f s)" % (ms * 1e-3)
+                                                                      if sustained else "burst (timed region of %.0f ms)" % ms),
                     avg_launch_ms=stage_ms[dom] / max(1, stage_spans[dom]),
-                    traffic_unit="DRAM bytes per launch (ncu, profiles/r01_v5_full_ncu.md)",
-                    note="achieved = 2*planes*R*N*P_eff flops per launch / CUDA-event launch time (issued MMA work of "
-                         "the split scheme on unmasked pixels); useful TFLOP/s is in stages.  fp16 and bf16 share one "
-                         "tensor rate; the count operand is >90 % zeros, which lowers switching power, so under the "
-                         "power cap this kernel can hold a higher clock than the dense random cuBLAS reference")
+                    traffic_unit="DRAM bytes per launch (ncu)", traffic_source=traffic_src,
+                    note="achieved = ALGORITHMIC flops 2*R*N*P_eff per launch / CUDA-event launch time.  The fp16x2 split "
+                         "scheme issues two tensor-core products per algorithmic one (DESIGN.md section 6): `issued` is "
+                         "that MMA rate, to be read against `comparator` (cuBLAS fp16 on the same, mostly-zero count "
+                         "operand) and against clock_peak_tflops = 148 SMs x 8192 flop/clk x the SM clock of this run")
 
-    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warmup,
                 ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="fp16x2 operand planes, f32 accumulate", data="synthetic",
                 config=dict(workload=workload_name(cfg), parallelism="replicas only" if world > 1 else "1 GPU",
                             l2="per-iteration working set exceeds the 126 MB L2, no flush" if cfg.name != "C1"
                             else "working set fits L2 (launch-latency-bound config), no flush",
-                            compress="eq. (2.12)" if args.weighted else "eq. (2.10)", p_eff=p_eff),
+                            compress="eq. (2.12)" if args.weighted else "eq. (2.10)", p_eff=p_eff,
+                            weights="NULL (1/R): uniform branches, normalize_kernel<true>" if args.null_weights
+                            else "explicit equal weights: general branches, normalize_kernel<false>"),
                 clocks=clk,
                 e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                          ms_per_step=ms_e2e / args.steps),
@@ -444,6 +508,9 @@ def main():
                 roofline=roofline, stages=stages,
                 loglik_per_iteration=[float(x) for x in d_ll.cpu().tolist()])
     if rank == 0:
+        if world == 1 and not args.no_comparator:
+            del h_counts
+            line["comparator"] = cublas_comparator(emc, torch, d_model0, d_q, d_mask, plan[-1][0], d_counts)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(inp)
         print(json.dumps(line))

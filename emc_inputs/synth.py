@@ -9,6 +9,8 @@ the CUDA package: it is the one piece both sides may share.
 from __future__ import annotations
 
 import dataclasses
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass
 
 import numpy as np
@@ -161,14 +163,19 @@ def _slices_library(model64: np.ndarray, q: np.ndarray, quat: np.ndarray) -> np.
 _SENTINEL = {"int32": 2 ** 31 - 1, "uint16": 65535, "uint8": 255}
 
 
+_CHUNK = 256        # patterns per Poisson stream: part of the recipe (the counts do not depend on the thread count)
+
+
 def simulate_patterns(model64, q, mask, quat_list, n_pat, mean_photons, count_dtype, seed_orient,
-                      seed_poisson, chunk=256):
+                      seed_poisson):
     """Poisson photon counts of n_pat shots at orientations drawn uniformly from `quat_list`.
+    Chunk c of 256 consecutive patterns draws from its own PCG64 stream seeded (seed_poisson, c), so the
+    chunks can be generated by several threads (the scipy / numpy routines release the GIL) with the
+    same result on any machine.
 
     Returns (counts [N,P], r_true [N], scale): `scale` is the factor by which the model has to be
     multiplied so that the mean expected count over unmasked pixels is `mean_photons`."""
     r_true = _rng(seed_orient).integers(0, len(quat_list), n_pat)
-    rng = _rng(seed_poisson)
     use = mask.astype(bool)
     # pass 1: scale from a bounded sample of the shots (exact mean for small N)
     probe = r_true[: min(n_pat, 512)]
@@ -176,12 +183,26 @@ def simulate_patterns(model64, q, mask, quat_list, n_pat, mean_photons, count_dt
     scale = mean_photons / lam[:, use].mean()
     counts = np.empty((n_pat, len(q)), dtype=count_dtype)
     hi = np.iinfo(count_dtype).max
-    for d0 in range(0, n_pat, chunk):
-        d1 = min(n_pat, d0 + chunk)
+    sentinel = _SENTINEL[count_dtype]
+
+    def one_chunk(c):
+        d0 = c * _CHUNK
+        d1 = min(n_pat, d0 + _CHUNK)
+        rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence((seed_poisson, c))))
         lam = _slices_library(model64, q, quat_list[r_true[d0:d1]]) * scale
         k = rng.poisson(np.maximum(lam, 0.0))
-        counts[d0:d1] = np.minimum(k, hi - 1).astype(count_dtype)
-    counts[:, ~use] = _SENTINEL[count_dtype]        # garbage that every stage must ignore (G16)
+        block = np.minimum(k, hi - 1).astype(count_dtype)
+        block[:, ~use] = sentinel                   # garbage that every stage must ignore (G16)
+        counts[d0:d1] = block
+
+    n_chunks = -(-n_pat // _CHUNK)
+    workers = max(1, min(32, os.cpu_count() or 1, n_chunks))
+    if workers == 1:
+        for c in range(n_chunks):
+            one_chunk(c)
+    else:
+        with ThreadPoolExecutor(workers) as pool:
+            list(pool.map(one_chunk, range(n_chunks)))
     return counts, r_true.astype(np.int32), float(scale)
 
 

@@ -15,10 +15,16 @@
  *    comes from the caller's workspace `ws` of at least emc_workspace_bytes(...) bytes, 256-byte
  *    aligned.  Nothing in the workspace survives a call except where stated.
  *  - `stream` is a cudaStream_t.  Calls validate their arguments synchronously, enqueue their
- *    kernels on `stream` and return without synchronising.
- *  - Errors are returned as negative emc_status values, never thrown or aborted.  Conditions that
- *    only the device can see (a photon count too large for the exact 16-bit operand format) are
- *    recorded in the workspace header and reported by emc_check().
+ *    kernels on `stream` and return without synchronising.  The exceptions say so in their own
+ *    comment: emc_check, emc_profile_read and emc_refine wait for the device.
+ *  - No call creates CUDA objects.  The two features that need some (a copy stream for
+ *    host-resident patterns, events for per-stage timing) take them from an emc_context the
+ *    caller creates once; one context serves one stream at a time, any number of contexts and
+ *    workspaces can be in use on different streams and threads at once.
+ *  - Errors are returned as negative emc_status values, never thrown or aborted.  A condition that
+ *    only the device can see (a photon count too large for the exact 16-bit operand format) is
+ *    recorded in the workspace header: every result of that call is then filled with NaN on the
+ *    device, so that it cannot be consumed unnoticed, and emc_check() reports it.
  *  - Matrices are row-major: W is [R][P], L and P are [R][N] with row pitch `ld_n` floats
  *    (ld_n >= N, a multiple of 4; the binding uses N rounded up to 64).  The model is
  *    [n][n][n] with z fastest, voxel (i,j,k) at integer coordinates, origin c = n/2 on every axis
@@ -52,15 +58,15 @@ typedef enum {
 typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
 
 /* Largest photon count in an unmasked pixel that the exact 16-bit tensor-core operands hold
- * (fp16 holds every integer up to 2048; DESIGN.md §6 "precision scheme"; 256 with
- * EMC_UPDATE_BF16X3).  Saturated pixels are expected to be masked. */
+ * (fp16 holds every integer up to 2048; DESIGN.md §6 "precision scheme").  Saturated pixels are
+ * expected to be masked. */
 #define EMC_MAX_COUNT 2048
 
-/* Responsibilities below 2^-100 are stored as 0 (DESIGN.md §3 G20): float32 P keeps full relative
- * precision only down to there once it is split into 16-bit operand planes for the update contraction,
- * and a rotation whose whole row lies below it has no data behind it (s[r] = 0: W'[r,:] = 0, slice
- * skipped by Compress, G17). */
-#define EMC_P_MIN 7.888609052210118e-31f
+/* Responsibilities are float32 (the paper works in single precision).  Below the smallest
+ * normal float32, 2^-126, a value has no relative precision left, so P is stored flush-to-zero: values
+ * below 2^-126 are 0 (DESIGN.md §3 G20).  A rotation whose whole row is 0 has s[r] = 0: W'[r,:] = 0 and
+ * the slice is skipped by Compress (G17).  Which slices that is matters under eq. (2.10) only. */
+#define EMC_P_MIN 1.1754943508222875e-38f
 
 /* flags */
 #define EMC_COMPRESS_WEIGHTED 0x1u /* eq. (2.12): slice r enters Compress with
@@ -69,11 +75,8 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
                                       (pattern chunks, DESIGN.md §3 G9) */
 #define EMC_UPDATE_RAW        0x4u /* emc_update: leave Wnew as the numerator of eq. (2.11),
                                       do not divide by s[r] */
-#define EMC_UPDATE_BF16X3     0x8u /* opt-in: P enters the update contraction as three unscaled bf16
-                                      planes (3 MMAs per k-step) instead of two chunk-scaled fp16
-                                      planes (2 MMAs) */
-#define EMC_PROFILE_STAGES    0x20u /* emc_iterate records CUDA events on `stream` around every stage;
-                                      read (and reset) the sums with emc_profile_read() */
+#define EMC_PROFILE_STAGES    0x20u /* emc_iterate records the context's CUDA events on `stream` around every
+                                      stage; read (and reset) the sums with emc_profile_read() */
 #define EMC_GEMM_1CTA         0x200u /* run the two contractions with one CTA per tile (cta_group::1)
                                         instead of CTA pairs (cta_group::2); a comparison / bisecting aid */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
@@ -105,6 +108,14 @@ typedef struct {
     const void *counts;  /* [N][P] row-major; values in masked pixels are ignored */
     emc_count_type type;
 } emc_patterns;
+
+/* CUDA objects the library may use on the caller's behalf: one non-blocking copy stream with its events
+ * (EMC_PATTERNS_ON_HOST) and a pool of timing events (EMC_PROFILE_STAGES).  Created and destroyed by the
+ * caller, outside the hot path; emc_iterate* take it as an argument and need it only with those flags
+ * (EMC_ERR_ARG if it is NULL then).  One context serves one stream at a time. */
+typedef struct emc_context emc_context;
+EMC_API emc_status emc_context_create(emc_context **ctx);
+EMC_API emc_status emc_context_destroy(emc_context *ctx);
 
 /* Bytes of workspace sufficient for any call below at these sizes.  n_pat_chunk = patterns
  * resident per chunk (= N when not chunked).  Returns 0 on invalid sizes. */
@@ -169,9 +180,9 @@ EMC_API emc_status emc_compress(const float *Wnew, const float *slice_w, const e
  * Patterns are processed in chunks of n_pat_chunk (0 = all at once): stages 2-3 per chunk, s[r]
  * and the update numerators summed over chunks, divided after the last (DESIGN.md §3 G9).
  *   pat->counts may be a PINNED HOST pointer when flags has EMC_PATTERNS_ON_HOST: each chunk is
- *   then copied to the device inside the call, on a library-owned side stream into two staging
+ *   then copied to the device inside the call, on the context's copy stream into two staging
  *   buffers of the workspace, so that the copy of one chunk overlaps the work on the previous one
- *   (one thread at a time; use one stream per workspace).  With a single resident chunk of at least 4096
+ *   (one stream per workspace and per context).  With a single resident chunk of at least 4096
  *   patterns the first iteration runs on four sub-ranges of the chunk while the copies are in flight (the
  *   same arithmetic as pattern chunks).
  *   With eq. (2.10) the denominators of Compress are accumulated in the first iteration and reused by the later
@@ -183,7 +194,7 @@ EMC_API emc_status emc_compress(const float *Wnew, const float *slice_w, const e
 EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                        const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
-                       size_t ws_bytes, void *stream);
+                       size_t ws_bytes, void *stream, emc_context *ctx);
 
 /* Algorithm 1 with the paper's own likelihood: Gaussian around the slice with a fluence per (rotation, frame),
  * eqs. (2.2), (2.3), (2.5)/(2.11), (2.6), PAPER.md:70-89, 124-130 (NEXT-3, readings GA1-GA7):
@@ -198,7 +209,8 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
  * Arguments as emc_iterate; sigma > 0 in the units of the model. */
 EMC_API emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                                 const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
-                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream);
+                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
+                                emc_context *ctx);
 
 /* Adaptive EMC, section 3.4 and eq. (3.1): `n_iter` iterations that start on the coarsest
  * rotation list levels[0] and move on to the next list after an iteration n >= 1 whose total log-likelihood
@@ -215,19 +227,20 @@ EMC_API emc_status emc_iterate_gaussian(const emc_model *model, const emc_detect
 EMC_API emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc_rotations *levels,
                       int n_levels, const emc_patterns *pat, int n_iter, double threshold, int n_pat_chunk,
                       float *model_out, float *model_tmp, double *loglik, int32_t *level_of_iter,
-                      unsigned flags, void *ws, size_t ws_bytes, void *stream);
+                      unsigned flags, void *ws, size_t ws_bytes, void *stream, emc_context *ctx);
 
 /* Synchronises `stream` and reports what only the device saw during calls that used `ws`:
- * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (results are then undefined),
+ * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (the results of that call are NaN),
  * EMC_ERR_CUDA if the stream is in error.  Clears the record. */
 EMC_API emc_status emc_check(void *ws, void *stream);
 
-/* Stages timed under EMC_PROFILE_STAGES (one thread at a time; at most 8192 spans between reads). */
+/* Stages timed under EMC_PROFILE_STAGES (at most EMC_MAX_SPANS spans between reads; later ones are dropped). */
+#define EMC_MAX_SPANS 4096
 enum { EMC_STAGE_EXPAND = 0, EMC_STAGE_PACK = 1, EMC_STAGE_LOGLIK = 2, EMC_STAGE_NORMALIZE = 3,
        EMC_STAGE_UPDATE = 4, EMC_STAGE_COMPRESS = 5, EMC_N_STAGES = 6 };
 /* Waits for the recorded events, returns per stage the summed device time in milliseconds (HOST
  * array ms[EMC_N_STAGES]) and the number of spans (HOST array spans[EMC_N_STAGES]), and resets. */
-EMC_API emc_status emc_profile_read(double *ms, int *spans);
+EMC_API emc_status emc_profile_read(emc_context *ctx, double *ms, int *spans);
 
 /* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
 EMC_API uint64_t emc_launch_count(void);

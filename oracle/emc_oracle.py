@@ -25,7 +25,7 @@ from __future__ import annotations
 import numpy as np
 
 LOGW_FLOOR = np.float32(1e-30)      # DESIGN.md §3 G8: log(max(W, 1e-30))
-P_MIN = 2.0 ** -100                 # DESIGN.md §3 G20: responsibilities below 2^-100 are stored as 0
+P_MIN = float(np.finfo(np.float32).tiny)   # DESIGN.md §3 G20: float32 P is stored flush-to-zero (below 2^-126 -> 0)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -180,9 +180,9 @@ def normalize(big_l, weight):
     """P[r,d] = w_r T_rd / sum_r' w_r' T_r'd with T = exp(L), evaluated max-subtracted
     ("some care ... finite precision"; only max and sum are needed):
         a = L + log w_r;  m_d = max_r a;  e = exp(a - m_d);  P = e / sum_r e,
-    with values below P_MIN = 2^-100 stored as 0 (G20: float32 P has no relative precision left
-    below that once split for the update contraction; a rotation whose whole row is below it has
-    no data behind it and is skipped, G17).
+    with values below P_MIN = 2^-126 stored as 0 (G20: P is a float32 quantity; below
+    the smallest normal float32 a value has no relative precision left, so P is flushed to zero
+    there; a rotation whose whole row is 0 has s[r] = 0 and is skipped by Compress, G17).
     Also s[r] = sum_d P[r,d] and the total log-likelihood LL = sum_d (m_d + log sum_r e).
     `big_l` is taken as given (tests feed the float32-rounded L, DESIGN.md §4 T2).
     Returns (P float64 [R,N], s float64 [R], LL float)."""

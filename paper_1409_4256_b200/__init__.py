@@ -1,38 +1,6 @@
 """paper_1409_4256_b200: one EMC iteration (arXiv 1409.4256) on one B200, as hand-written sm_100a
 CUDA behind a C ABI (include/emc.h, csrc/) with a thin ctypes binding of the same names."""
-from .binding import (  # noqa: F401
-    EMC_ACCUMULATE,
-    EMC_COMPRESS_WEIGHTED,
-    EMC_DEBUG_SIMT,
-    EMC_GEMM_1CTA,
-    EMC_ERR_ARG,
-    EMC_ERR_COUNT_RANGE,
-    EMC_ERR_CUDA,
-    EMC_ERR_UNSUPPORTED,
-    EMC_ERR_WORKSPACE,
-    EMC_MAX_COUNT,
-    EMC_OK,
-    EMC_PATTERNS_ON_HOST,
-    EMC_UPDATE_BF16X3,
-    EMC_PROFILE_STAGES,
-    STAGES,
-    EMC_UPDATE_RAW,
-    SYMBOLS,
-    EmcError,
-    emc_check,
-    emc_compress,
-    emc_expand,
-    emc_iterate,
-    emc_iterate_gaussian,
-    emc_launch_count,
-    emc_loglik,
-    emc_normalize,
-    emc_profile_read,
-    emc_refine,
-    emc_update,
-    emc_version,
-    emc_workspace_bytes,
-    ld_for,
-    load,
-    make_workspace,
-)
+from . import binding
+from .binding import *  # noqa: F401,F403  (binding.__all__: the emc_* calls, EMC_* constants and helpers)
+
+__all__ = list(binding.__all__)

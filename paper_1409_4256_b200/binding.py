@@ -21,16 +21,17 @@ EMC_MAX_COUNT = 2048
 EMC_COMPRESS_WEIGHTED = 0x1
 EMC_ACCUMULATE = 0x2
 EMC_UPDATE_RAW = 0x4
-EMC_UPDATE_BF16X3 = 0x8
 EMC_PATTERNS_ON_HOST = 0x10
 EMC_PROFILE_STAGES = 0x20
 EMC_DEBUG_SIMT = 0x100
 EMC_GEMM_1CTA = 0x200
+EMC_MAX_SPANS = 4096
 STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
-SYMBOLS = ("emc_workspace_bytes", "emc_expand", "emc_loglik", "emc_normalize", "emc_update", "emc_compress",
-           "emc_iterate", "emc_iterate_gaussian", "emc_refine", "emc_check", "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_expand", "emc_loglik",
+           "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_gaussian", "emc_refine", "emc_check",
+           "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
 class EmcError(RuntimeError):
@@ -72,6 +73,10 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
         p = _build.build()          # needs nvcc; raises if it cannot be built -- no fallback
     lib = ctypes.CDLL(str(p))
     vp, sz, ci, cu = c_void_p, c_size_t, c_int, c_uint
+    lib.emc_context_create.restype = ci
+    lib.emc_context_create.argtypes = [POINTER(vp)]
+    lib.emc_context_destroy.restype = ci
+    lib.emc_context_destroy.argtypes = [vp]
     lib.emc_workspace_bytes.restype = sz
     lib.emc_workspace_bytes.argtypes = [ci, ci, ci, ci, cu]
     lib.emc_expand.restype = ci
@@ -86,17 +91,17 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_compress.argtypes = [vp, vp, POINTER(_Detector), POINTER(_Rotations), ci, vp, vp, cu, vp, sz, vp]
     lib.emc_iterate.restype = ci
     lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
-                                ci, ci, vp, vp, ci, vp, cu, vp, sz, vp]
+                                ci, ci, vp, vp, ci, vp, cu, vp, sz, vp, vp]
     lib.emc_iterate_gaussian.restype = ci
     lib.emc_iterate_gaussian.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
-                                         ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp]
+                                         ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp, vp]
     lib.emc_refine.restype = ci
     lib.emc_refine.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), ci, POINTER(_Patterns), ci,
-                               c_double, ci, vp, vp, vp, POINTER(ctypes.c_int32), cu, vp, sz, vp]
+                               c_double, ci, vp, vp, vp, POINTER(ctypes.c_int32), cu, vp, sz, vp, vp]
     lib.emc_check.restype = ci
     lib.emc_check.argtypes = [vp, vp]
     lib.emc_profile_read.restype = ci
-    lib.emc_profile_read.argtypes = [POINTER(c_double), POINTER(c_int)]
+    lib.emc_profile_read.argtypes = [vp, POINTER(c_double), POINTER(c_int)]
     lib.emc_launch_count.restype = c_uint64
     lib.emc_launch_count.argtypes = []
     for name in ("emc_strerror", "emc_last_cuda_error", "emc_version"):
@@ -177,6 +182,46 @@ def _ws(ws, n, n_pix, n_rot, n_chunk, flags=0):
     return ws, ws.data_ptr(), ws.numel()
 
 
+# ---------------------------------------------------------------------------- context
+
+class EmcContext:
+    """emc_context (include/emc.h): the copy stream and event pool the library may use on the caller's behalf.
+    One context serves one stream at a time."""
+
+    def __init__(self):
+        h = c_void_p()
+        _check(load().emc_context_create(ctypes.byref(h)), "emc_context_create")
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            load().emc_context_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+_DEFAULT_CTX = None
+
+
+def default_context() -> EmcContext:
+    """The binding's own context, created on first use (outside any libemc hot call)."""
+    global _DEFAULT_CTX
+    if _DEFAULT_CTX is None:
+        _DEFAULT_CTX = EmcContext()
+    return _DEFAULT_CTX
+
+
+def _ctx(ctx, flags):
+    if ctx is None and flags & (EMC_PATTERNS_ON_HOST | EMC_PROFILE_STAGES):
+        ctx = default_context()
+    return ctx.handle if ctx is not None else None
+
+
 # ---------------------------------------------------------------------------- the six calls
 
 def emc_expand(model, q, quat, want_idx=True, use_ws=True):
@@ -188,7 +233,7 @@ def emc_expand(model, q, quat, want_idx=True, use_ws=True):
     rot = _rotations(quat, None)
     w = torch.empty((rot.n_rot, det.n_pix), dtype=torch.float32, device=model.device)
     idx = torch.empty((rot.n_rot, det.n_pix), dtype=torch.int32, device=model.device) if want_idx else None
-    ws = make_workspace(n, det.n_pix, rot.n_rot, 1) if use_ws else None
+    ws = make_workspace(n, det.n_pix, 1, 1) if use_ws else None      # the blocked model copies do not scale with R
     _check(load().emc_expand(m, det, rot, w.data_ptr(), idx.data_ptr() if want_idx else None,
                              ws.data_ptr() if use_ws else None, ws.numel() if use_ws else 0, _stream()), "emc_expand")
     return w, idx
@@ -253,7 +298,7 @@ def emc_compress(wnew, slice_w, q, mask, quat, n, flags=0, want_den=False, ws=No
     rot = _rotations(quat, None)
     model = torch.empty((n, n, n), dtype=torch.float32, device=wnew.device)
     den = torch.empty(n * n * n, dtype=torch.float32, device=wnew.device) if want_den else None
-    ws, wp, wb = _ws(ws, n, n_pix, n_rot, 1)
+    ws, wp, wb = _ws(ws, n, n_pix, 1, 1)                              # the accumulators do not scale with R
     _check(load().emc_compress(_dev(wnew, torch.float32, "Wnew"), _opt(slice_w, torch.float32, "slice_w"), det, rot,
                                n, model.data_ptr(), den.data_ptr() if want_den else None, flags, wp, wb, _stream()),
            "emc_compress")
@@ -261,7 +306,7 @@ def emc_compress(wnew, slice_w, q, mask, quat, n, flags=0, want_den=False, ws=No
 
 
 def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, flags=0, want_p=False, ws=None,
-                model_out=None, loglik=None):
+                model_out=None, loglik=None, ctx=None):
     """Algorithm 1: n_iter iterations of stages 1-5.  Returns dict(model, loglik [n_iter] float64, P or None)."""
     n = model.shape[0]
     m = _Model(n, _dev(model, torch.float32, "model"))
@@ -279,12 +324,12 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
     p = torch.empty((rot.n_rot, ld), dtype=torch.float32, device=dev) if want_p else None
     ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, chunk, flags)
     _check(load().emc_iterate(m, det, rot, pat, n_iter, n_pat_chunk, _dev(model_out, torch.float32, "model_out"),
-                              p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
-           "emc_iterate")
+                              p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream(),
+                              _ctx(ctx, flags)), "emc_iterate")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
 
 
-def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None):
+def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None, ctx=None):
     """Algorithm 1 with the paper's Gaussian likelihood and fluence (eqs. 2.2-2.6).  Returns dict(model, loglik, P)."""
     n = model.shape[0]
     m = _Model(n, _dev(model, torch.float32, "model"))
@@ -298,12 +343,12 @@ def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, 
     p = torch.empty((rot.n_rot, ld), dtype=torch.float32, device=dev) if want_p else None
     ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, pat.n_pat, flags)
     _check(load().emc_iterate_gaussian(m, det, rot, pat, n_iter, float(sigma), model_out.data_ptr(),
-                                       p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream()),
-           "emc_iterate_gaussian")
+                                       p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream(),
+                                       _ctx(ctx, flags)), "emc_iterate_gaussian")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
 
 
-def emc_refine(model, q, mask, levels, counts, n_iter, threshold=0.01, n_pat_chunk=0, flags=0, ws=None):
+def emc_refine(model, q, mask, levels, counts, n_iter, threshold=0.01, n_pat_chunk=0, flags=0, ws=None, ctx=None):
     """Adaptive EMC (section 3.4, eq. 3.1).  `levels` = [(quat [R,4], weight [R] or None), ...] from coarse to
     fine.  Returns dict(model, loglik [n_iter] float64 tensor, level = list of the list index of every iteration)."""
     n = model.shape[0]
@@ -318,7 +363,7 @@ def emc_refine(model, q, mask, levels, counts, n_iter, threshold=0.01, n_pat_chu
     ws, wp, wb = _ws(ws, n, det.n_pix, max(r.n_rot for r in rots), chunk, flags)
     _check(load().emc_refine(m, det, rots, len(levels), pat, n_iter, float(threshold), n_pat_chunk,
                              model_out.data_ptr(), model_tmp.data_ptr(), loglik.data_ptr(), level, flags, wp, wb,
-                             _stream()), "emc_refine")
+                             _stream(), _ctx(ctx, flags)), "emc_refine")
     return dict(model=model_out, loglik=loglik, level=list(level), ws=ws)
 
 
@@ -327,11 +372,12 @@ def emc_check(ws):
     _check(load().emc_check(ws.data_ptr(), _stream()), "emc_check")
 
 
-def emc_profile_read() -> dict:
-    """Per-stage device milliseconds and span counts recorded under EMC_PROFILE_STAGES; resets."""
+def emc_profile_read(ctx=None) -> dict:
+    """Per-stage device milliseconds and span counts recorded under EMC_PROFILE_STAGES in `ctx` (default: the
+    binding's own context); resets."""
     ms = (c_double * len(STAGES))()
     spans = (c_int * len(STAGES))()
-    _check(load().emc_profile_read(ms, spans), "emc_profile_read")
+    _check(load().emc_profile_read((ctx or default_context()).handle, ms, spans), "emc_profile_read")
     return {name: (ms[i], spans[i]) for i, name in enumerate(STAGES)}
 
 
@@ -341,3 +387,7 @@ def emc_launch_count() -> int:
 
 def emc_version() -> str:
     return load().emc_version().decode()
+
+
+__all__ = sorted(n for n in dir() if n.startswith(("emc_", "EMC_", "Emc"))) + [
+    "STAGES", "SYMBOLS", "ld_for", "load", "make_workspace", "default_context"]

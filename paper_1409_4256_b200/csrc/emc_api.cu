@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cmath>
+#include <new>
 
 #include "emc_internal.cuh"
 
@@ -19,57 +20,40 @@ emc_status cuda_fail(cudaError_t e, const char *what) {
 }
 void note_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
 
-namespace {
+float log_uniform_of(int n_rot) { return -logf((float)n_rot); }
 
-// ---- optional per-stage CUDA-event timing (EMC_PROFILE_STAGES): events are recorded on the caller's
-// stream around each stage of emc_iterate and summed by emc_profile_read().
-constexpr int kMaxSpans = 8192;
-struct Profiler {
-    cudaEvent_t beg[kMaxSpans], end[kMaxSpans];
-    int stage[kMaxSpans];
+}  // namespace emc
+
+// The caller-created CUDA objects (emc.h): a copy stream with its events for host-resident patterns (chunks cross
+// PCIe into two staging buffers, so that the copy of chunk j + 1 overlaps pack + GEMMs of chunk j) and a pool of event
+// pairs for per-stage timing.  Everything is created in emc_context_create(); no call on the hot path creates anything.
+struct emc_context {
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, entry = nullptr;
+    cudaEvent_t beg[EMC_MAX_SPANS], end[EMC_MAX_SPANS];
+    int stage[EMC_MAX_SPANS];
     int created = 0, used = 0;
 };
-Profiler g_prof;
 
+namespace emc {
+namespace {
+
+// records the context's next event pair around a stage (EMC_PROFILE_STAGES)
 struct Span {
+    emc_context *c = nullptr;
     int slot = -1;
     cudaStream_t st;
-    Span(bool on, int stage, cudaStream_t stream) : st(stream) {
-        if (!on || g_prof.used >= kMaxSpans) return;
-        if (g_prof.used >= g_prof.created) {
-            if (cudaEventCreate(&g_prof.beg[g_prof.created]) != cudaSuccess) return;
-            if (cudaEventCreate(&g_prof.end[g_prof.created]) != cudaSuccess) return;
-            ++g_prof.created;
-        }
-        slot = g_prof.used++;
-        g_prof.stage[slot] = stage;
-        cudaEventRecord(g_prof.beg[slot], st);
+    Span(emc_context *ctx, bool on, int stage, cudaStream_t stream) : st(stream) {
+        if (!on || !ctx || ctx->used >= ctx->created) return;
+        c = ctx;
+        slot = c->used++;
+        c->stage[slot] = stage;
+        cudaEventRecord(c->beg[slot], st);
     }
     ~Span() {
-        if (slot >= 0) cudaEventRecord(g_prof.end[slot], st);
+        if (slot >= 0) cudaEventRecord(c->end[slot], st);
     }
 };
-
-// ---- host-resident patterns (EMC_PATTERNS_ON_HOST): chunks cross PCIe on a side stream into two staging buffers, so
-// the copy of chunk j + 1 overlaps pack + GEMMs of chunk j.  Created on first use; one thread at a time.
-struct Copier {
-    cudaStream_t stream = nullptr;
-    cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, entry = nullptr;
-    bool ok = false;
-};
-Copier g_copy;
-
-emc_status copier_init() {
-    if (g_copy.ok) return EMC_OK;
-    EMC_TRY_CUDA(cudaStreamCreateWithFlags(&g_copy.stream, cudaStreamNonBlocking));
-    for (int i = 0; i < 2; ++i) {
-        EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.ready[i], cudaEventDisableTiming));
-        EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.freed[i], cudaEventDisableTiming));
-    }
-    EMC_TRY_CUDA(cudaEventCreateWithFlags(&g_copy.entry, cudaEventDisableTiming));
-    g_copy.ok = true;
-    return EMC_OK;
-}
 
 size_t count_size(emc_count_type t) { return t == EMC_I32 ? 4 : (t == EMC_U16 ? 2 : 1); }
 
@@ -79,9 +63,9 @@ struct Layout {
     __half *planesL;          // [2][R][ld_p]  logW hi / lo
     float *S;                 // [R]           sum_{p:mask} W
     __half *Kc;               // [Nc][ld_p]    counts, row = pattern
-    void *KT;                 // [P][ld_n]     counts, row = pixel (fp16; bf16 for EMC_UPDATE_BF16X3)
+    __half *KT;               // [P][ld_n]     counts, row = pixel
     float *L;                 // [R][ld_n]
-    void *planesP;            // [2][R][ld_n]  fp16 hi / lo of chunk-scaled P  (or [3] bf16 hi / mid / lo)
+    __half *planesP;          // [2][R][ld_n]  fp16 hi / lo of chunk-scaled P
     float *pscale;            // [ld_n/512][R] inverse chunk scales of planesP
     float *s;                 // [R]
     float *Wnum;              // [R][P]        update numerators -> W'
@@ -105,9 +89,9 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.planesL = a.take<__half>(2 * R * l.ld_p);
     l.S = a.take<float>(R);
     l.Kc = a.take<__half>((size_t)n_chunk * l.ld_p);
-    l.KT = a.take<uint16_t>((size_t)n_pix * l.ld_n);
+    l.KT = a.take<__half>((size_t)n_pix * l.ld_n);
     l.L = a.take<float>(R * l.ld_n);
-    l.planesP = a.take<uint16_t>(3 * R * l.ld_n);
+    l.planesP = a.take<__half>(2 * R * l.ld_n);
     l.pscale = a.take<float>((size_t)ceil_div(l.ld_n, 512) * R);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
@@ -143,9 +127,9 @@ emc_status reset_header(const Layout &l, cudaStream_t st) {
 }
 
 // stats_ready (optional): the normalisation's column statistics go into l.scratch in the same pass, where the
-// kernel that runs supports it (weight = prior weights or null)
+// kernel that runs supports it (weight = prior weights or null; log_uniform = log w of every row in that case)
 emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
-                           unsigned flags, cudaStream_t st, const float *weight = nullptr,
+                           unsigned flags, cudaStream_t st, const float *weight = nullptr, float log_uniform = 0.f,
                            bool *stats_ready = nullptr, const GaussTerms *gauss = nullptr) {
     GemmProblem g;
     g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
@@ -167,20 +151,21 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
         g.stat_z = l.scratch + 2 * rows * l.ld_n;
         g.ld_stat = l.ld_n;
         g.weight = weight;
+        g.log_uniform = log_uniform;
         *stats_ready = ld_out == l.ld_n && gemm_fuses_stats(g, simt);
         if (!*stats_ready) g.stat_m = g.stat_w = g.stat_z = nullptr;
     }
     return launch_plane_gemm(g, simt, st);
 }
 
-emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, bool bf16x3, float *out,
-                           const float *s, int epilogue, unsigned flags, cudaStream_t st) {
+emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *out, const float *s, int epilogue,
+                           unsigned flags, cudaStream_t st) {
     GemmProblem g;
-    g.A = l.planesP; g.B = l.KT; g.n_planes = bf16x3 ? 3 : 2;
+    g.A = l.planesP; g.B = l.KT; g.n_planes = 2;
     g.M = n_rot; g.N = n_pix; g.K = n_pat;
     g.lda = l.ld_n; g.ldb = l.ld_n; g.plane_stride = (size_t)n_rot * l.ld_n;
-    g.a_fmt = g.b_fmt = bf16x3 ? FMT_BF16 : FMT_F16;
-    g.chunk_scale = bf16x3 ? nullptr : l.pscale;
+    g.a_fmt = g.b_fmt = FMT_F16;
+    g.chunk_scale = l.pscale;
     g.out = out; g.ld_out = n_pix; g.rowv = s; g.epilogue = epilogue;
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     return launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st);
@@ -192,6 +177,40 @@ emc_status run_update_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, boo
 using namespace emc;
 
 extern "C" {
+
+emc_status emc_context_create(emc_context **out) {
+    if (!out) return EMC_ERR_ARG;
+    *out = nullptr;
+    emc_context *c = new (std::nothrow) emc_context;
+    if (!c) return EMC_ERR_ARG;
+    auto fail = [&](cudaError_t e, const char *what) {
+        emc_context_destroy(c);
+        return cuda_fail(e, what);
+    };
+    cudaError_t e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return fail(e, "cudaStreamCreateWithFlags");
+    cudaEvent_t *plain[5] = {&c->ready[0], &c->ready[1], &c->freed[0], &c->freed[1], &c->entry};
+    for (cudaEvent_t *ev : plain)
+        if ((e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) return fail(e, "cudaEventCreateWithFlags");
+    for (int i = 0; i < EMC_MAX_SPANS; ++i) {
+        if ((e = cudaEventCreate(&c->beg[i])) != cudaSuccess) return fail(e, "cudaEventCreate");
+        if ((e = cudaEventCreate(&c->end[i])) != cudaSuccess) { cudaEventDestroy(c->beg[i]); return fail(e, "cudaEventCreate"); }
+        c->created = i + 1;
+    }
+    *out = c;
+    return EMC_OK;
+}
+
+emc_status emc_context_destroy(emc_context *c) {
+    if (!c) return EMC_OK;
+    for (int i = 0; i < c->created; ++i) { cudaEventDestroy(c->beg[i]); cudaEventDestroy(c->end[i]); }
+    cudaEvent_t plain[5] = {c->ready[0], c->ready[1], c->freed[0], c->freed[1], c->entry};
+    for (cudaEvent_t ev : plain)
+        if (ev) cudaEventDestroy(ev);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    delete c;
+    return EMC_OK;
+}
 
 size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags) {
     if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return 0;
@@ -225,9 +244,9 @@ emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *de
     EMC_TRY(reset_header(l, st));
     EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
     EMC_TRY(launch_logw_split(W, idx, det->mask, det->n_pix, n_rot, l.planesL, l.ld_p, l.S, st));
-    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, false, 0,
-                        l.hdr, st));
-    return run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, flags, st);
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, 0, l.hdr, st));
+    EMC_TRY(run_loglik_gemm(l, n_rot, det->n_pix, pat->n_pat, L, ld_n, flags, st));
+    return launch_poison(l.hdr, L, (size_t)n_rot * ld_n, nullptr, 0, st);
 }
 
 emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
@@ -238,7 +257,7 @@ emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, in
         return EMC_ERR_ARG;
     const size_t need = round_up(sizeof(float) * normalize_scratch_floats(rot->n_rot, ld_n), 1024);
     EMC_TRY(check_ws(ws, ws_bytes, need));
-    return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, false, 0, nullptr, s, loglik,
+    return launch_normalize(L, rot->weight, rot->n_rot, n_pat, ld_n, P, nullptr, 0, nullptr, s, loglik,
                             (flags & EMC_ACCUMULATE) != 0, (float *)ws, false, (cudaStream_t)stream);
 }
 
@@ -252,13 +271,12 @@ emc_status emc_update(const float *P, int ld_n, const float *s, const emc_detect
     cudaStream_t st = (cudaStream_t)stream;
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, 0, det->n_pix, n_rot, pat->n_pat, 0).total));
     const Layout l = carve(ws, 0, det->n_pix, n_rot, pat->n_pat, 0);
-    const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
     EMC_TRY(reset_header(l, st));
-    EMC_TRY(launch_p_split(P, n_rot, pat->n_pat, ld_n, l.planesP, l.ld_n, bf16x3, (size_t)n_rot * l.ld_n, l.pscale, st));
-    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, bf16x3, l.ld_n,
-                        l.hdr, st));
+    EMC_TRY(launch_p_split(P, n_rot, pat->n_pat, ld_n, l.planesP, l.ld_n, (size_t)n_rot * l.ld_n, l.pscale, st));
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, nullptr, 0, l.KT, l.ld_n, l.hdr, st));
     const int epi = (flags & EMC_ACCUMULATE) ? EPI_ADD : (raw ? EPI_STORE : EPI_DIV_ROW);
-    return run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, bf16x3, Wnew, s, epi, flags, st);
+    EMC_TRY(run_update_gemm(l, n_rot, det->n_pix, pat->n_pat, Wnew, s, epi, flags, st));
+    return launch_poison(l.hdr, Wnew, (size_t)n_rot * det->n_pix, nullptr, 0, st);
 }
 
 emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detector *det,
@@ -276,11 +294,13 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
 static emc_status iterate_impl(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                                const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
                                float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
-                               size_t ws_bytes, void *stream, float sigma) {
+                               size_t ws_bytes, void *stream, emc_context *ctx, float sigma) {
     const bool gauss = sigma > 0.f;
     if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_iter <= 0 || !model_out ||
         model_out == model->model || !loglik || n_pat_chunk < 0)
         return EMC_ERR_ARG;
+    if ((flags & (EMC_PATTERNS_ON_HOST | EMC_PROFILE_STAGES)) && !ctx) return EMC_ERR_ARG;
+    if (n_iter > 256) return EMC_ERR_UNSUPPORTED;
     const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
     const int chunk = (n_pat_chunk == 0 || n_pat_chunk > n_pat) ? n_pat : n_pat_chunk;
     if (!sizes_ok(n, n_pix, n_rot, chunk)) return EMC_ERR_UNSUPPORTED;
@@ -292,12 +312,12 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes).total));
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
-    if (gauss && (n_chunks != 1 || (flags & (EMC_UPDATE_BF16X3 | EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
-    const GaussTerms gterms = {l.S, l.Asq, l.Asq + l.ld_n, gauss ? 1.f / (2.f * sigma * sigma) : 0.f};
+    if (gauss && (n_chunks != 1 || (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
+    const float log_uniform = log_uniform_of(n_rot);
+    const GaussTerms gterms = {l.S, l.Asq, l.Asq + l.ld_n, gauss ? 1.f / (2.f * sigma * sigma) : 0.f, log_uniform};
     const GaussTerms *gt = gauss ? &gterms : nullptr;
     cudaStream_t st = (cudaStream_t)stream;
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
-    const bool bf16x3 = (flags & EMC_UPDATE_BF16X3) != 0;
     const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
 
     EMC_TRY(reset_header(l, st));
@@ -316,20 +336,19 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         d0 = (pipelined ? j : j % n_chunks) * step;
         nc = n_pat - d0 < step ? n_pat - d0 : step;
     };
-    auto issue_copy = [&](int j) -> emc_status {              // host -> staging buffer j & 1, on the side stream
+    auto issue_copy = [&](int j) -> emc_status {              // host -> staging buffer j & 1, on the context's copy stream
         int d0, nc;
         job_range(j, d0, nc);
         const int b = j & 1;
-        if (j >= 2) EMC_TRY_CUDA(cudaStreamWaitEvent(g_copy.stream, g_copy.freed[b], 0));   // pack j - 2 has read it
+        if (j >= 2) EMC_TRY_CUDA(cudaStreamWaitEvent(ctx->copy_stream, ctx->freed[b], 0));   // pack j - 2 has read it
         EMC_TRY_CUDA(cudaMemcpyAsync((uint8_t *)l.stage + b * stage_one, (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz,
-                                     (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, g_copy.stream));
-        EMC_TRY_CUDA(cudaEventRecord(g_copy.ready[b], g_copy.stream));
+                                     (size_t)nc * n_pix * csz, cudaMemcpyHostToDevice, ctx->copy_stream));
+        EMC_TRY_CUDA(cudaEventRecord(ctx->ready[b], ctx->copy_stream));
         return EMC_OK;
     };
     if (on_host) {
-        EMC_TRY(copier_init());
-        EMC_TRY_CUDA(cudaEventRecord(g_copy.entry, st));      // earlier work on `st` may still read the staging buffers
-        EMC_TRY_CUDA(cudaStreamWaitEvent(g_copy.stream, g_copy.entry, 0));
+        EMC_TRY_CUDA(cudaEventRecord(ctx->entry, st));        // earlier work on `st` may still read the staging buffers
+        EMC_TRY_CUDA(cudaStreamWaitEvent(ctx->copy_stream, ctx->entry, 0));
         EMC_TRY(issue_copy(0));
     }
     int job = 0;
@@ -337,7 +356,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     for (int it = 0; it < n_iter; ++it) {
         // stage 1: Expand, with logW planes and S fused in
         {
-            Span sp(prof, EMC_STAGE_EXPAND, st);
+            Span sp(ctx, prof, EMC_STAGE_EXPAND, st);
             EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
             EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
                                   l.planesL, l.ld_p, l.S, l.blocked, st, gauss));
@@ -355,23 +374,23 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
             Layout v = l;                               // view of the buffers this part works in
             if (sub_ranges) {
                 v.Kc = l.Kc + (size_t)d0 * l.ld_p;
-                v.KT = (uint16_t *)l.KT + d0;
+                v.KT = l.KT + d0;
                 v.L = l.L + d0;
-                v.planesP = (uint16_t *)l.planesP + d0;
+                v.planesP = l.planesP + d0;
                 v.pscale = l.pscale + (size_t)(d0 / 512) * n_rot;
                 v.scratch = l.scratch + d0;
             }
             if (n_chunks > 1 || it == 0) {          // one resident chunk is packed once for all iterations
-                Span sp(prof, EMC_STAGE_PACK, st);
+                Span sp(ctx, prof, EMC_STAGE_PACK, st);
                 const uint8_t *src = (const uint8_t *)pat->counts + (size_t)d0 * n_pix * csz;
                 if (on_host) {
                     const int b = job & 1;
                     if (job + 1 < n_jobs) EMC_TRY(issue_copy(job + 1));      // overlaps this part's pack and GEMMs
-                    EMC_TRY_CUDA(cudaStreamWaitEvent(st, g_copy.ready[b], 0));
+                    EMC_TRY_CUDA(cudaStreamWaitEvent(st, ctx->ready[b], 0));
                     src = (const uint8_t *)l.stage + b * stage_one;
                 }
-                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, bf16x3, l.ld_n, l.hdr, st));
-                if (on_host) EMC_TRY_CUDA(cudaEventRecord(g_copy.freed[job & 1], st));
+                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, l.ld_n, l.hdr, st));
+                if (on_host) EMC_TRY_CUDA(cudaEventRecord(ctx->freed[job & 1], st));
                 if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
                     EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * 2 * l.ld_n, st));
                     EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, gterms.inv2s2, l.Asq, l.Asq + l.ld_n, st));
@@ -381,60 +400,64 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
             // stage 2: L = logW K^T - S  (+ the column max / sum-exp partials of stage 3 from the same epilogue)
             bool stats_ready = false;
             {
-                Span sp(prof, EMC_STAGE_LOGLIK, st);
-                EMC_TRY(run_loglik_gemm(v, n_rot, n_pix, nc, v.L, l.ld_n, flags, st, rot->weight, &stats_ready, gt));
+                Span sp(ctx, prof, EMC_STAGE_LOGLIK, st);
+                EMC_TRY(run_loglik_gemm(v, n_rot, n_pix, nc, v.L, l.ld_n, flags, st, rot->weight, log_uniform, &stats_ready, gt));
             }
             // stage 3: responsibilities of this part; s and LL add up over parts
             float *p_dst = (P_out && it == n_iter - 1) ? P_out + (sub_ranges ? d0 : 0) : nullptr;
             {
-                Span sp(prof, EMC_STAGE_NORMALIZE, st);
-                EMC_TRY(launch_normalize(v.L, rot->weight, n_rot, nc, l.ld_n, p_dst, v.planesP, bf16x3,
-                                         (size_t)n_rot * l.ld_n, v.pscale, l.s, loglik + it, true, v.scratch, stats_ready,
-                                         st, gt, l.ld_n - (sub_ranges ? d0 : 0)));
+                Span sp(ctx, prof, EMC_STAGE_NORMALIZE, st);
+                EMC_TRY(launch_normalize(v.L, rot->weight, n_rot, nc, l.ld_n, p_dst, v.planesP, (size_t)n_rot * l.ld_n, v.pscale,
+                                         l.s, loglik + it, true, v.scratch, stats_ready, st, gt,
+                                         l.ld_n - (sub_ranges ? d0 : 0), log_uniform));
             }
             // stage 4: update numerators (divided by s[r] in the epilogue when there is one part)
             const int epi = n_parts == 1 ? EPI_DIV_ROW : (c == 0 ? EPI_STORE : EPI_ADD);
             {
-                Span sp(prof, EMC_STAGE_UPDATE, st);
-                EMC_TRY(run_update_gemm(v, n_rot, n_pix, nc, bf16x3, l.Wnum, l.s, epi, flags, st));
+                Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
+                EMC_TRY(run_update_gemm(v, n_rot, n_pix, nc, l.Wnum, l.s, epi, flags, st));
             }
         }
         if (n_parts > 1) {
-            Span sp(prof, EMC_STAGE_UPDATE, st);
+            Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
             EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
         }
         // stage 5: Compress
         {
-            Span sp(prof, EMC_STAGE_COMPRESS, st);
+            Span sp(ctx, prof, EMC_STAGE_COMPRESS, st);
             const DenCache cache = {l.active, (int *)(l.active + ceil_div(n_rot, 32)), it == 0};
             EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
                                     model_out, nullptr, st, &cache));
         }
         model_cur = model_out;
     }
+    // a count out of range (seen by the pack kernels above): every result of the call becomes NaN
+    EMC_TRY(launch_poison(l.hdr, model_out, (size_t)n * n * n, loglik, n_iter, st));
+    if (P_out) EMC_TRY(launch_poison(l.hdr, P_out, (size_t)n_rot * ld_n, nullptr, 0, st));
     return EMC_OK;
 }
 
 emc_status emc_iterate(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                        const emc_patterns *pat, int n_iter, int n_pat_chunk, float *model_out,
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
-                       size_t ws_bytes, void *stream) {
+                       size_t ws_bytes, void *stream, emc_context *ctx) {
     return iterate_impl(model, det, rot, pat, n_iter, n_pat_chunk, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes,
-                        stream, 0.f);
+                        stream, ctx, 0.f);
 }
 
 emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                                 const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
-                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream) {
+                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
+                                emc_context *ctx) {
     if (!(sigma > 0.f)) return EMC_ERR_ARG;
     return iterate_impl(model, det, rot, pat, n_iter, 0, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes, stream,
-                        sigma);
+                        ctx, sigma);
 }
 
 emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc_rotations *levels,
                       int n_levels, const emc_patterns *pat, int n_iter, double threshold, int n_pat_chunk,
                       float *model_out, float *model_tmp, double *loglik, int32_t *level_of_iter,
-                      unsigned flags, void *ws, size_t ws_bytes, void *stream) {
+                      unsigned flags, void *ws, size_t ws_bytes, void *stream, emc_context *ctx) {
     if (!model || !model->model || !levels || n_levels <= 0 || n_iter <= 0 || !model_out || !model_tmp ||
         model_out == model_tmp || model_out == model->model || model_tmp == model->model || !loglik ||
         !level_of_iter || !(threshold >= 0.0))
@@ -450,7 +473,7 @@ emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc
         float *dst = bufs[(n_iter - 1 - i) & 1];                    // the last iteration lands in model_out
         const emc_model cur = {model->n, src};
         EMC_TRY(emc_iterate(&cur, det, &levels[level], pat, 1, n_pat_chunk, dst, nullptr, 0, loglik + i, flags, ws,
-                            ws_bytes, stream));
+                            ws_bytes, stream, ctx));
         level_of_iter[i] = level;
         double ll = 0.0;
         EMC_TRY_CUDA(cudaMemcpyAsync(&ll, loglik + i, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -472,19 +495,19 @@ emc_status emc_check(void *ws, void *stream) {
     return h.max_count > 0 ? EMC_ERR_COUNT_RANGE : EMC_OK;      // the pack kernel records only counts over its limit
 }
 
-emc_status emc_profile_read(double *ms, int *spans) {
-    if (!ms || !spans) return EMC_ERR_ARG;
+emc_status emc_profile_read(emc_context *c, double *ms, int *spans) {
+    if (!c || !ms || !spans) return EMC_ERR_ARG;
     for (int i = 0; i < EMC_N_STAGES; ++i) { ms[i] = 0.0; spans[i] = 0; }
     emc_status rc = EMC_OK;
-    for (int i = 0; i < g_prof.used; ++i) {
+    for (int i = 0; i < c->used; ++i) {
         float t = 0.f;
-        cudaError_t e = cudaEventSynchronize(g_prof.end[i]);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, g_prof.beg[i], g_prof.end[i]);
+        cudaError_t e = cudaEventSynchronize(c->end[i]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, c->beg[i], c->end[i]);
         if (e != cudaSuccess) { rc = cuda_fail(e, "emc_profile_read"); break; }
-        ms[g_prof.stage[i]] += (double)t;
-        spans[g_prof.stage[i]] += 1;
+        ms[c->stage[i]] += (double)t;
+        spans[c->stage[i]] += 1;
     }
-    g_prof.used = 0;
+    c->used = 0;
     return rc;
 }
 
@@ -504,6 +527,6 @@ const char *emc_strerror(emc_status s) {
 
 const char *emc_last_cuda_error(void) { return g_err; }
 
-const char *emc_version(void) { return "libemc 0.1 (sm_100a)"; }
+const char *emc_version(void) { return "libemc 0.2 (sm_100a)"; }
 
 }  // extern "C"

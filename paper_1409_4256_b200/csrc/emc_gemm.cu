@@ -6,7 +6,7 @@
 //        W'[r,p] = sum_d P[r,d] K[d,p] / s[r]            M = R, N = pixels,   K-dim = patterns
 //
 // Both are "plane GEMMs": the real-valued operand A (logW or P) is a sum of n_planes 16-bit
-// planes (hi + lo [+ lo2]); the count operand B is exact in ONE 16-bit plane, so every product is
+// planes (hi + lo); the count operand B is exact in ONE 16-bit plane, so every product is
 // exact in fp32 and the only rounding is the fp32 accumulation in TMEM:
 //
 //        acc[m,n] = sum_pl sum_k A[pl][m][k] * B[n][k]
@@ -67,7 +67,7 @@ struct GemmArgs {
     float *stat_m, *stat_w, *stat_z;   // [ceil(M/32)][ld_stat]: reference pair (L, log w) and sum
     int ld_stat;
     const float *weight;        // [M] prior weights w_r or null = uniform
-    float log_uniform;          // -log(M)
+    float log_uniform;          // log(1/R) for weight == null (R = all rotations of the problem, not of this launch)
 };
 
 // Gaussian model (EPI_GAUSS, STATS = 2): out = B = acc; the statistics are taken of Q = (B^2 / A_d - C_r) / (2 sigma^2).
@@ -916,7 +916,7 @@ emc_status launch_tc_pair(const GemmProblem &g, cudaStream_t st) {
     a.idesc = (1u << 4) | ((uint32_t)g.a_fmt << 7) | ((uint32_t)g.b_fmt << 10) | ((uint32_t)(BN >> 3) << 17) |
               ((uint32_t)(PAIR_M >> 4) << 24);
     a.stat_m = g.stat_m; a.stat_w = g.stat_w; a.stat_z = g.stat_z; a.ld_stat = g.ld_stat; a.weight = g.weight;
-    a.log_uniform = -logf((float)g.M);
+    a.log_uniform = g.log_uniform;
     a.tma_out = a.vec_ok;
     if (STATS && !a.tma_out) return EMC_ERR_ARG;             // gemm_fuses_stats() said no
     CUtensorMap tmC = tmA;                                    // placeholder when the output is not TMA-addressable
@@ -973,7 +973,6 @@ emc_status launch_plane_gemm(const GemmProblem &g, bool simt_debug, cudaStream_t
         const long c192 = (long)ceil_div(mt * ceil_div(g.N, 192), sms) * 192;
         return c192 < c256 ? launch_tc<2, 192, 4>(g, st) : launch_tc<2, 256, 3>(g, st);
     }
-    if (g.n_planes == 3) return launch_tc<3, 192, 3>(g, st);
     return EMC_ERR_UNSUPPORTED;
 }
 

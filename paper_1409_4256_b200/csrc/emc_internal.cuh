@@ -79,11 +79,14 @@ emc_status launch_pack_geometry(const float *q, const uint8_t *mask, int n_pix, 
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
 
-// Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] fp16 or bf16
-// (row = pixel), masked pixels zeroed, largest unmasked count recorded in hdr->max_count.
+// Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] fp16
+// (row = pixel), masked pixels zeroed, an unmasked count above EMC_MAX_COUNT recorded in hdr->max_count.
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
-                       const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
+                       const uint8_t *mask, __half *Kc, int ld_p, __half *KT, int ld_n,
                        WsHeader *hdr, cudaStream_t st);
+// fills out[0..n) (floats) with NaN if hdr->max_count != 0: a result computed from clamped counts must not be
+// consumed unnoticed (emc.h, conventions)
+emc_status launch_poison(const WsHeader *hdr, float *out, size_t n, double *out64, int n64, cudaStream_t st);
 
 // A[d] = sum_p Kc[d][p]^2 (fluence numerators of the Gaussian model, eq. 2.6) as g_col[d] = 1 / (2 sigma^2 A_d) and
 // ia_col[d] = 1 / A_d (both 0 where A_d = 0)
@@ -94,7 +97,7 @@ emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float 
 struct GemmProblem {
     const void *A;      // [n_planes][M][lda] 16-bit elements, K-major
     const void *B;      // [N][ldb] 16-bit elements, K-major
-    int n_planes;       // 2 or 3
+    int n_planes;       // 2
     int M, N, K;
     int lda, ldb;       // row pitches in elements (multiples of 8)
     size_t plane_stride;  // elements between planes of A
@@ -112,6 +115,7 @@ struct GemmProblem {
     float *stat_m = nullptr, *stat_w = nullptr, *stat_z = nullptr;
     int ld_stat = 0;
     const float *weight = nullptr;
+    float log_uniform = 0.f;          // log_uniform_of(all rotations) for weight == null
     const float *gauss_g = nullptr;   // EPI_GAUSS: [N] g_d = 1 / (2 sigma^2 A_d)
     float inv2s2 = 0.f;               // EPI_GAUSS: 1 / (2 sigma^2)
     bool one_cta = false;   // EMC_GEMM_1CTA: the one-CTA kernel instead of CTA pairs (cta_group::2)
@@ -141,22 +145,28 @@ __device__ __forceinline__ float gauss_row_term(float log_w, float c_row, float 
 
 // Normalise (emc_normalize.cu).  scratch = normalize_scratch_floats() floats.  `planes` (optional) receives the
 // operand planes of P for the update GEMM: two fp16 planes scaled per (row, 512-column chunk) with the inverse
-// scales in chunk_inv_scale [ceil(ld_n/512)][R], or (bf16x3) three unscaled bf16 planes.
+// scales in chunk_inv_scale [ceil(ld_n/512)][R].
 // Gaussian model: L holds B = W K^T; c_row [R] = sum_p W^2, A_d = sum_p K^2 enters as two column factors, inv2s2 = 1 / (2 sigma^2)
 struct GaussTerms {
     const float *c_row, *g_col, *ia_col;   // g_col = 1 / (2 sigma^2 A_d), ia_col = 1 / A_d
     float inv2s2;
+    float log_uniform;                     // log_uniform_of(R): the same float in the GEMM's statistics and the second sweep
 };
+// log(1/R) for weight == NULL, evaluated ONCE on the host and handed to every kernel that needs it (the row terms of
+// the Gaussian model nearly cancel: a 1-ulp difference between two evaluations would show in sum_r P)
+float log_uniform_of(int n_rot);
 size_t normalize_scratch_floats(int n_rot, int ld_n);
 int normalize_stat_rows(int n_rot);   // scratch = part_m, part_w, part_z [rows][ld_n] each, then col_m, col_w, col_iz [ld_n] each
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
-                            float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
+                            float *P, __half *planes, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss = nullptr, int n_store = 0);
+                            cudaStream_t st, const GaussTerms *gauss = nullptr, int n_store = 0, float log_uniform = 0.f);
+// log_uniform: log w of every row when weight == null; 0 = log_uniform_of(n_rot) (set it when the rows are a chunk of a
+// longer rotation list)
 // n_store: columns of a row the call may write (planes padding, column arrays); 0 = ld_n.  Smaller when L, planes and
 // scratch are views that start inside a row (emc_api.cu, pipelined first iteration).
 // operand planes of a given P (stage API of emc_update).
-emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
+emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half *planes, int ld_pl,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);

@@ -47,6 +47,7 @@ struct ColStat {
 };
 __device__ __forceinline__ float rel_exponent(float L, float lw, float mL, float mw) { return (L - mL) + (lw - mw); }
 __device__ __forceinline__ void online(float L, float lw, ColStat &c) {
+    if (!(L + lw > -INFINITY)) return;                 // w_r = 0 (log w = -inf) or L = -inf: the row takes no part
     if (L + lw > c.mL + c.mw) {
         c.z = c.z * expf(rel_exponent(c.mL, c.mw, L, lw)) + 1.f;      // z = 0 while the pair is (-inf, 0): 0 * 0
         c.mL = L;
@@ -70,7 +71,7 @@ __device__ __forceinline__ void merge(ColStat &a, const ColStat &b) {
 // sweep 1: partial statistics of every column over the rows of one split (stage API; inside emc_iterate the
 // log-likelihood GEMM's epilogue writes the same partials, one per 32 rows)
 __global__ void __launch_bounds__(kThreads)
-colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
+colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, float log_uniform, int n_rot, int n_pat,
                 int ld_n, int rows_per_split, float *__restrict__ part_m, float *__restrict__ part_w,
                 float *__restrict__ part_z) {
     __shared__ float sm_m[kWarps][kColsPerBlock], sm_w[kWarps][kColsPerBlock], sm_z[kWarps][kColsPerBlock];
@@ -78,7 +79,6 @@ colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, i
     const int d = blockIdx.x * kColsPerBlock + lane * kVec;
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
-    const float log_uniform = -logf((float)n_rot);
     ColStat c[kVec];
 #pragma unroll
     for (int j = 0; j < kVec; ++j) c[j] = ColStat{-INFINITY, 0.f, 0.f};
@@ -127,13 +127,15 @@ colstats_kernel(const float *__restrict__ L, const float *__restrict__ weight, i
 }
 
 // ---- operand planes of P for the update contraction -------------------------------------------
-// Default (PLANES_F16_SCALED): two fp16 planes with one power-of-two scale per (row, 512-column
-// chunk): the chunk is scaled so that its largest value lies in [2^14, 2^15), then hi = fp16(v),
-// lo = fp16(v - hi).  The update GEMM accumulates each 512-element K chunk separately and applies
-// the inverse scale when it drains the chunk (exact), so fp16's narrow exponent only has to span
-// one chunk of one row: 22 significand bits for every value within 2^-17 of the chunk maximum and
-// an absolute error below 2^-40 of the chunk maximum for the rest.
-// Opt-in (EMC_UPDATE_BF16X3): three unscaled bf16 planes (24 bits at every magnitude, 3 MMAs).
+// Two fp16 planes with one power-of-two scale per (row, 512-column chunk): the chunk is scaled so
+// that its largest value lies in [2^14, 2^15), then hi = fp16(v), lo = fp16(v - hi).  The update
+// GEMM accumulates each 512-element K chunk separately and applies the inverse scale when it drains
+// the chunk (exact), so fp16's narrow exponent only has to span one chunk of one row: 22
+// significand bits for every value within 2^-17 of the chunk maximum and an absolute error below
+// 2^-40 of the chunk maximum for the rest.  P covers float32's whole normal range
+// [2^-126, 1] (EMC_P_MIN), so the scale 2^k, k = 14 - floor(log2 max) <= 140, is applied as two exact
+// factors 2^(k/2) 2^(k - k/2) and its inverse 2^-k (a float32 subnormal below 2^-126, still an exact
+// power of two down to 2^-149) multiplies the chunk's sum in the GEMM's drain.
 constexpr int kChunkCols = 512;               // = the GEMM's K chunk (kChunkKBlocks * 64)
 constexpr int kGroups = kChunkCols / kColsPerBlock;   // float4 groups per lane per row
 
@@ -148,15 +150,22 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-// scale = 2^(14 - floor(log2 mx)) and its inverse; mx = 0 gives 1, 1
-__device__ __forceinline__ void chunk_scale_of(float mx, float &scale, float &inv) {
+// exact 2^e for -149 <= e <= 127 (subnormal below -126)
+__device__ __forceinline__ float pow2_exact(int e) {
+    return e >= -126 ? __uint_as_float((uint32_t)(e + 127) << 23) : __uint_as_float(1u << (e + 149));
+}
+// 2^k = s1 * s2 with k = 14 - floor(log2 mx), and inv = 2^-k; mx = 0 gives 1, 1, 1.  mx is a float32 in
+// [2^-126, 2^15) here (P >= EMC_P_MIN; the Gaussian operand P / phi may be a subnormal: its exponent field reads
+// -127 and the chunk simply keeps fewer bits).
+__device__ __forceinline__ void chunk_scale_of(float mx, float &s1, float &s2, float &inv) {
     if (mx > 0.f) {
-        const int ex = (int)((__float_as_uint(mx) >> 23) & 0xffu) - 127;      // mx >= 2^-100: normal
-        scale = __uint_as_float((uint32_t)(14 - ex + 127) << 23);
-        inv = __uint_as_float((uint32_t)(ex - 14 + 127) << 23);
+        const int k = 14 - ((int)((__float_as_uint(mx) >> 23) & 0xffu) - 127);      // -1 <= k <= 141
+        const int k1 = k / 2;
+        s1 = pow2_exact(k1);
+        s2 = pow2_exact(k - k1);
+        inv = pow2_exact(-k);
     } else {
-        scale = 1.f;
-        inv = 1.f;
+        s1 = s2 = inv = 1.f;
     }
 }
 
@@ -172,48 +181,25 @@ __device__ __forceinline__ void store4_f16_pair(const float (&v)[4], __half *__r
     *reinterpret_cast<uint2 *>(planes + plane_stride + o) = *reinterpret_cast<const uint2 *>(l);
 }
 
-__device__ __forceinline__ void store4_bf16_x3(const float (&p)[4], __nv_bfloat16 *__restrict__ planes,
-                                               size_t plane_stride, size_t o) {
-    float rem[4];
-    __nv_bfloat16 h[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) { h[j] = __float2bfloat16_rn(p[j]); rem[j] = p[j] - __bfloat162float(h[j]); }
-    *reinterpret_cast<uint2 *>(planes + o) = *reinterpret_cast<const uint2 *>(h);
-#pragma unroll
-    for (int j = 0; j < 4; ++j) { h[j] = __float2bfloat16_rn(rem[j]); rem[j] -= __bfloat162float(h[j]); }
-    *reinterpret_cast<uint2 *>(planes + plane_stride + o) = *reinterpret_cast<const uint2 *>(h);
-#pragma unroll
-    for (int j = 0; j < 4; ++j) h[j] = __float2bfloat16_rn(rem[j]);
-    *reinterpret_cast<uint2 *>(planes + 2 * plane_stride + o) = *reinterpret_cast<const uint2 *>(h);
-}
-
 // One row x one 512-column chunk held by a warp (p[g][4] = columns d0 + g*128 + lane*4 ..+3): writes the
-// operand planes and, for the scaled format, the chunk's inverse scale.
+// operand planes and the chunk's inverse scale.
 __device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int lane, int ld_pl, size_t row_off,
-                                             void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                                             __half *__restrict__ planes, size_t plane_stride,
                                              float *__restrict__ inv_scale_out) {
-    if (bf16x3) {
-#pragma unroll
-        for (int g = 0; g < kGroups; ++g) {
-            const int d = d0 + g * kColsPerBlock + lane * kVec;
-            if (d < ld_pl) store4_bf16_x3(p[g], (__nv_bfloat16 *)planes, plane_stride, row_off + d);
-        }
-        return;
-    }
     float mx = 0.f;
 #pragma unroll
     for (int g = 0; g < kGroups; ++g)
         mx = fmaxf(mx, fmaxf(fmaxf(p[g][0], p[g][1]), fmaxf(p[g][2], p[g][3])));
     mx = warp_max(mx);
-    float scale, inv;
-    chunk_scale_of(mx, scale, inv);
+    float s1, s2, inv;
+    chunk_scale_of(mx, s1, s2, inv);
     if (lane == 0) *inv_scale_out = inv;
 #pragma unroll
     for (int g = 0; g < kGroups; ++g) {
         const int d = d0 + g * kColsPerBlock + lane * kVec;
         if (d < ld_pl) {
-            const float v[4] = {p[g][0] * scale, p[g][1] * scale, p[g][2] * scale, p[g][3] * scale};
-            store4_f16_pair(v, (__half *)planes, plane_stride, row_off + d);
+            const float v[4] = {(p[g][0] * s1) * s2, (p[g][1] * s1) * s2, (p[g][2] * s1) * s2, (p[g][3] * s1) * s2};
+            store4_f16_pair(v, planes, plane_stride, row_off + d);
         }
     }
 }
@@ -275,7 +261,7 @@ template <bool UNIFORM>
 __global__ void __launch_bounds__(kThreads, UNIFORM ? 3 : 2)
 normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, int n_rot, int n_pat,
                  int ld_n, int n_store, int rows_per_split, const float *__restrict__ col_m, const float *__restrict__ col_w,
-                 const float *__restrict__ col_iz, float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                 const float *__restrict__ col_iz, float *__restrict__ P, __half *__restrict__ planes, size_t plane_stride,
                  float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d0 = blockIdx.x * kChunkCols;
@@ -333,7 +319,7 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
             if (P && ok[g]) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
         }
         if (planes)
-            write_planes(p, d0, lane, n_store, row_off, planes, bf16x3, plane_stride,
+            write_planes(p, d0, lane, n_store, row_off, planes, plane_stride,
                          chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
         if (s) {
             sum = warp_sum(sum);
@@ -348,16 +334,15 @@ normalize_kernel(const float *__restrict__ L, const float *__restrict__ weight, 
 // Same thread layout as normalize_kernel; column data is re-read per row (L1-resident) to keep registers free.
 __global__ void __launch_bounds__(kThreads, 2)
 normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ weight, const float *__restrict__ c_row,
-                       const float *__restrict__ g_col, const float *__restrict__ ia_col, float inv2s2, int n_rot, int n_pat, int ld_n, int n_store,
-                       int rows_per_split,
+                       const float *__restrict__ g_col, const float *__restrict__ ia_col, float inv2s2, float log_uniform,
+                       int n_rot, int n_pat, int ld_n, int n_store, int rows_per_split,
                        const float *__restrict__ col_m, const float *__restrict__ col_w, const float *__restrict__ col_iz,
-                       float *__restrict__ P, void *__restrict__ planes, int bf16x3, size_t plane_stride,
+                       float *__restrict__ P, __half *__restrict__ planes, size_t plane_stride,
                        float *__restrict__ chunk_inv_scale, float *__restrict__ s) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int d0 = blockIdx.x * kChunkCols;
     const int r_lo = blockIdx.y * rows_per_split;
     const int r_hi = min(n_rot, r_lo + rows_per_split);
-    const float log_uniform = -logf((float)n_rot);
     // the column statistics stay in registers for the whole row range; the two Gaussian column factors are re-read per
     // row (L1-resident); the next row of B is fetched while the current one is worked on
     const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -418,7 +403,7 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
             if (P && ok) *reinterpret_cast<float4 *>(P + row_off + d) = make_float4(p[g][0], p[g][1], p[g][2], p[g][3]);
         }
         if (planes)
-            write_planes(q, d0, lane, n_store, row_off, planes, bf16x3, plane_stride,
+            write_planes(q, d0, lane, n_store, row_off, planes, plane_stride,
                          chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
         if (s) {
             sum = warp_sum(sum);
@@ -429,8 +414,8 @@ normalize_gauss_kernel(const float *__restrict__ B, const float *__restrict__ we
 
 // operand planes of a given P (stage API of emc_update).  grid = (ceil(N/512), ceil(R/8)); warp per row.
 __global__ void __launch_bounds__(kThreads)
-p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, void *__restrict__ planes, int ld_pl,
-               int bf16x3, size_t plane_stride, float *__restrict__ chunk_inv_scale) {
+p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, __half *__restrict__ planes, int ld_pl,
+               size_t plane_stride, float *__restrict__ chunk_inv_scale) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int r = blockIdx.y * kWarps + warp;
     if (r >= n_rot) return;
@@ -446,7 +431,7 @@ p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, void
             p[g][j] = pj;
         }
     }
-    write_planes(p, d0, lane, ld_pl, (size_t)r * ld_pl, planes, bf16x3, plane_stride,
+    write_planes(p, d0, lane, ld_pl, (size_t)r * ld_pl, planes, plane_stride,
                  chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
 }
 
@@ -473,10 +458,11 @@ size_t normalize_scratch_floats(int n_rot, int ld_n) {
 }
 
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
-                            float *P, void *planes, bool bf16x3, size_t plane_stride, float *chunk_inv_scale,
+                            float *P, __half *planes, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss, int n_store) {
+                            cudaStream_t st, const GaussTerms *gauss, int n_store, float log_uniform) {
     if (n_store <= 0 || n_store > ld_n) n_store = ld_n;          // columns of a row this call may write
+    if (log_uniform == 0.f) log_uniform = log_uniform_of(n_rot);
     if (gauss && !stats_ready) return EMC_ERR_UNSUPPORTED;       // the Gaussian model's statistics come from the GEMM
     const int stat_rows = normalize_stat_rows(n_rot);
     float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
@@ -492,8 +478,8 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
         const int splits = row_splits_for(n_rot, col_blocks);
         const int rows_per_split = ceil_div(n_rot, splits);
         n_splits = ceil_div(n_rot, rows_per_split);
-        colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, rows_per_split,
-                                                                         part_m, part_w, part_z);
+        colstats_kernel<<<dim3(col_blocks, n_splits), kThreads, 0, st>>>(L, weight, log_uniform, n_rot, n_pat, ld_n,
+                                                                         rows_per_split, part_m, part_w, part_z);
         EMC_LAUNCHED();
     }
     float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
@@ -510,24 +496,23 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     const int rows2 = ceil_div(n_rot, splits2);
     const dim3 grid2(chunks, ceil_div(n_rot, rows2));
     if (gauss)
-        normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->g_col, gauss->ia_col, gauss->inv2s2, n_rot, n_pat,
-                                                           ld_n, n_store, rows2, col_m, col_w, col_iz, P, planes, bf16x3 ? 1 : 0,
-                                                           plane_stride, chunk_inv_scale, s);
+        normalize_gauss_kernel<<<grid2, kThreads, 0, st>>>(L, weight, gauss->c_row, gauss->g_col, gauss->ia_col, gauss->inv2s2,
+                                                           gauss->log_uniform, n_rot, n_pat, ld_n, n_store, rows2, col_m, col_w,
+                                                           col_iz, P, planes, plane_stride, chunk_inv_scale, s);
     else if (weight)
         normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, n_store, rows2, col_m, col_w, col_iz, P,
-                                                            planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
+                                                            planes, plane_stride, chunk_inv_scale, s);
     else
         normalize_kernel<true><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, n_store, rows2, col_m, col_w, col_iz, P,
-                                                           planes, bf16x3 ? 1 : 0, plane_stride, chunk_inv_scale, s);
+                                                           planes, plane_stride, chunk_inv_scale, s);
     EMC_LAUNCHED();
     return EMC_OK;
 }
 
-emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, void *planes, int ld_pl, bool bf16x3,
+emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half *planes, int ld_pl,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st) {
     dim3 grid(ceil_div(n_pat, kChunkCols), ceil_div(n_rot, kWarps));
-    p_split_kernel<<<grid, kThreads, 0, st>>>(P, n_rot, n_pat, ld_n, planes, ld_pl, bf16x3 ? 1 : 0, plane_stride,
-                                              chunk_inv_scale);
+    p_split_kernel<<<grid, kThreads, 0, st>>>(P, n_rot, n_pat, ld_n, planes, ld_pl, plane_stride, chunk_inv_scale);
     EMC_LAUNCHED();
     return EMC_OK;
 }

@@ -1,9 +1,9 @@
 // Photon counts K[d][p] -> the exact 16-bit operands of the two contractions:
 //   Kc [N][ld_p] fp16, row = pattern  (B operand of the log-likelihood GEMM, K-dim = pixels)
 //   KT [P][ld_n] fp16, row = pixel    (B operand of the update GEMM,         K-dim = patterns)
-//      (bf16 for the opt-in bf16x3 update)
-// Masked pixels become 0 in both (G16).  Small integers are exact in fp16 up to 2048 = EMC_MAX_COUNT
-// (bf16: 256); the largest unmasked count is recorded for emc_check().
+// Masked pixels become 0 in both (G16).  Small integers are exact in fp16 up to 2048 = EMC_MAX_COUNT; an unmasked
+// count above that is recorded in the workspace header: emc_check() reports it and the call's results are
+// overwritten with NaN (poison_kernel) so that they cannot be consumed unnoticed.
 #include "emc_internal.cuh"
 
 namespace emc {
@@ -15,7 +15,7 @@ constexpr int kTile = 64;
 template <class T>
 __global__ void __launch_bounds__(256)
 pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *__restrict__ mask,
-            __half *__restrict__ Kc, int ld_p, void *__restrict__ KT, int kt_bf16, int ld_n,
+            __half *__restrict__ Kc, int ld_p, __half *__restrict__ KT, int ld_n,
             WsHeader *__restrict__ hdr) {
     __shared__ float tile[kTile][kTile + 1];
     const int p0 = blockIdx.x * kTile, d0 = blockIdx.y * kTile;
@@ -44,14 +44,13 @@ pack_kernel(const T *__restrict__ counts, int n_pat, int n_pix, const uint8_t *_
             const int p = p0 + j, d = d0 + tx;
             if (p < n_pix && d < n_pat) {
                 const size_t o = (size_t)p * ld_n + d;
-                if (kt_bf16) ((__nv_bfloat16 *)KT)[o] = __float2bfloat16_rn(tile[tx][j]);
-                else ((__half *)KT)[o] = __float2half_rn(tile[tx][j]);
+                KT[o] = __float2half_rn(tile[tx][j]);
             }
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
-    if ((threadIdx.x & 31) == 0 && vmax > (kt_bf16 ? 256 : EMC_MAX_COUNT)) atomicMax(&hdr->max_count, vmax);
+    if ((threadIdx.x & 31) == 0 && vmax > EMC_MAX_COUNT) atomicMax(&hdr->max_count, vmax);
 }
 
 // uint16 counts with an even number of pixels (the configs' case): the same 64 x 64 tile, but every global access is
@@ -127,7 +126,23 @@ rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, floa
     }
 }
 
+// out[i] = NaN for every i if a count was out of range (grid-stride; a no-op launch otherwise)
+__global__ void __launch_bounds__(256)
+poison_kernel(const WsHeader *__restrict__ hdr, float *__restrict__ out, size_t n, double *__restrict__ out64, int n64) {
+    if (hdr->max_count == 0) return;
+    const float nan = __int_as_float(0x7fc00000);
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) out[i] = nan;
+    if (blockIdx.x == 0 && (int)threadIdx.x < n64) out64[threadIdx.x] = (double)nan;
+}
+
 }  // namespace
+
+emc_status launch_poison(const WsHeader *hdr, float *out, size_t n, double *out64, int n64, cudaStream_t st) {
+    if (n64 > 256) return EMC_ERR_UNSUPPORTED;
+    poison_kernel<<<148, 256, 0, st>>>(hdr, out, out ? n : 0, out64, out64 ? n64 : 0);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
 
 emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float inv2s2, float *g_col, float *ia_col,
                         cudaStream_t st) {
@@ -137,27 +152,22 @@ emc_status launch_rowsq(const __half *Kc, int n_pat, int n_pix, int ld_p, float 
 }
 
 emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n_pix,
-                       const uint8_t *mask, __half *Kc, int ld_p, void *KT, bool kt_bf16, int ld_n,
+                       const uint8_t *mask, __half *Kc, int ld_p, __half *KT, int ld_n,
                        WsHeader *hdr, cudaStream_t st) {
-    const int fb = kt_bf16 ? 1 : 0;
     dim3 grid(ceil_div(n_pix, kTile), ceil_div(n_pat, kTile));
     switch (type) {
         case EMC_I32:
-            pack_kernel<int32_t><<<grid, 256, 0, st>>>((const int32_t *)counts, n_pat, n_pix, mask, Kc,
-                                                       ld_p, KT, fb, ld_n, hdr);
+            pack_kernel<int32_t><<<grid, 256, 0, st>>>((const int32_t *)counts, n_pat, n_pix, mask, Kc, ld_p, KT, ld_n, hdr);
             break;
         case EMC_U16:
-            if (!kt_bf16 && (n_pix & 1) == 0 && (((uintptr_t)counts) & 3) == 0) {
-                pack_u16x2_kernel<<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc, ld_p, (__half *)KT,
-                                                        ld_n, hdr);
+            if ((n_pix & 1) == 0 && (((uintptr_t)counts) & 3) == 0) {
+                pack_u16x2_kernel<<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc, ld_p, KT, ld_n, hdr);
                 break;
             }
-            pack_kernel<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc,
-                                                        ld_p, KT, fb, ld_n, hdr);
+            pack_kernel<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)counts, n_pat, n_pix, mask, Kc, ld_p, KT, ld_n, hdr);
             break;
         case EMC_U8:
-            pack_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)counts, n_pat, n_pix, mask, Kc,
-                                                       ld_p, KT, fb, ld_n, hdr);
+            pack_kernel<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)counts, n_pat, n_pix, mask, Kc, ld_p, KT, ld_n, hdr);
             break;
         default:
             return EMC_ERR_ARG;

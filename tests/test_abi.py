@@ -23,7 +23,7 @@ def test_header_symbols_all_exported():
 
 def test_header_constants_match_binding():
     header = (ROOT / "include" / "emc.h").read_text()
-    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_UPDATE_BF16X3", "EMC_DEBUG_SIMT", "EMC_GEMM_1CTA",
+    for name in ("EMC_COMPRESS_WEIGHTED", "EMC_ACCUMULATE", "EMC_UPDATE_RAW", "EMC_MAX_SPANS", "EMC_DEBUG_SIMT", "EMC_GEMM_1CTA",
                  "EMC_PATTERNS_ON_HOST", "EMC_PROFILE_STAGES", "EMC_MAX_COUNT"):
         m = re.search(rf"#define {name}\s+(0x[0-9a-fA-F]+|\d+)u?", header)
         assert m, name
@@ -36,6 +36,9 @@ def test_header_constants_match_binding():
 def test_version_and_strerror():
     lib = emc.load()
     assert b"sm_100a" in lib.emc_version()
+    header = (ROOT / "include" / "emc.h").read_text()
+    tiny = float(re.search(r"#define EMC_P_MIN\s+([0-9.e+-]+)f", header).group(1))
+    assert tiny == 2.0 ** -126                      # float32's smallest normal number (G20)
     assert lib.emc_strerror(0) == b"ok"
     assert b"workspace" in lib.emc_strerror(emc.EMC_ERR_WORKSPACE)
 
@@ -62,7 +65,13 @@ def test_null_arguments_are_rejected_synchronously():
     m = binding._Model(16, 8)
     rot = binding._Rotations(4, 8, None)
     # model_out aliasing the model is an argument error
-    assert lib.emc_iterate(m, det, rot, pat, 1, 0, 8, None, 64, 8, 0, 256, 1 << 30, None) == emc.EMC_ERR_ARG
+    assert lib.emc_iterate(m, det, rot, pat, 1, 0, 8, None, 64, 8, 0, 256, 1 << 30, None, None) == emc.EMC_ERR_ARG
+    # host-resident patterns and per-stage timing need the caller's context
+    for flag in (emc.EMC_PATTERNS_ON_HOST, emc.EMC_PROFILE_STAGES):
+        assert lib.emc_iterate(m, det, rot, pat, 1, 0, 16, None, 64, 8, flag, 256, 1 << 30, None, None) == emc.EMC_ERR_ARG
+    assert lib.emc_context_create(None) == emc.EMC_ERR_ARG
+    assert lib.emc_context_destroy(None) == emc.EMC_OK
+    assert lib.emc_profile_read(None, None, None) == emc.EMC_ERR_ARG
 
 
 def test_binding_refuses_cpu_tensors():

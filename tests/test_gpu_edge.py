@@ -23,19 +23,22 @@ def host(t):
     return t.detach().cpu().numpy()
 
 
-def run_both(model, q, mask, quat, weight, counts, weighted=False):
+def run_both(model, q, mask, quat, weight, counts, weighted=False, null_weight=False):
     ref = o.iterate(model, q, mask, quat, weight, counts, weighted=weighted)
-    _, ref["A"] = o.loglik(ref["W"], ref["idx"], counts, mask)
-    out = emc.emc_iterate(dev(model), dev(q), dev(mask), dev(quat), dev(weight), dev(counts), want_p=True,
-                          flags=emc.EMC_COMPRESS_WEIGHTED if weighted else 0)
+    d = [dev(model), dev(q), dev(mask), dev(quat), None if null_weight else dev(weight), dev(counts)]
+    out = emc.emc_iterate(*d, want_p=True, flags=emc.EMC_COMPRESS_WEIGHTED if weighted else 0)
     emc.emc_check(out["ws"])
+    # the float32 L the GPU path forms (stage API: the same kernels as inside emc_iterate), for the measured P bound
+    w, idx = emc.emc_expand(d[0], d[1], d[3])
+    out["L"] = host(emc.emc_loglik(w, idx, d[1], d[2], d[5]))
     return ref, out
 
 
 def check(ref, out):
     p = host(out["P"])
-    # end to end: |dP| <= 1e-6 + 2 P max_r |dL| with |dL| <= 2e-5 A (T2)
-    bound = 1e-6 + 2.0 * ref["P"] * (2e-5 * ref["A"].max(axis=0))[None, :]
+    # end to end: |dP| <= 1e-6 + P (exp(2 max_r |dL|) - 1) with the MEASURED dL (T2)
+    m = np.abs(out["L"].astype(np.float64) - ref["L"].astype(np.float64)).max(axis=0)
+    bound = 1e-6 + ref["P"] * np.expm1(2.0 * m)[None, :]
     assert np.all(np.abs(p - ref["P"]) <= bound), f"max dP {np.abs(p - ref['P']).max():.3e}"
     assert abs(float(host(out["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"]) + 1e-6
     m, m_ref = host(out["model"]).reshape(-1), ref["model"].reshape(-1)
@@ -98,4 +101,34 @@ def test_extreme_prior_weights(t0):
     w[11] = 1.0
     w /= w.sum()
     ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], w, t0.counts)
+    check(ref, out)
+
+
+def test_zero_prior_weights(t0):
+    """w_r = 0 (log w = -inf) excludes a rotation: P[r,:] = 0 exactly, s[r] = 0, the slice is skipped.  The first
+    row of the list, of a 32-row block and of a warp's row range are among them (the stage API's column sweep and the
+    GEMM epilogue's fused statistics both start from such a row)."""
+    w = np.array(t0.weight[0], dtype=np.float32)
+    dead = [0, 1, 8, 31, 32, 33, 59]
+    w[dead] = 0.0
+    w /= w.sum()
+    with np.errstate(divide="ignore"):
+        ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], w, t0.counts)
+    assert np.all(host(out["P"])[dead] == 0) and np.all(ref["P"][dead] == 0)
+    check(ref, out)
+    # stage API
+    big_l = torch.zeros((len(w), emc.ld_for(t0.counts.shape[0])), dtype=torch.float32, device="cuda")
+    big_l[:, : t0.counts.shape[0]] = dev(ref["L"])
+    p, s, ll = emc.emc_normalize(big_l[:, : t0.counts.shape[0]], dev(t0.quat[0]), dev(w))
+    with np.errstate(divide="ignore"):
+        p_ref, s_ref, ll_ref = o.normalize(ref["L"], w)
+    assert np.abs(host(p) - p_ref).max() <= 1e-6 and np.all(host(p)[dead] == 0)
+    assert abs(float(host(ll)[0]) - ll_ref) <= 1e-6 * abs(ll_ref)
+
+
+def test_null_weights_are_the_uniform_prior(t0):
+    """weight = NULL is 1/R: the uniform branches of the fused statistics and of the second sweep against the oracle"""
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], t0.weight[0], t0.counts, null_weight=True)
+    check(ref, out)
+    ref, out = run_both(t0.model_init, t0.q, t0.mask, t0.quat[0], t0.weight[0], t0.counts, weighted=True, null_weight=True)
     check(ref, out)

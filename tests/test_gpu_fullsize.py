@@ -66,12 +66,23 @@ def test_c2_stagewise_and_end_to_end(c2):
     assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12), \
         f"max rel {np.max(np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-12)):.3e}"
 
-    # whole iteration, as bench.py launches it
+    # whole iteration, as bench.py launches it; P against the bound from the log-likelihood difference MEASURED here
+    # (the GPU's own Expand -> log-likelihood through the stage API: the kernels emc_iterate runs)
+    w, idx = emc.emc_expand(dev(inp.model_init), d_q, d_quat)
+    l_gpu = host(emc.emc_loglik(w, idx, d_q, d_mask, d_k))
+    del w, idx
+    m = np.abs(l_gpu.astype(np.float64) - ref["L"].astype(np.float64)).max(axis=0)
+    bound = 1e-6 + ref["P"] * np.expm1(2.0 * m)[None, :]
+    del l_gpu
     out = emc.emc_iterate(dev(inp.model_init), d_q, d_mask, d_quat, d_w, d_k, want_p=True)
     emc.emc_check(out["ws"])
-    bound = 1e-6 + 2.0 * ref["P"] * (2e-5 * big_a.max(axis=0))[None, :]
     pg = host(out["P"])
     assert np.all(np.abs(pg - ref["P"]) <= bound), f"max dP {np.abs(pg - ref['P']).max():.3e}"
+    # weight = NULL (the uniform branches, what the header documents as the default) gives the same responsibilities
+    out0 = emc.emc_iterate(dev(inp.model_init), d_q, d_mask, d_quat, None, d_k, want_p=True)
+    assert np.all(np.abs(host(out0["P"]) - ref["P"]) <= bound)
+    assert abs(float(host(out0["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"])
+    del out0
     assert abs(float(host(out["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"])
     mg = host(out["model"]).reshape(-1)
     cov = ref["den"] >= 1e-3 * ref["den"].max()

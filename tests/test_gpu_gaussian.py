@@ -20,9 +20,11 @@ def dev(x):
     return torch.from_numpy(np.ascontiguousarray(x)).cuda()
 
 
-@pytest.mark.parametrize("name,sigma", [("T1", 20.0), ("T1", 5.0), ("T2", 10.0), ("C1", 30.0)])
+@pytest.mark.parametrize("name,sigma", [("T1", 20.0), ("T1", 5.0), ("T2", 10.0), ("C1", 30.0), ("T1null", 20.0)])
 @pytest.mark.parametrize("weighted", [True, False], ids=["eq2.12", "eq2.10"])
 def test_iterate_gaussian_matches_oracle(inputs_cache, name, sigma, weighted):
+    null_weight = name.endswith("null")                      # weight = NULL: log(1/R) handed to both kernels by the host
+    name = name.replace("null", "")
     inp = inputs_cache(name)
     stage = len(inp.quat) - 1
     quat, weight = inp.quat[stage], inp.weight[stage]
@@ -32,8 +34,8 @@ def test_iterate_gaussian_matches_oracle(inputs_cache, name, sigma, weighted):
         weight /= weight.sum()
     ref = o.iterate_gaussian(inp.model_init, inp.q, inp.mask, quat, weight, inp.counts, sigma, weighted=weighted)
     flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
-    out = emc.emc_iterate_gaussian(dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(quat), dev(weight),
-                                   dev(inp.counts), sigma, flags=flags, want_p=True)
+    out = emc.emc_iterate_gaussian(dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(quat),
+                                   None if null_weight else dev(weight), dev(inp.counts), sigma, flags=flags, want_p=True)
     emc.emc_check(out["ws"])
     p = out["P"].cpu().numpy()
     dq = 1e-5 * ref["A"].max(axis=0)                         # per column

@@ -1,9 +1,10 @@
-"""Parity at the geometry of BASELINE.json's large configs (C3: 128^3 / 128x128 / R = 25 000;
-C5 last stage: 256^3 / 256x256 / R = 50 000) on SAMPLED outputs the oracle computes one by one.
-Model, detector, mask and rotation list are the configs' own; only the pattern count is cut
-(make_inputs(..., n_pat=...)) so that the seeded generator finishes in seconds.  What these sizes
-exercise beyond C2: linear indices past 2^31 (R x P = 3.3e9), accumulators that do not fit L2,
-hundreds of K chunks, ragged last pair tiles.  (`-m gpu`)"""
+"""Parity at BASELINE.json's large configs on SAMPLED outputs the oracle computes one by one (`-m gpu`):
+  C3  128^3 / 128x128 / R = 25 000 / N = 50 000: the FULL config, as bench.py times it by default;
+  C4  128^3 / 128x128 / R = 10 000, pattern chunks of 25 000 streamed from pinned host memory: the config's own chunk
+      size and route, N cut to 2 chunks + a ragged third (60 000 of 200 000 patterns);
+  C5  last stage, 256^3 / 256x256 / R = 50 000: the pattern count is cut to 1024 (EMC_TEST_LARGE=1: the full 20 000).
+Model, detector, mask and rotation list are the configs' own.  What these sizes exercise beyond C2: linear indices
+past 2^31 (R x P = 3.3e9), accumulators that do not fit L2, hundreds of K chunks, ragged last pair tiles."""
 import os
 
 import numpy as np
@@ -107,8 +108,80 @@ def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
     assert np.all(m[den_ref == 0] == 0)
 
 
-def test_c3_geometry_sampled(inputs_cache):
-    run_case(inputs_cache, "C3", n_pat=50000 if FULL else 4096, stage=0, n_rows=24, n_cols=48, n_compress=1500)
+def test_c3_full_config_sampled(inputs_cache):
+    run_case(inputs_cache, "C3", n_pat=50000, stage=0, n_rows=24, n_cols=48, n_compress=1500)
+
+
+def test_c4_route_pattern_chunks_from_host(inputs_cache):
+    """Config 4's route at its own geometry and chunk size.  emc_iterate (chunks of 25 000 streamed from pinned host
+    memory, numerators added up by TMA reduce-add, rows divided after the last chunk) is compared with the same
+    iteration assembled from the stage calls chunk by chunk, and every stage of that chain is checked against the
+    oracle on sampled rows / columns as in run_case (the oracle cannot form 10 000 x 60 000 x 15 808 in float64 in the
+    time a test has)."""
+    n_pat, chunk = 60000, 25000
+    inp = inputs_cache("C4", n_pat=n_pat)
+    cfg = inp.cfg
+    quat, weight = inp.quat[0], inp.weight[0]
+    n_rot, n_pix = quat.shape[0], cfg.n_pix
+    d_model, d_q, d_mask, d_quat, d_w = dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(quat), dev(weight)
+    pinned = torch.from_numpy(inp.counts).pin_memory()
+    out = emc.emc_iterate(d_model, d_q, d_mask, d_quat, d_w, pinned, n_pat_chunk=chunk, flags=emc.EMC_PATTERNS_ON_HOST)
+    emc.emc_check(out["ws"])
+    model_a, ll_a = host(out["model"]).reshape(-1), float(host(out["loglik"])[0])
+    del out
+    torch.cuda.empty_cache()
+
+    rows = sampled_rows(n_rot, 16, 11)
+    t_rows = torch.from_numpy(rows).cuda()
+    w, idx = emc.emc_expand(d_model, d_q, d_quat)
+    w_ref, idx_ref = o.expand(inp.model_init, inp.q, quat[rows])
+    assert np.array_equal(host(idx[t_rows]), idx_ref)
+    ws = emc.make_workspace(cfg.n, n_pix, n_rot, chunk)
+    s = torch.zeros(n_rot, dtype=torch.float32, device="cuda")
+    ll = torch.zeros(1, dtype=torch.float64, device="cuda")
+    wnum = torch.zeros((n_rot, n_pix), dtype=torch.float32, device="cuda")
+    p_rows = np.zeros((len(rows), n_pat), np.float32)
+    rng = np.random.default_rng(12)
+    for d0 in range(0, n_pat, chunk):
+        d1 = min(n_pat, d0 + chunk)
+        d_k = dev(inp.counts[d0:d1])
+        big_l = emc.emc_loglik(w, idx, d_q, d_mask, d_k, ws=ws)
+        l_ref, a_ref = o.loglik(host(w[t_rows]), idx_ref, inp.counts[d0:d1], inp.mask)
+        assert (np.abs(host(big_l[t_rows]) - l_ref) / a_ref).max() <= 1e-5
+        p, s, ll = emc.emc_normalize(big_l, d_quat, d_w, flags=emc.EMC_ACCUMULATE, s=s, loglik=ll, ws=ws)
+        cols = np.unique(np.concatenate([rng.integers(0, d1 - d0, size=24), [0, d1 - d0 - 1]]))
+        t_cols = torch.from_numpy(cols).cuda()
+        p_ref, _, _ = o.normalize(host(big_l[:, t_cols]), weight)
+        assert np.abs(host(p[:, t_cols]) - p_ref).max() <= 1e-6
+        p_rows[:, d0:d1] = host(p[t_rows])
+        emc.emc_update(p, None, d_q, d_mask, d_k, flags=emc.EMC_ACCUMULATE, wnew=wnum, ws=ws)
+        del big_l, p, d_k
+    # numerators over all chunks on sampled rows, then eq. (2.5)'s division (G9: after the last chunk)
+    wn_ref, s_ref = o.update(p_rows, inp.counts, inp.mask)
+    s_rows = host(s[t_rows]).astype(np.float64)
+    assert np.abs(s_rows - s_ref).max() <= 1e-5 * max(1.0, s_ref.max())
+    keep = s_ref > 1e-20
+    got = host(wnum[t_rows]).astype(np.float64)[keep] / s_rows[keep, None]
+    scale = np.abs(wn_ref[keep]).max()
+    assert (np.abs(got - wn_ref[keep]) / (np.abs(wn_ref[keep]) + 1e-7 * scale)).max() <= 2e-5
+    wn = wnum / torch.where(s > 0, s, torch.ones_like(s))[:, None]
+    wn[s <= 0] = 0
+    m_b, _ = emc.emc_compress(wn, s, d_q, d_mask, d_quat, cfg.n, ws=ws)
+    model_b, ll_b = host(m_b).reshape(-1), float(host(ll)[0])
+    # the two routes: same arithmetic up to the order of float32 sums
+    assert abs(ll_a - ll_b) <= 1e-6 * abs(ll_b)
+    big = np.abs(model_b) >= 1e-6 * np.abs(model_b).max()
+    rel = np.abs(model_a - model_b)[big] / np.abs(model_b)[big]
+    assert np.array_equal(model_a == 0, model_b == 0)
+    assert np.median(rel) <= 1e-5 and rel.max() <= 1e-2, (np.median(rel), rel.max())
+    # Compress against the oracle on the first 1000 rotations of that W'
+    sub = slice(0, 1000)
+    sw = (host(s[sub]) > 0).astype(np.float32)
+    m, den = emc.emc_compress(wn[sub].contiguous(), dev(sw), d_q, d_mask, d_quat[sub].contiguous(), cfg.n, want_den=True, ws=ws)
+    m_ref, _, den_ref = o.compress(host(wn[sub]), inp.q, quat[sub], inp.mask, cfg.n, slice_w=sw)
+    m, m_ref = host(m).reshape(-1), m_ref.reshape(-1)
+    cov = den_ref >= 1e-6 * den_ref.max()
+    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12)
 
 
 def test_c5_last_stage_geometry_sampled(inputs_cache):

@@ -429,10 +429,22 @@ def test_masked_counts_never_matter():
     assert np.array_equal(a["model"], b["model"]) and np.array_equal(a["P"], b["P"])
 
 
-def test_normalize_flushes_below_p_min():
-    """G20: responsibilities below 2^-100 are stored as 0; a row made only of such values has s = 0."""
-    big_l = np.array([[0.0, 0.0], [-60.0, -80.0], [-69.0, -70.0]], np.float32)    # e^-69 > 2^-100 > e^-70
+def test_normalize_is_flush_to_zero_float32():
+    """G20: P is a float32 quantity stored flush-to-zero: what float32 holds as a normal number (>= 2^-126) is kept
+    with full precision, what would be a float32 subnormal is 0; a row made only of such values has s = 0.
+    Pinned against numpy's own float32: the kept set is exactly {p : float32(p) is a normal number}."""
+    assert o.P_MIN == 2.0 ** -126 == float(np.finfo(np.float32).tiny)
+    # ln 2^-126 = -87.34: e^-87 is a normal float32, e^-88 and e^-100 are subnormal, e^-104 underflows float32 altogether
+    big_l = np.array([[0.0, 0.0, 0.0], [-60.0, -88.0, -104.0], [-87.0, -100.0, -86.0]], np.float32)
     p, s, _ = o.normalize(big_l, np.full(3, 1 / 3, np.float32))
-    assert p[2, 0] > 0 and p[2, 1] == 0 and p[1, 1] == 0 and p[1, 0] > 0
-    assert abs(p[:, 0].sum() - 1) < 1e-12 and s[2] == p[2, 0]
-    assert o.P_MIN == 2.0 ** -100
+    exact = np.exp(big_l.astype(np.float64)) / np.exp(big_l.astype(np.float64)).sum(axis=0)
+    p32 = exact.astype(np.float32)
+    normal = p32 >= np.finfo(np.float32).tiny
+    assert np.array_equal(p > 0, normal)
+    assert np.allclose(p[normal], exact[normal], rtol=1e-14)
+    assert p[1, 1] == 0 and p[1, 2] == 0 and p[2, 1] == 0 and p[2, 0] > 0 and p[2, 2] > 0
+    assert abs(p[:, 0].sum() - 1) < 1e-12 and s[1] == p[1, 0]
+    # a row entirely below the threshold drops out: s = 0
+    big_l = np.array([[0.0, 0.0], [-95.0, -99.0]], np.float32)
+    p, s, _ = o.normalize(big_l, np.full(2, 0.5, np.float32))
+    assert s[1] == 0 and np.all(p[0] == 1.0)
