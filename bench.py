@@ -323,7 +323,8 @@ def main():
     warmup = max(args.warmup, 3)
 
     dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
-    d_model0, d_q, d_mask, d_counts = dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.counts)
+    q2d = inp.q.reshape(cfg.n_det, cfg.n_det, 3)           # row-major 2-D detector: emc_detector.row_len = n_det
+    d_model0, d_q, d_mask, d_counts = dev(inp.model_init), dev(q2d), dev(inp.mask), dev(inp.counts)
     # consecutive iterations on the same rotation list go into one emc_iterate call
     plan = []
     for s in range(cfg.n_iter):
@@ -396,7 +397,7 @@ def main():
     # ---- end to end through the C ABI with HOST buffers
     h_counts = torch.from_numpy(inp.counts).pin_memory()
     h_model = torch.from_numpy(inp.model_init).pin_memory()
-    h_q, h_mask = torch.from_numpy(inp.q).pin_memory(), torch.from_numpy(inp.mask).pin_memory()
+    h_q, h_mask = torch.from_numpy(q2d).pin_memory(), torch.from_numpy(inp.mask).pin_memory()
     h_rot = [(torch.from_numpy(np.ascontiguousarray(q)).pin_memory(), torch.from_numpy(w).pin_memory())
              for _, _, _, q, w in plan]
     h_out = torch.empty_like(h_model).pin_memory()

@@ -93,6 +93,9 @@ typedef struct {
     int n_pix;           /* P */
     const float *q;      /* [P][3] (x,y,z) in voxel units relative to the origin c */
     const uint8_t *mask; /* [P], 1 = use, 0 = missing/saturated; NULL = use all */
+    int row_len;         /* pixels per detector row when the P pixels are a row-major 2-D array (n_pix % row_len == 0),
+                            0 = no 2-D structure known.  A locality hint only: Expand and Compress then give each warp a
+                            4 x 8 tile of pixels instead of 32 consecutive ones; results do not depend on it. */
 } emc_detector;
 
 /* The discretised rotation space (R_j) with prior weights w_j. */
@@ -120,6 +123,9 @@ EMC_API emc_status emc_context_destroy(emc_context *ctx);
 /* Bytes of workspace sufficient for any call below at these sizes.  n_pat_chunk = patterns
  * resident per chunk (= N when not chunked).  Returns 0 on invalid sizes. */
 EMC_API size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags);
+/* Bytes sufficient for emc_expand and emc_compress alone (the stage calls that touch no patterns): the corner blocks
+ * of the model or of the accumulators plus the packed geometry.  Returns 0 on invalid sizes. */
+EMC_API size_t emc_workspace_bytes_geometry(int n, int n_pix, int n_rot);
 
 /* Stage 1, Expand (e-step), eq. (2.9), PAPER.md:113-116:
  *   W[r,p] = sum_l f(p_l - R_r q_p) model[l],  f = trilinear weights of the 8 voxels around
@@ -129,8 +135,8 @@ EMC_API size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk,
  *   idx [R][P] int32, out, or NULL: linear index (b_x*n + b_y)*n + b_z of the base corner
  *       b = floor(x), or -1 outside the grid.  The coordinate arithmetic is pinned (DESIGN.md §3
  *       G4) so this map is bit-exact against the oracle.
- *   ws  workspace or NULL.  With a workspace (n even) the model is first re-laid as blocked
- *       staggered copies so that a sample is two 16-byte loads; without, plain gathers. */
+ *   ws  workspace or NULL.  With a workspace the model is first re-laid as one 32-byte block of the 8 corner
+ *       values per base corner, so that a sample is one 32-byte load; without, plain gathers. */
 EMC_API emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                       float *W, int32_t *idx, void *ws, size_t ws_bytes, void *stream);
 

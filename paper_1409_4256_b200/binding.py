@@ -29,7 +29,7 @@ EMC_MAX_SPANS = 4096
 STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
-SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_expand", "emc_loglik",
+SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
            "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_gaussian", "emc_refine", "emc_check",
            "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
@@ -49,7 +49,7 @@ class _Model(Structure):
 
 
 class _Detector(Structure):
-    _fields_ = [("n_pix", c_int), ("q", c_void_p), ("mask", c_void_p)]
+    _fields_ = [("n_pix", c_int), ("q", c_void_p), ("mask", c_void_p), ("row_len", c_int)]
 
 
 class _Rotations(Structure):
@@ -79,6 +79,8 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_context_destroy.argtypes = [vp]
     lib.emc_workspace_bytes.restype = sz
     lib.emc_workspace_bytes.argtypes = [ci, ci, ci, ci, cu]
+    lib.emc_workspace_bytes_geometry.restype = sz
+    lib.emc_workspace_bytes_geometry.argtypes = [ci, ci, ci]
     lib.emc_expand.restype = ci
     lib.emc_expand.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), vp, vp, vp, sz, vp]
     lib.emc_loglik.restype = ci
@@ -142,10 +144,12 @@ def ld_for(n_pat: int) -> int:
 
 
 def _detector(q, mask):
-    n_pix = q.shape[0]
-    if mask is not None and mask.shape[0] != n_pix:
+    """q is [P, 3], or [rows, row_len, 3] for a row-major 2-D detector (emc_detector.row_len, a locality hint)."""
+    row_len = q.shape[1] if q.dim() == 3 else 0
+    n_pix = q.numel() // 3
+    if mask is not None and mask.numel() != n_pix:
         raise ValueError("mask length != number of pixels")
-    return _Detector(n_pix, _dev(q, torch.float32, "q"), _opt(mask, torch.uint8, "mask"))
+    return _Detector(n_pix, _dev(q, torch.float32, "q"), _opt(mask, torch.uint8, "mask"), row_len)
 
 
 def _rotations(quat, weight):
@@ -173,6 +177,14 @@ def make_workspace(n, n_pix, n_rot, n_pat_chunk, flags=0, device="cuda") -> torc
     nbytes = emc_workspace_bytes(n, n_pix, n_rot, n_pat_chunk, flags)
     if nbytes == 0:
         raise EmcError(EMC_ERR_UNSUPPORTED, "emc_workspace_bytes")
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def make_geometry_workspace(n, n_pix, n_rot, device="cuda") -> torch.Tensor:
+    """Workspace for emc_expand / emc_compress alone (emc_workspace_bytes_geometry)."""
+    nbytes = load().emc_workspace_bytes_geometry(n, n_pix, n_rot)
+    if nbytes == 0:
+        raise EmcError(EMC_ERR_UNSUPPORTED, "emc_workspace_bytes_geometry")
     return torch.empty(nbytes, dtype=torch.uint8, device=device)
 
 
@@ -233,7 +245,7 @@ def emc_expand(model, q, quat, want_idx=True, use_ws=True):
     rot = _rotations(quat, None)
     w = torch.empty((rot.n_rot, det.n_pix), dtype=torch.float32, device=model.device)
     idx = torch.empty((rot.n_rot, det.n_pix), dtype=torch.int32, device=model.device) if want_idx else None
-    ws = make_workspace(n, det.n_pix, 1, 1) if use_ws else None      # the blocked model copies do not scale with R
+    ws = make_geometry_workspace(n, det.n_pix, rot.n_rot) if use_ws else None
     _check(load().emc_expand(m, det, rot, w.data_ptr(), idx.data_ptr() if want_idx else None,
                              ws.data_ptr() if use_ws else None, ws.numel() if use_ws else 0, _stream()), "emc_expand")
     return w, idx
@@ -298,7 +310,9 @@ def emc_compress(wnew, slice_w, q, mask, quat, n, flags=0, want_den=False, ws=No
     rot = _rotations(quat, None)
     model = torch.empty((n, n, n), dtype=torch.float32, device=wnew.device)
     den = torch.empty(n * n * n, dtype=torch.float32, device=wnew.device) if want_den else None
-    ws, wp, wb = _ws(ws, n, n_pix, 1, 1)                              # the accumulators do not scale with R
+    if ws is None:
+        ws = make_geometry_workspace(n, n_pix, n_rot)
+    wp, wb = ws.data_ptr(), ws.numel()
     _check(load().emc_compress(_dev(wnew, torch.float32, "Wnew"), _opt(slice_w, torch.float32, "slice_w"), det, rot,
                                n, model.data_ptr(), den.data_ptr() if want_den else None, flags, wp, wb, _stream()),
            "emc_compress")
@@ -390,4 +404,4 @@ def emc_version() -> str:
 
 
 __all__ = sorted(n for n in dir() if n.startswith(("emc_", "EMC_", "Emc"))) + [
-    "STAGES", "SYMBOLS", "ld_for", "load", "make_workspace", "default_context"]
+    "STAGES", "SYMBOLS", "ld_for", "load", "make_workspace", "make_geometry_workspace", "default_context"]

@@ -69,8 +69,9 @@ struct Layout {
     float *pscale;            // [ld_n/512][R] inverse chunk scales of planesP
     float *s;                 // [R]
     float *Wnum;              // [R][P]        update numerators -> W'
-    float2 *acc;              // [8 G]         8 staggered grids of 64-byte (num, den) corner blocks
-    float *blocked;           // [8 G]         blocked staggered model copies (Expand)
+    float2 *acc;              // [8 G]         one 64-byte (num, den) corner block per base corner (Compress)
+    float *blocked;           // [8 G]         one 32-byte corner block of the model per base corner (Expand)
+    float4 *geom;             // [P + 3 R]     packed pixel geometry and rotation matrices (launch_geometry)
     float *scratch;           // normalise partials
     float *Asq;               // [2][ld_n]     1 / (2 sigma^2 A_d) and 1 / A_d, A_d = sum_p K^2 (Gaussian model)
     uint32_t *active;         // [R/32 + 1]    slices den was accumulated for (+ the device flag), Compress
@@ -95,8 +96,9 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.pscale = a.take<float>((size_t)ceil_div(l.ld_n, 512) * R);
     l.s = a.take<float>(R);
     l.Wnum = a.take<float>(R * n_pix);
-    l.acc = a.take<float2>(compress_scratch_float2(n, n_pix));
-    l.blocked = a.take<float>(n >= 2 ? expand_scratch_floats(n, n_pix) : 0);
+    l.acc = a.take<float2>(compress_scratch_float2(n));
+    l.blocked = a.take<float>(expand_scratch_floats(n, n_pix, n_rot));
+    l.geom = a.take<float4>(geometry_float4(n_pix, n_rot));
     l.scratch = a.take<float>(normalize_scratch_floats(n_rot, l.ld_n));
     l.Asq = a.take<float>((size_t)2 * l.ld_n);
     l.active = a.take<uint32_t>((size_t)ceil_div(n_rot, 32) + 1);
@@ -115,7 +117,9 @@ emc_status check_ws(void *ws, size_t ws_bytes, size_t need) {
     return EMC_OK;
 }
 
-bool det_ok(const emc_detector *d) { return d && d->n_pix > 0 && d->q; }
+bool det_ok(const emc_detector *d) {
+    return d && d->n_pix > 0 && d->q && d->row_len >= 0 && (d->row_len == 0 || d->n_pix % d->row_len == 0);
+}
 bool rot_ok(const emc_rotations *r) { return r && r->n_rot > 0 && r->quat; }
 bool pat_ok(const emc_patterns *p) {
     return p && p->n_pat > 0 && p->counts && (p->type == EMC_I32 || p->type == EMC_U16 || p->type == EMC_U8);
@@ -218,17 +222,29 @@ size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigne
     return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage).total;
 }
 
+size_t emc_workspace_bytes_geometry(int n, int n_pix, int n_rot) {
+    if (!sizes_ok(n, n_pix, n_rot, 1)) return 0;
+    size_t blocks = round_up(sizeof(float2) * compress_scratch_float2(n), 1024);
+    const size_t eb = round_up(sizeof(float) * expand_scratch_floats(n, n_pix, n_rot), 1024);
+    if (eb > blocks) blocks = eb;
+    return blocks + round_up(sizeof(float4) * geometry_float4(n_pix, n_rot), 1024);
+}
+
 emc_status emc_expand(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                       float *W, int32_t *idx, void *ws, size_t ws_bytes, void *stream) {
     if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || (!W && !idx)) return EMC_ERR_ARG;
     if (!sizes_ok(model->n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
     float *blocked = nullptr;
+    Geometry geo;
     if (ws) {
-        EMC_TRY(check_ws(ws, ws_bytes, round_up(sizeof(float) * expand_scratch_floats(model->n, det->n_pix), 1024)));
+        const size_t b_bytes = round_up(sizeof(float) * expand_scratch_floats(model->n, det->n_pix, rot->n_rot), 1024);
+        EMC_TRY(check_ws(ws, ws_bytes, b_bytes + sizeof(float4) * geometry_float4(det->n_pix, rot->n_rot)));
         blocked = (float *)ws;
+        EMC_TRY(launch_geometry(det->q, det->mask, det->n_pix, det->row_len, rot->quat, rot->n_rot,
+                                (float4 *)((uint8_t *)ws + b_bytes), &geo, (cudaStream_t)stream));
     }
     return launch_expand(model->model, model->n, det->q, det->mask, det->n_pix, rot->quat, rot->n_rot, W, idx,
-                         nullptr, 0, nullptr, blocked, (cudaStream_t)stream);
+                         nullptr, 0, nullptr, blocked, blocked ? &geo : nullptr, (cudaStream_t)stream);
 }
 
 emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *det,
@@ -284,10 +300,13 @@ emc_status emc_compress(const float *Wnew, const float *slice_w, const emc_detec
                         unsigned flags, void *ws, size_t ws_bytes, void *stream) {
     if (!Wnew || !det_ok(det) || !rot_ok(rot) || !model_out) return EMC_ERR_ARG;
     if (!sizes_ok(n, det->n_pix, rot->n_rot, 1)) return EMC_ERR_UNSUPPORTED;
-    const size_t need = round_up(sizeof(float2) * compress_scratch_float2(n, det->n_pix), 1024);
-    EMC_TRY(check_ws(ws, ws_bytes, need));
-    return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, det->q, det->mask, det->n_pix,
-                           rot->quat, rot->n_rot, n, (float2 *)ws, model_out, den_out, (cudaStream_t)stream);
+    const size_t a_bytes = round_up(sizeof(float2) * compress_scratch_float2(n), 1024);
+    EMC_TRY(check_ws(ws, ws_bytes, a_bytes + sizeof(float4) * geometry_float4(det->n_pix, rot->n_rot)));
+    Geometry geo;
+    EMC_TRY(launch_geometry(det->q, det->mask, det->n_pix, det->row_len, rot->quat, rot->n_rot,
+                            (float4 *)((uint8_t *)ws + a_bytes), &geo, (cudaStream_t)stream));
+    return launch_compress(Wnew, slice_w, (flags & EMC_COMPRESS_WEIGHTED) != 0, geo, n, (float2 *)ws, model_out, den_out,
+                           (cudaStream_t)stream);
 }
 
 // Algorithm 1 for both likelihood models; sigma > 0 selects the paper's Gaussian model (section 11 of DESIGN.md)
@@ -353,13 +372,15 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     }
     int job = 0;
     const float *model_cur = model->model;
+    Geometry geo;                                            // once per call: the rotation list is the same in every iteration
+    EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, rot->quat, n_rot, l.geom, &geo, st));
     for (int it = 0; it < n_iter; ++it) {
         // stage 1: Expand, with logW planes and S fused in
         {
             Span sp(ctx, prof, EMC_STAGE_EXPAND, st);
             EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
             EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                                  l.planesL, l.ld_p, l.S, l.blocked, st, gauss));
+                                  l.planesL, l.ld_p, l.S, l.blocked, &geo, st, gauss));
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
@@ -426,8 +447,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         {
             Span sp(ctx, prof, EMC_STAGE_COMPRESS, st);
             const DenCache cache = {l.active, (int *)(l.active + ceil_div(n_rot, 32)), it == 0};
-            EMC_TRY(launch_compress(l.Wnum, l.s, weighted, det->q, det->mask, n_pix, rot->quat, n_rot, n, l.acc,
-                                    model_out, nullptr, st, &cache));
+            EMC_TRY(launch_compress(l.Wnum, l.s, weighted, geo, n, l.acc, model_out, nullptr, st, &cache));
         }
         model_cur = model_out;
     }

@@ -5,20 +5,20 @@
 //
 // with the same trilinear weights f and the same pinned sample geometry as Expand.
 //
-// Measured on B200 (DESIGN.md §7 "Compress"): what bounds the scatter is the chip's rate of fp32 reductions into
-// L2, which depends on how the bytes are grouped: 64 bytes per sample as four unrelated 16-byte reductions cost
-// 347 us per 2e7 samples, as ONE contiguous 64-byte group issued by four adjacent lanes 224 us (and a
-// cp.reduce.async.bulk of the same 64 bytes, or any mix of the two, the same 225 us); shared-memory atomics are
-// slower than all of them.  So the design (a) moves a sample's 8 corners x (num, den) = 64 bytes in four 16-byte
-// red.global.add.v4.f32 (16 bytes per lane is the widest reduction there is), and (b) makes those 64 bytes
-// CONTIGUOUS and lets four adjacent lanes issue them in
-// one instruction: the accumulator is not a voxel grid but 8 staggered grids of 2x2x2 blocks, one per parity
-// (b_x&1, b_y&1, b_z&1) of the base corner; grid c holds, for every base of that parity, one aligned 64-byte
-// block {num, den} x corner (4 dx + 2 dy + dz), blocks ordered [b_x/2][b_y/2][b_z/2].  After computing its
-// own sample a lane hands (block, t_x, t_y, t_z, W') to its group of four by shuffles, and the group adds the
-// four samples' blocks one after the other, each lane carrying the corner pair (dx, dy, dz = 0..1) it owns.
-// The divide kernel gathers a voxel's 8 contributions.  64 G bytes of accumulators (16 MB at 64^3, 134 MB at
-// 128^3); n odd falls back to 8-byte reductions on a plain (num, den) grid.
+// Measured on B200 (DESIGN.md section 7 "Compress"): what bounds the scatter is the chip's rate of fp32 reductions
+// into L2, which depends on how the bytes are grouped: 64 bytes per sample as four unrelated 16-byte reductions cost
+// 347 us per 2e7 samples, as ONE contiguous 64-byte group issued by four adjacent lanes 224 us; shared-memory
+// atomics on fp32 are CAS loops (ATOMS.CAST.SPIN) at 2 cycles per lane and slower than all of them.  So the design
+// (a) moves a sample's 8 corners x (num, den) = 64 bytes in four 16-byte red.global.add.v4.f32 (16 bytes per lane is
+// the widest reduction there is), and (b) makes those 64 bytes CONTIGUOUS and lets four adjacent lanes issue them in
+// one instruction: the accumulator is not a voxel grid but one aligned 64-byte block {num, den} x corner
+// (4 dx + 2 dy + dz) per BASE CORNER, acc[(b_x n + b_y) n + b_z] (the block index is the index map itself).
+// After computing its own sample a lane hands (block, t_x, t_y, t_z, W') to its group of four by shuffles, and the
+// group adds the four samples' blocks one after the other, each lane carrying the corner quad (dx; num or den) it owns.
+// A warp works on a 4 x 8 tile of detector pixels at a time (emc_geometry.cuh TileMap).
+// The divide kernel gathers a voxel's 8 contributions.  64 G bytes of accumulators (16 MB at 64^3, 134 MB at 128^3).
+#include <algorithm>
+
 #include "emc_geometry.cuh"
 #include "emc_internal.cuh"
 
@@ -27,15 +27,10 @@ namespace emc {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kPixPerThread = 4;
-constexpr int kPixPerBlock = kThreads * kPixPerThread;
+constexpr int kWarps = kThreads / 32;
 
-__device__ __forceinline__ void red_add_v2(float2 *addr, float a, float b) {
-    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b) : "memory");
-}
-
-__device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float c, float d) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+__device__ __forceinline__ void red_add_v4(float4 *addr, const float4 v) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
 // Block layout: 16 floats = num of the 8 corners (order 4 dx + 2 dy + dz), then den of the 8 corners; as float4s:
@@ -45,7 +40,7 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
 // slices are skipped (s[r] = 0).  Inside emc_iterate the iterations after the first therefore run NUM_ONLY (32 bytes
 // per sample, two lanes per sample) as long as the set of skipped slices is the one den was accumulated for;
 // active_check_kernel decides that on the device and the scatter kernel branches on its flag, so no host
-// synchronisation is needed (probe: 153 us against 224 us per 2e7 samples).
+// synchronisation is needed.
 
 // One thread per rotation, one warp per word: bits[r / 32] = mask of slices with s[r] > 0; *changed = 1 if it differs
 // from the stored mask (or force), else left as the caller zeroed it.
@@ -68,9 +63,13 @@ compress_clear_kernel(float4 *__restrict__ acc, size_t n_blocks, const int *__re
     if (*changed != 0 || (t & 2) == 0) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
+// Warp-wide: every lane calls it with its own sample (blk < 0: none).
 // FULL: four rounds, the four lanes of a group add the 64-byte block of the sample of lane grp + k.
 // NUM_ONLY: two rounds, lanes 0-1 add the 32 num bytes of the sample of lane grp + 2k, lanes 2-3 of grp + 2k + 1.
-// A lane carries the four corners (dx, dy, dz), dy, dz = 0..1, of num (or den).  Warp-wide: every lane calls it.
+// A lane carries the four corners (dx, dy, dz), dy, dz = 0..1, of num (or den); it gets the sample by shuffles and forms
+// its own four products.  (Measured against parking each lane's 16 products in shared memory and reading them back
+// transposed: 232 us against 240 us per C2 stage; the shared-memory traffic costs more L1 wavefronts than the
+// shuffles, and the multiplier has room: issue slots 36 % busy.)
 template <bool NUM_ONLY>
 __device__ __forceinline__ void scatter_rounds(float4 *__restrict__ acc, int blk, float stx, float sty, float stz, float v,
                                                float om, unsigned lane) {
@@ -92,52 +91,61 @@ __device__ __forceinline__ void scatter_rounds(float4 *__restrict__ acc, int blk
             const float a0 = wx * (1.f - ty), a1 = wx * ty;
             const float z0 = 1.f - tz;
             const float sc = is_den ? 1.f : vv;
-            red_add_v4(acc + 4 * (size_t)b + slot, (a0 * z0) * sc, (a0 * tz) * sc, (a1 * z0) * sc, (a1 * tz) * sc);
+            red_add_v4(acc + 4 * (size_t)b + slot, make_float4((a0 * z0) * sc, (a0 * tz) * sc, (a1 * z0) * sc, (a1 * tz) * sc));
         }
     }
 }
 
-// grid = (R, ceil(P / kPixPerBlock)); n even.  acc = [8][(n/2)^3] blocks of 4 float4.  changed: device flag of
-// active_check_kernel, 0 = den is still valid, add num only; null = add both.
-__global__ void __launch_bounds__(kThreads)
+// One warp per (rotation, band) work item (a stride loop covers item counts beyond the grid limit); it walks along its
+// band kTilesPerStep tiles at a time (emc_geometry.cuh).  acc = [n^3] blocks of 4 float4.  changed: device flag
+// of active_check_kernel, 0 = den is still valid, add num only; null = add both.
+__global__ void __launch_bounds__(kThreads, 4)
 compress_scatter_blocked_kernel(const float *__restrict__ Wn, const float *__restrict__ slice_w, int weighted,
-                                const float4 *__restrict__ qm, int n_pix,
-                                const float *__restrict__ quat, int n, float4 *__restrict__ acc,
+                                const float4 *__restrict__ qm, const TileMap tm, int n_rot, int n_pix,
+                                const float4 *__restrict__ rotm, int n, float4 *__restrict__ acc,
                                 const int *__restrict__ changed) {
-    __shared__ float rm[9];
     const bool num_only = changed && *changed == 0;   // uniform over the grid
-    const int r = blockIdx.x;
-    float om = 1.f;
-    if (slice_w) {
-        const float sw = slice_w[r];
-        if (!(sw > 0.f)) return;                 // slice skipped (G17); uniform over the block
-        if (weighted) om = sw;
-    }
-    if (threadIdx.x == 0) {
-        RotMat m = rotation_matrix(quat + 4 * (size_t)r);
-#pragma unroll
-        for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
-    }
-    __syncthreads();
-    const unsigned h = (unsigned)n >> 1;
-    const unsigned per_copy = h * h * h;
     const unsigned lane = threadIdx.x & 31u;
-#pragma unroll
-    for (int j = 0; j < kPixPerThread; ++j) {
-        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
-        // every lane stays in the loop (the exchange below is warp-wide); a lane without a sample carries blk = -1
-        const int pc = p < n_pix ? p : n_pix - 1;
-        const float4 g = qm[pc];                               // (q, mask) in one 16-byte load
-        const Sample s = locate(rm, g.x, g.y, g.z, n);
-        const bool ok = p < n_pix && s.base >= 0 && g.w != 0.f;
-        const float v = ok ? Wn[(size_t)r * n_pix + pc] : 0.f;
-        int blk = -1;
-        if (ok) {
-            const unsigned c = ((s.bx & 1u) << 2) | ((s.by & 1u) << 1) | (s.bz & 1u);
-            blk = (int)(c * per_copy + (((unsigned)s.bx >> 1) * h + ((unsigned)s.by >> 1)) * h + ((unsigned)s.bz >> 1));
+    const int n_items = n_rot * tm.n_bands;
+    for (int item = blockIdx.x * kWarps + (threadIdx.x >> 5); item < n_items; item += gridDim.x * kWarps) {
+        const int r = item / tm.n_bands;
+        float om = 1.f;
+        if (slice_w) {
+            const float sw = slice_w[r];
+            if (!(sw > 0.f)) continue;           // slice skipped (G17); uniform over the warp
+            if (weighted) om = sw;
         }
-        if (num_only) scatter_rounds<true>(acc, blk, s.tx, s.ty, s.tz, v, om, lane);
-        else scatter_rounds<false>(acc, blk, s.tx, s.ty, s.tz, v, om, lane);
+        float rm[9];
+        load_rotation(rotm, r, rm);
+        const Band band(tm, item - r * tm.n_bands, (int)lane);
+        const float *const w_row = Wn + (size_t)r * n_pix;
+        for (int t0 = 0; t0 < band.n_tiles; t0 += kTilesPerStep) {
+            // the geometry and the loads of four tiles first (independent), then the four exchanges
+            Sample smp[kTilesPerStep];
+            float val[kTilesPerStep];
+            int blk[kTilesPerStep];
+            float4 g[kTilesPerStep];
+            int pix[kTilesPerStep];
+#pragma unroll
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                pix[j] = band.pixel(t0 + j);
+                g[j] = qm[max(pix[j], 0)];                     // (q, mask) in one 16-byte load
+                val[j] = w_row[max(pix[j], 0)];
+            }
+#pragma unroll
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                // every lane stays in the loop (the exchange is warp-wide); a lane without a sample carries blk = -1
+                smp[j] = locate(rm, g[j].x, g[j].y, g[j].z, n);
+                const bool ok = pix[j] >= 0 && smp[j].base >= 0 && g[j].w != 0.f;
+                blk[j] = ok ? smp[j].base : -1;
+            }
+#pragma unroll
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                if (__all_sync(0xffffffffu, blk[j] < 0)) continue;     // warp-uniform: nothing to send (ragged edge, masked tile)
+                if (num_only) scatter_rounds<true>(acc, blk[j], smp[j].tx, smp[j].ty, smp[j].tz, val[j], om, lane);
+                else scatter_rounds<false>(acc, blk[j], smp[j].tx, smp[j].ty, smp[j].tz, val[j], om, lane);
+            }
+        }
     }
 }
 
@@ -149,15 +157,12 @@ compress_divide_blocked_kernel(const float *__restrict__ acc, int n, float *__re
     const size_t g = (size_t)n * n * n;
     if (l >= g) return;
     const int z = (int)(l % n), y = (int)((l / n) % n), x = (int)(l / ((size_t)n * n));
-    const unsigned h = (unsigned)n >> 1;
-    const size_t per_copy = (size_t)h * h * h;
     float num = 0.f, den = 0.f;
 #pragma unroll
     for (int d = 0; d < 8; ++d) {
         const int bx = x - (d >> 2), by = y - ((d >> 1) & 1), bz = z - (d & 1);
         if (bx < 0 || by < 0 || bz < 0 || bx > n - 2 || by > n - 2 || bz > n - 2) continue;
-        const unsigned c = ((bx & 1u) << 2) | ((by & 1u) << 1) | (bz & 1u);
-        const size_t blk = c * per_copy + (((size_t)(bx >> 1) * h + (by >> 1)) * h + (bz >> 1));
+        const size_t blk = ((size_t)bx * n + by) * n + bz;
         num += acc[16 * blk + d];
         den += acc[16 * blk + 8 + d];
     }
@@ -165,98 +170,37 @@ compress_divide_blocked_kernel(const float *__restrict__ acc, int n, float *__re
     if (den_out) den_out[l] = den;
 }
 
-// grid = (R, ceil(P / kPixPerBlock))
-__global__ void __launch_bounds__(kThreads)
-compress_scatter_kernel(const float *__restrict__ Wn, const float *__restrict__ slice_w, int weighted,
-                        const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix,
-                        const float *__restrict__ quat, int n, float2 *__restrict__ acc) {
-    __shared__ float rm[9];
-    const int r = blockIdx.x;
-    float om = 1.f;
-    if (slice_w) {
-        const float sw = slice_w[r];
-        if (!(sw > 0.f)) return;                 // slice skipped (G17); uniform over the block
-        if (weighted) om = sw;
-    }
-    if (threadIdx.x == 0) {
-        RotMat m = rotation_matrix(quat + 4 * (size_t)r);
-#pragma unroll
-        for (int i = 0; i < 9; ++i) rm[i] = m.m[i];
-    }
-    __syncthreads();
-    const int nn = n * n;
-#pragma unroll
-    for (int j = 0; j < kPixPerThread; ++j) {
-        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
-        if (p >= n_pix) continue;
-        if (mask && mask[p] == 0) continue;
-        const Sample s = locate(rm, q[3 * p], q[3 * p + 1], q[3 * p + 2], n);
-        if (s.base < 0) continue;
-        const float v = Wn[(size_t)r * n_pix + p];
-        const float x1 = s.tx * om, x0 = (1.f - s.tx) * om;
-        const float y1 = s.ty, y0 = 1.f - s.ty, z1 = s.tz, z0 = 1.f - s.tz;
-        float2 *b = acc + s.base;
-        float f;
-        f = x0 * y0 * z0; red_add_v2(b, f * v, f);
-        f = x0 * y0 * z1; red_add_v2(b + 1, f * v, f);
-        f = x0 * y1 * z0; red_add_v2(b + n, f * v, f);
-        f = x0 * y1 * z1; red_add_v2(b + n + 1, f * v, f);
-        f = x1 * y0 * z0; red_add_v2(b + nn, f * v, f);
-        f = x1 * y0 * z1; red_add_v2(b + nn + 1, f * v, f);
-        f = x1 * y1 * z0; red_add_v2(b + nn + n, f * v, f);
-        f = x1 * y1 * z1; red_add_v2(b + nn + n + 1, f * v, f);
-    }
-}
-
-__global__ void __launch_bounds__(256)
-compress_divide_kernel(const float2 *__restrict__ acc, size_t g, float *__restrict__ model_out,
-                       float *__restrict__ den_out) {
-    const size_t l = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (l >= g) return;
-    const float2 a = acc[l];
-    model_out[l] = a.y > 0.f ? a.x / a.y : 0.f;
-    if (den_out) den_out[l] = a.y;
-}
-
 }  // namespace
 
-size_t compress_scratch_float2(int n, int n_pix) { return (size_t)8 * n * n * n + (size_t)2 * n_pix; }
+size_t compress_scratch_float2(int n) { return (size_t)8 * n * n * n; }
 
-emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const float *q,
-                           const uint8_t *mask, int n_pix, const float *quat, int n_rot, int n,
+emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const Geometry &geo, int n,
                            float2 *acc, float *model_out, float *den_out, cudaStream_t st, const DenCache *cache) {
     const size_t g = (size_t)n * n * n;
-    dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
-    if ((n & 1) == 0) {
-        float4 *acc4 = reinterpret_cast<float4 *>(acc);          // 8 grids x (n/2)^3 blocks x 64 B = 8 G float2
-        const float *accf = reinterpret_cast<const float *>(acc);
-        const int w = weighted ? 1 : 0;
-        float4 *qm = reinterpret_cast<float4 *>(acc + 8 * g);     // after the accumulators
-        EMC_TRY(launch_pack_geometry(q, mask, n_pix, qm, st));
-        if (cache && slice_w && !weighted) {
-            // den is reused while the set of skipped slices stays the one it was accumulated for (decided on the device)
-            EMC_TRY_CUDA(cudaMemsetAsync(cache->changed, 0, sizeof(int), st));
-            active_check_kernel<<<ceil_div(n_rot, 256), 256, 0, st>>>(slice_w, n_rot, cache->active,
-                                                                                 cache->changed, cache->force ? 1 : 0);
-            EMC_LAUNCHED();
-            compress_clear_kernel<<<(unsigned)((4 * g + 255) / 256), 256, 0, st>>>(acc4, g, cache->changed);   // g blocks of 64 B
-            EMC_LAUNCHED();
-            compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, w, qm, n_pix, quat, n, acc4,
-                                                                       cache->changed);
-            EMC_LAUNCHED();
-        } else {
-            EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * 8 * sizeof(float2), st));
-            compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, w, qm, n_pix, quat, n, acc4, nullptr);
-            EMC_LAUNCHED();
-        }
-        compress_divide_blocked_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(accf, n, model_out, den_out);
+    const int n_pix = geo.n_pix, n_rot = geo.n_rot;
+    float4 *acc4 = reinterpret_cast<float4 *>(acc);          // n^3 blocks x 64 B = 8 G float2
+    const float *accf = reinterpret_cast<const float *>(acc);
+    const int w = weighted ? 1 : 0;
+    const TileMap tm = make_tile_map(n_pix, geo.row_len);
+    const long long items = (long long)n_rot * tm.n_bands;
+    const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
+    if (cache && slice_w && !weighted) {
+        // den is reused while the set of skipped slices stays the one it was accumulated for (decided on the device)
+        EMC_TRY_CUDA(cudaMemsetAsync(cache->changed, 0, sizeof(int), st));
+        active_check_kernel<<<ceil_div(n_rot, 256), 256, 0, st>>>(slice_w, n_rot, cache->active, cache->changed,
+                                                                  cache->force ? 1 : 0);
         EMC_LAUNCHED();
-        return EMC_OK;
+        compress_clear_kernel<<<(unsigned)((4 * g + 255) / 256), 256, 0, st>>>(acc4, g, cache->changed);   // g blocks of 64 B
+        EMC_LAUNCHED();
+        compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, w, geo.qm, tm, n_rot, n_pix, geo.rotm, n, acc4,
+                                                                   cache->changed);
+        EMC_LAUNCHED();
+    } else {
+        EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * 8 * sizeof(float2), st));
+        compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, w, geo.qm, tm, n_rot, n_pix, geo.rotm, n, acc4, nullptr);
+        EMC_LAUNCHED();
     }
-    EMC_TRY_CUDA(cudaMemsetAsync(acc, 0, g * sizeof(float2), st));
-    compress_scatter_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, weighted ? 1 : 0, q, mask, n_pix, quat, n, acc);
-    EMC_LAUNCHED();
-    compress_divide_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(acc, g, model_out, den_out);
+    compress_divide_blocked_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(accf, n, model_out, den_out);
     EMC_LAUNCHED();
     return EMC_OK;
 }

@@ -5,6 +5,8 @@
 //
 // Fused into the same pass: logW = log(max(W,1e-30)) split into two fp16 planes
 // (hi, lo) with masked / outside samples zeroed, and S[r] = sum_{p:mask} W[r,p].
+#include <algorithm>
+
 #include "emc_geometry.cuh"
 #include "emc_internal.cuh"
 
@@ -33,8 +35,13 @@ __device__ __forceinline__ float block_sum(float v, float *red) {
 
 // logW -> two fp16 planes: hi = fp16(lw), lo = fp16(lw - hi); 22 significand bits in all.
 // gauss (the paper's Gaussian model): the operand is W itself, not log W
+// FAST: __logf (one MUFU.LG2 and a multiply; absolute error <= 2^-21.41 on [0.5, 2], else <= 3 ulp, CUDA Math API) in
+// the place of logf (about 22 instructions, 1 ulp): |d logW| <= 3.6e-7 max(1, |logW|), against T1's 1e-5 (K |logW| + W)
+// summed over the pixels -- the same order as the fp32 accumulation error of the contraction.
+template <bool FAST = false>
 __device__ __forceinline__ void split_logw(float w, bool live, __half &hi, __half &lo, int gauss = 0) {
-    float lw = live ? (gauss ? w : logf(fmaxf(w, 1e-30f))) : 0.f;
+    const float lg = FAST ? __logf(fmaxf(w, 1e-30f)) : logf(fmaxf(w, 1e-30f));
+    float lw = live ? (gauss ? w : lg) : 0.f;
     hi = __float2half_rn(lw);
     lo = __float2half_rn(lw - __half2float(hi));
 }
@@ -90,25 +97,18 @@ expand_kernel(const float *__restrict__ model, int n, const float *__restrict__ 
     }
 }
 
-// ---- blocked, staggered copies of the model (n even) -----------------------------------------
+// ---- corner blocks of the model ---------------------------------------------------------------
 // A sample reads the 2x2x2 voxels at its base corner b.  In the plain [n][n][n] layout these are 8
-// gathers on 4 different cache lines.  Here the model is re-laid as 8 copies, one per parity
-// (b_x&1, b_y&1, b_z&1) of the base; copy c holds, for every base of that parity, the 8 corner values
-// as one aligned 32-byte block (corner order 4*dx + 2*dy + dz), blocks ordered [b_x/2][b_y/2][b_z/2].
-// One sample = two 16-byte loads from one sector-aligned block; z-adjacent bases share a cache line.
-// Cost: 32 G bytes written once per iteration (8 MB at 64^3), L2-resident up to n = 128.
+// gathers on 4 different cache lines.  Here the model is re-laid as one aligned 32-byte block per BASE
+// CORNER: blocked[(b_x n + b_y) n + b_z] = the 8 corner values (order 4 dx + 2 dy + dz), i.e. the block index is
+// the index map itself.  One sample = ONE 32-byte gather; a 128-byte line holds the blocks of 4 z-adjacent bases
+// (2 x 2 x 5 voxels).  Cost: 32 G bytes written once per iteration (8 MB at 64^3), L2-resident up to n = 128.
 __global__ void __launch_bounds__(256)
 build_blocked_kernel(const float *__restrict__ model, int n, float4 *__restrict__ blocked) {
-    const int h = n >> 1;
-    const size_t per_copy = (size_t)h * h * h;
+    const size_t g = (size_t)n * n * n;
     const size_t t = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (t >= 8 * per_copy) return;
-    const int c = (int)(t / per_copy);
-    size_t i = t - (size_t)c * per_copy;
-    const int bk = 2 * (int)(i % h) + (c & 1);
-    i /= h;
-    const int bj = 2 * (int)(i % h) + ((c >> 1) & 1);
-    const int bi = 2 * (int)(i / h) + ((c >> 2) & 1);
+    if (t >= g) return;
+    const int bk = (int)(t % n), bj = (int)((t / n) % n), bi = (int)(t / ((size_t)n * n));
     float v[8];
 #pragma unroll
     for (int d = 0; d < 8; ++d) {
@@ -119,83 +119,117 @@ build_blocked_kernel(const float *__restrict__ model, int n, float4 *__restrict_
     blocked[2 * t + 1] = make_float4(v[4], v[5], v[6], v[7]);
 }
 
-// One 32-byte corner block in one request (LDG.256): a divergent gather costs the L1 one tag lookup per lane and
-// instruction, so two 16-byte loads of the same block cost twice as much as this.
+// One 32-byte corner block in one request (LDG.256): a divergent gather costs the L1 one tag lookup per distinct
+// line and instruction, so two 16-byte loads of the same block cost twice as much as this.
 __device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b) {
     asm volatile("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                  : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
                  : "l"(p));
 }
 
-// q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0): one coalesced 16-byte load per sample
+// q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0): one 16-byte load per sample; the rotation matrices
+// (float64 arithmetic, G4) once per rotation instead of once per thread block
 __global__ void __launch_bounds__(256)
-pack_geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix, float4 *__restrict__ qm) {
-    const int p = blockIdx.x * 256 + threadIdx.x;
-    if (p >= n_pix) return;
-    qm[p] = make_float4(q[3 * p], q[3 * p + 1], q[3 * p + 2], (mask && mask[p] == 0) ? 0.f : 1.f);
+geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, int n_pix, const float *__restrict__ quat,
+                int n_rot, float4 *__restrict__ qm, float4 *__restrict__ rotm) {
+    const int t = blockIdx.x * 256 + threadIdx.x;
+    if (t < n_pix) qm[t] = make_float4(q[3 * t], q[3 * t + 1], q[3 * t + 2], (mask && mask[t] == 0) ? 0.f : 1.f);
+    if (t < n_rot) {
+        const RotMat m = rotation_matrix(quat + 4 * (size_t)t);
+        rotm[3 * (size_t)t] = make_float4(m.m[0], m.m[1], m.m[2], 0.f);
+        rotm[3 * (size_t)t + 1] = make_float4(m.m[3], m.m[4], m.m[5], 0.f);
+        rotm[3 * (size_t)t + 2] = make_float4(m.m[6], m.m[7], m.m[8], 0.f);
+    }
 }
 
-// The kernel is bound by instruction issue (about 180 warp instructions per 32 samples before this version,
-// ncu r01_v2), not by memory, so it is specialised on the outputs it has to write, reads its geometry as one
-// float4 per pixel and has no divergent control flow: a lane past the end of the detector repeats the last
-// pixel and only its stores are predicated.
+// One WARP per (rotation, band) work item (a stride loop covers item counts beyond the grid limit).  A warp works on a
+// 4 x 8 TILE of detector pixels at a time (its 32 samples cover about 3 x 6 voxels of the slice: 21 distinct corner
+// blocks per gather against 25 for 32 pixels of a detector row), four tiles per step in PHASES so that the loads of
+// a phase are all in flight together: geometry loads; coordinates; gathers; interpolation and outputs.  The kernel
+// is specialised on the outputs it has to write and has no divergent control flow: a lane without a pixel repeats
+// pixel 0 and only its stores are predicated.  What bounds it (ncu, profiles/r02_expand_compress.md): the issue
+// slots (125 warp instructions per 32 samples, 62 % of the slots used) with the waits for the gather exposed; capping
+// registers for more warps per SM (spills) or making the warps persistent over long bands were both slower.
+// S_part [R][n_bands]: sum_{p:mask} W (or W^2) of each band, summed per rotation in a fixed order by rowsum_kernel
+// (bitwise reproducible S, no atomics).
+constexpr int kWarps = kThreads / 32;
 template <bool W_OUT, bool IDX_OUT, bool PLANES>
-__global__ void __launch_bounds__(kThreads)
-expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, int n_pix,
-                      const float *__restrict__ quat, float *__restrict__ W, int32_t *__restrict__ idx,
-                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S, int gauss) {
-    __shared__ float rm_s[9];
-    __shared__ float red[kThreads / 32];
-    const int r = blockIdx.x;
-    if (threadIdx.x == 0) {
-        RotMat m = rotation_matrix(quat + 4 * (size_t)r);
+__global__ void __launch_bounds__(kThreads, 4)
+expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, const TileMap tm,
+                      const float4 *__restrict__ rotm, int n_rot, int n_pix, float *__restrict__ W, int32_t *__restrict__ idx,
+                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S_part, int gauss) {
+    const int lane = threadIdx.x & 31;
+    const int n_items = n_rot * tm.n_bands;
+    for (int item = blockIdx.x * kWarps + (threadIdx.x >> 5); item < n_items; item += gridDim.x * kWarps) {
+        const int r = item / tm.n_bands;
+        float rm[9];
+        load_rotation(rotm, r, rm);
+        const Band band(tm, item - r * tm.n_bands, lane);
+        float *const w_row = W_OUT ? W + (size_t)r * n_pix : nullptr;
+        int32_t *const i_row = IDX_OUT ? idx + (size_t)r * n_pix : nullptr;
+        __half *const hi_row = PLANES ? planes + (size_t)r * ld_p : nullptr;
+        __half *const lo_row = PLANES ? hi_row + plane_stride : nullptr;
+        float part = 0.f;
+        for (int t0 = 0; t0 < band.n_tiles; t0 += kTilesPerStep) {
+            int pix[kTilesPerStep];
+            float4 g[kTilesPerStep];
 #pragma unroll
-        for (int i = 0; i < 9; ++i) rm_s[i] = m.m[i];
-    }
-    __syncthreads();
-    float rm[9];
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                pix[j] = band.pixel(t0 + j);
+                g[j] = qm[max(pix[j], 0)];
+            }
+            Sample s[kTilesPerStep];
+            float4 lo4[kTilesPerStep], hi4[kTilesPerStep];
 #pragma unroll
-    for (int i = 0; i < 9; ++i) rm[i] = rm_s[i];
-    const unsigned h = (unsigned)n >> 1;
-    const unsigned per_copy = h * h * h;                    // 8 * per_copy <= 2^30 for n <= 1024
-    float part = 0.f;
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                s[j] = locate(rm, g[j].x, g[j].y, g[j].z, n);
+                // outside samples read block 0 (any valid address) and are zeroed afterwards
+                ldg256(blocked + 2 * (size_t)(unsigned)max(s[j].base, 0), lo4[j], hi4[j]);
+            }
 #pragma unroll
-    for (int j = 0; j < kPixPerThread; ++j) {
-        const int p = blockIdx.y * kPixPerBlock + j * kThreads + threadIdx.x;
-        const bool in = p < n_pix;
-        const float4 g = qm[in ? p : n_pix - 1];
-        const Sample s = locate(rm, g.x, g.y, g.z, n);
-        const bool inside = s.base >= 0;
-        // outside samples read block 0 (any valid address) and are zeroed afterwards
-        const unsigned bx = inside ? (unsigned)s.bx : 0u, by = inside ? (unsigned)s.by : 0u, bz = inside ? (unsigned)s.bz : 0u;
-        const unsigned c = ((bx & 1u) << 2) | ((by & 1u) << 1) | (bz & 1u);
-        const unsigned blk = c * per_copy + ((bx >> 1) * h + (by >> 1)) * h + (bz >> 1);
-        float4 lo4, hi4;
-        ldg256(blocked + 2 * (size_t)blk, lo4, hi4);
-        const float z0 = 1.f - s.tz, y0 = 1.f - s.ty, x0 = 1.f - s.tx;
-        const float c00 = lo4.x * z0 + lo4.y * s.tz;
-        const float c01 = lo4.z * z0 + lo4.w * s.tz;
-        const float c10 = hi4.x * z0 + hi4.y * s.tz;
-        const float c11 = hi4.z * z0 + hi4.w * s.tz;
-        float w = (c00 * y0 + c01 * s.ty) * x0 + (c10 * y0 + c11 * s.ty) * s.tx;
-        w = inside ? w : 0.f;
-        const size_t o = (size_t)r * n_pix + p;
-        if (W_OUT && in) W[o] = w;
-        if (IDX_OUT && in) idx[o] = s.base;
-        const bool use = in && g.w != 0.f;
-        if (PLANES && in) {
-            __half hi, lo;
-            split_logw(w, use && inside, hi, lo, gauss);
-            const size_t po = (size_t)r * ld_p + p;
-            planes[po] = hi;
-            planes[plane_stride + po] = lo;
+            for (int j = 0; j < kTilesPerStep; ++j) {
+                const bool in = pix[j] >= 0, inside = s[j].base >= 0;
+                const int pc = max(pix[j], 0);
+                const float tx = s[j].tx, ty = s[j].ty, tz = s[j].tz;
+                const float z0 = 1.f - tz, y0 = 1.f - ty, x0 = 1.f - tx;
+                const float c00 = lo4[j].x * z0 + lo4[j].y * tz;
+                const float c01 = lo4[j].z * z0 + lo4[j].w * tz;
+                const float c10 = hi4[j].x * z0 + hi4[j].y * tz;
+                const float c11 = hi4[j].z * z0 + hi4[j].w * tz;
+                float w = (c00 * y0 + c01 * ty) * x0 + (c10 * y0 + c11 * ty) * tx;
+                w = inside ? w : 0.f;
+                if (W_OUT && in) w_row[pc] = w;
+                if (IDX_OUT && in) i_row[pc] = s[j].base;
+                const bool use = in && g[j].w != 0.f;
+                if (PLANES) {
+                    __half hi, lo;
+                    split_logw<true>(w, use && inside, hi, lo, gauss);
+                    if (in) {
+                        hi_row[pc] = hi;
+                        lo_row[pc] = lo;
+                    }
+                }
+                part += use ? (gauss ? w * w : w) : 0.f;
+            }
         }
-        part += use ? (gauss ? w * w : w) : 0.f;
+        if (PLANES) {                                        // S accompanies the planes (log-likelihood operands)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+            if (lane == 0) S_part[item] = part;
+        }
     }
-    if (PLANES) {                                            // S accompanies the planes (log-likelihood operands)
-        const float t = block_sum(part, red);
-        if (threadIdx.x == 0) atomicAdd(S + r, t);
-    }
+}
+
+// S[r] = sum of the row's band partials, in a fixed order (one warp per rotation)
+__global__ void __launch_bounds__(256)
+rowsum_kernel(const float *__restrict__ S_part, int n_rot, int n_bands, float *__restrict__ S) {
+    const int r = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (r >= n_rot) return;
+    float t = 0.f;
+    for (int b = lane; b < n_bands; b += 32) t += S_part[(size_t)r * n_bands + b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) S[r] = t;
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -226,33 +260,41 @@ logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
 
 }  // namespace
 
-static size_t expand_blocked_floats(int n) { return (size_t)8 * n * n * n; }
-// blocked model copies + one float4 of geometry per pixel
-emc_status launch_pack_geometry(const float *q, const uint8_t *mask, int n_pix, float4 *qm, cudaStream_t st) {
-    pack_geometry_kernel<<<ceil_div(n_pix, 256), 256, 0, st>>>(q, mask, n_pix, qm);
+size_t geometry_float4(int n_pix, int n_rot) { return (size_t)n_pix + 3 * (size_t)n_rot; }
+
+emc_status launch_geometry(const float *q, const uint8_t *mask, int n_pix, int row_len, const float *quat, int n_rot,
+                           float4 *buf, Geometry *out, cudaStream_t st) {
+    float4 *qm = buf, *rotm = buf + n_pix;
+    const int n = n_pix > n_rot ? n_pix : n_rot;
+    geometry_kernel<<<ceil_div(n, 256), 256, 0, st>>>(q, mask, n_pix, quat, n_rot, qm, rotm);
     EMC_LAUNCHED();
+    *out = Geometry{qm, rotm, n_pix, n_rot, row_len};
     return EMC_OK;
 }
 
-size_t expand_scratch_floats(int n, int n_pix) { return (n & 1) ? 0 : expand_blocked_floats(n) + (size_t)4 * n_pix; }
+// corner blocks of the model + the band partials of S (at most one band per 4 pixels... per 32 pixels of a row)
+size_t expand_scratch_floats(int n, int n_pix, int n_rot) {
+    return (size_t)8 * n * n * n + (size_t)n_rot * (size_t)((n_pix + 31) / 32 + 1);
+}
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, cudaStream_t st, bool gauss) {
-    dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
+                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss) {
     const int g = gauss ? 1 : 0;
     if (planes && !S) return EMC_ERR_ARG;
-    if (blocked && (n & 1) == 0) {
-        const size_t blocks = (size_t)n * n * n;              // 8 copies x (n/2)^3 blocks
-        float4 *qm = reinterpret_cast<float4 *>(blocked + expand_blocked_floats(n));
+    if (blocked && geo) {
+        const size_t blocks = (size_t)n * n * n;              // one 32-byte block per base corner
         build_blocked_kernel<<<(unsigned)((blocks + 255) / 256), 256, 0, st>>>(model, n, (float4 *)blocked);
-        EMC_LAUNCHED();
-        pack_geometry_kernel<<<ceil_div(n_pix, 256), 256, 0, st>>>(q, mask, n_pix, qm);
         EMC_LAUNCHED();
         const float4 *b4 = (const float4 *)blocked;
         const size_t ps = (size_t)n_rot * ld_p;
+        const TileMap tm = make_tile_map(n_pix, geo->row_len);
+        // band partials of S live behind the corner blocks (expand_scratch_floats)
+        float *S_part = blocked + (size_t)8 * n * n * n;
+        const long long items = (long long)n_rot * tm.n_bands;
+        const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
 #define EMC_EXPAND_CASE(w_, i_, p_)                                                                                   \
-    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, qm, n_pix, quat, W, idx, planes, ld_p, ps, S, g)
+    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g)
         const int sel = (W ? 4 : 0) | (idx ? 2 : 0) | (planes ? 1 : 0);
         switch (sel) {
             case 1: EMC_EXPAND_CASE(false, false, true); break;
@@ -263,8 +305,13 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         }
 #undef EMC_EXPAND_CASE
         EMC_LAUNCHED();
+        if (planes) {
+            rowsum_kernel<<<ceil_div(n_rot, 8), 256, 0, st>>>(S_part, n_rot, tm.n_bands, S);
+            EMC_LAUNCHED();
+        }
         return EMC_OK;
     }
+    dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
     expand_kernel<<<grid, kThreads, 0, st>>>(model, n, q, mask, n_pix, quat, W, idx, planes, ld_p,
                                              (size_t)n_rot * ld_p, S, g);
     EMC_LAUNCHED();

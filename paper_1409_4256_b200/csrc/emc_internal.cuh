@@ -64,17 +64,27 @@ struct Arena {
 enum PlaneFormat { FMT_F16 = 0, FMT_BF16 = 1 };   // = the UMMA instruction descriptor encoding
 
 // ---------------------------------------------------------------- stage launchers (device work)
+// Sample geometry prepared once per call (emc_expand.cu): q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0),
+// the rotation matrices as three float4 per rotation (rows of R_r, .w unused), the detector's row length for the tiling.
+struct Geometry {
+    const float4 *qm;     // [P]
+    const float4 *rotm;   // [R][3]
+    int n_pix, n_rot, row_len;
+};
+size_t geometry_float4(int n_pix, int n_rot);   // float4s of scratch behind a Geometry
+emc_status launch_geometry(const float *q, const uint8_t *mask, int n_pix, int row_len, const float *quat, int n_rot,
+                           float4 *buf, Geometry *out, cudaStream_t st);
+
 // Expand (emc_expand.cu).  Any of W, idx, planes may be null.  planes = [2][R][ld_p] fp16 (hi, lo)
-// of logW with masked / outside samples zeroed; S[r] += sum_{p:mask} W (S zeroed by the caller).  gauss: the planes
+// of logW with masked / outside samples zeroed; S[r] = sum_{p:mask} W (the plain-gather kernel adds into S: zero it first).  gauss: the planes
 // hold W itself and S[r] += sum_{p:mask} W^2 (the operands of the paper's Gaussian model).
-// `blocked` = scratch of expand_scratch_floats(n, n_pix) floats (blocked model copies + packed geometry; then W / idx
-// or planes, not both), or null (plain gathers).
-size_t expand_scratch_floats(int n, int n_pix);
+// `blocked` = scratch of expand_scratch_floats() floats (corner blocks of the model, band partials of S) with `geo`
+// prepared, or both null:
+// plain gathers from q / mask / quat.
+size_t expand_scratch_floats(int n, int n_pix, int n_rot);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, cudaStream_t st, bool gauss = false);
-// q and the mask as one float4 per pixel (x, y, z, use ? 1 : 0)
-emc_status launch_pack_geometry(const float *q, const uint8_t *mask, int n_pix, float4 *qm, cudaStream_t st);
+                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss = false);
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
@@ -171,9 +181,9 @@ emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
 
-// Compress (emc_compress.cu).  acc = compress_scratch_float2(n, n_pix) float2 of scratch (8 staggered grids of corner
-// blocks + packed geometry), zeroed inside.
-size_t compress_scratch_float2(int n, int n_pix);
+// Compress (emc_compress.cu).  acc = compress_scratch_float2(n) float2 of scratch (one 64-byte (num, den) corner
+// block per base corner), zeroed inside.
+size_t compress_scratch_float2(int n);
 // cache (optional, eq. 2.10 with slice_w only): den survives in `acc` from one call to the next and is reused while the
 // set {r: slice_w[r] > 0} stays the one in cache->active; force = accumulate it afresh (first iteration, new list).
 struct DenCache {
@@ -181,8 +191,7 @@ struct DenCache {
     int *changed;       // device flag, scratch
     bool force;
 };
-emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const float *q,
-                           const uint8_t *mask, int n_pix, const float *quat, int n_rot, int n,
+emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const Geometry &geo, int n,
                            float2 *acc, float *model_out, float *den_out, cudaStream_t st,
                            const DenCache *cache = nullptr);
 

@@ -57,7 +57,7 @@ def test_null_arguments_are_rejected_synchronously():
     lib = emc.load()
     assert lib.emc_expand(None, None, None, None, None, None, 0, None) == emc.EMC_ERR_ARG
     assert lib.emc_check(None, None) == emc.EMC_ERR_ARG
-    det = binding._Detector(16, 8, None)
+    det = binding._Detector(16, 8, None, 0)
     pat = binding._Patterns(4, 8, emc.binding.EMC_U16)
     # misaligned / missing workspace
     assert lib.emc_loglik(8, None, det, pat, 4, 16, 64, 0, None, 0, None) == emc.EMC_ERR_WORKSPACE

@@ -30,7 +30,7 @@ def c2(inputs_cache):
 def test_c2_stagewise_and_end_to_end(c2):
     inp, ref = c2
     cfg = inp.cfg
-    d_q, d_mask, d_quat, d_w, d_k = dev(inp.q), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]), dev(inp.counts)
+    d_q, d_mask, d_quat, d_w, d_k = dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]), dev(inp.counts)
 
     # stage 1: index map bit-exact over all 5000 x 4096 samples
     w, idx = emc.emc_expand(dev(inp.model_init), d_q, d_quat)

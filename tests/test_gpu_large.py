@@ -41,7 +41,7 @@ def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
     cfg = inp.cfg
     quat, weight = inp.quat[stage], inp.weight[stage]
     n_rot, n_pix = quat.shape[0], cfg.n_pix
-    d_q, d_mask, d_quat, d_k = dev(inp.q), dev(inp.mask), dev(quat), dev(inp.counts)
+    d_q, d_mask, d_quat, d_k = dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask), dev(quat), dev(inp.counts)
     rows = sampled_rows(n_rot, n_rows, 7)
     if n_rot * n_pix > 2 ** 31:                                       # rows on both sides of the 32-bit boundary
         edge = 2 ** 31 // n_pix
@@ -123,7 +123,7 @@ def test_c4_route_pattern_chunks_from_host(inputs_cache):
     cfg = inp.cfg
     quat, weight = inp.quat[0], inp.weight[0]
     n_rot, n_pix = quat.shape[0], cfg.n_pix
-    d_model, d_q, d_mask, d_quat, d_w = dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(quat), dev(weight)
+    d_model, d_q, d_mask, d_quat, d_w = dev(inp.model_init), dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask), dev(quat), dev(weight)
     pinned = torch.from_numpy(inp.counts).pin_memory()
     out = emc.emc_iterate(d_model, d_q, d_mask, d_quat, d_w, pinned, n_pat_chunk=chunk, flags=emc.EMC_PATTERNS_ON_HOST)
     emc.emc_check(out["ws"])

@@ -49,7 +49,9 @@ class Case:
         self.inp, self.cfg = inp, inp.cfg
         self.quat, self.weight = inp.quat[stage], inp.weight[stage]
         self.d_model = dev(inp.model_init)
-        self.d_q = dev(inp.q)
+        nd = inp.cfg.n_det
+        self.d_q = dev(inp.q.reshape(nd, nd, 3))   # row-major 2-D detector: emc_detector.row_len = n_det (4 x 8 pixel tiles)
+        self.d_q_flat = dev(inp.q)                  # [P, 3]: row_len = 0, 32 consecutive pixels per warp
         self.d_mask = dev(inp.mask)
         self.d_quat = dev(self.quat)
         self.d_weight = dev(self.weight)
@@ -69,9 +71,9 @@ def ref(case):
     return o.iterate(inp.model_init, inp.q, inp.mask, case.quat, case.weight, inp.counts)
 
 
-@pytest.mark.parametrize("use_ws", [True, False], ids=["blocked", "gather"])
-def test_expand_index_map_bit_exact_and_slices(case, ref, use_ws):
-    w, idx = emc.emc_expand(case.d_model, case.d_q, case.d_quat, use_ws=use_ws)
+@pytest.mark.parametrize("use_ws,tiled", [(True, True), (True, False), (False, False)], ids=["blocked-tiles", "blocked-rows", "gather"])
+def test_expand_index_map_bit_exact_and_slices(case, ref, use_ws, tiled):
+    w, idx = emc.emc_expand(case.d_model, case.d_q if tiled else case.d_q_flat, case.d_quat, use_ws=use_ws)
     assert np.array_equal(host(idx), ref["idx"])                     # T4: bit-exact
     w = host(w)
     scale = np.abs(ref["W"]).max()
