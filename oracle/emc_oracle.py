@@ -295,6 +295,92 @@ def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=Fal
 
 
 # ----------------------------------------------------------------------------------------------
+# Rotation chunks (the paper's own streaming, "chunk C_c", 203; DESIGN.md section 11 NEXT-2)
+# ----------------------------------------------------------------------------------------------
+
+def _merge_max_sum(m, z, a):
+    """(m, z) <- merged with the (max, sum) of the rows `a` of one chunk.  A column in which nothing
+    finite has been seen yet (zero weights: a = -inf) carries m = -inf, z = 0."""
+    m_c = a.max(axis=0)
+    live_c, live = np.isfinite(m_c), np.isfinite(m)
+    with np.errstate(invalid="ignore"):
+        z_c = np.where(live_c, np.exp(a - np.where(live_c, m_c, 0.0)[None, :]).sum(axis=0), 0.0)
+        m_new = np.maximum(m, m_c)
+        ref = np.where(np.isfinite(m_new), m_new, 0.0)
+        z = np.where(live, z * np.exp(np.where(live, m, 0.0) - ref), 0.0) + np.where(live_c, z_c * np.exp(np.where(live_c, m_c, 0.0) - ref), 0.0)
+    return m_new, z
+
+
+def normalize_rotation_chunks(big_l, weight, n_rot_chunk):
+    """The normalisation of `normalize` when the rotations arrive in chunks C_c and only one chunk of
+    L is held at a time.  "Only maximal rotational probabilities and sums are necessary":
+    sweep 1 carries, per pattern d, the running maximum m_d and the running sum z_d of exp(a - m_d)
+    over the chunks seen so far,
+        m' = max(m, m_c),   z' = z exp(m - m') + z_c exp(m_c - m'),
+    with (m_c, z_c) the max and sum of chunk c alone; sweep 2 revisits every chunk with the final
+    (m_d, z_d):  P = exp(a - m_d) / z_d.  Same flush (G20), same s and LL as `normalize`.
+    Returns (P float64 [R,N], s float64 [R], LL float)."""
+    big_l = np.asarray(big_l).astype(np.float64)
+    lw = np.log(np.asarray(weight).astype(np.float64))
+    n_rot, n_pat = big_l.shape
+    m = np.full(n_pat, -np.inf)
+    z = np.zeros(n_pat)
+    for r0 in range(0, n_rot, n_rot_chunk):                     # sweep 1
+        a = big_l[r0:r0 + n_rot_chunk] + lw[r0:r0 + n_rot_chunk, None]
+        m, z = _merge_max_sum(m, z, a)
+    p = np.empty_like(big_l)
+    for r0 in range(0, n_rot, n_rot_chunk):                     # sweep 2
+        a = big_l[r0:r0 + n_rot_chunk] + lw[r0:r0 + n_rot_chunk, None]
+        p[r0:r0 + n_rot_chunk] = np.exp(a - m[None, :]) / z[None, :]
+    p[p < P_MIN] = 0.0                                          # G20
+    return p, p.sum(axis=1), float((m + np.log(z)).sum())
+
+
+def iterate_rotation_chunks(model, q, mask, quat, weight, counts, n_rot_chunk, weighted=False):
+    """One iteration of Algorithm 1 with the rotation list streamed in chunks of `n_rot_chunk`
+    (PAPER.md:164-166): nothing of size R x N or R x P is ever held.
+      sweep 1, per chunk: expand -> loglik -> merge the chunk's (max, sum) into the running ones
+      sweep 2, per chunk: expand -> loglik (again) -> P with the final (max, sum) -> update -> the
+               chunk's contribution to the numerator and denominator grids of Compress
+      last: model' = num / den (division as the final step).
+    Stage boundaries carry float32 as in `iterate`.  Returns dict(model, s, LL, den)."""
+    counts = np.asarray(counts)
+    quat = np.asarray(quat, dtype=np.float32)
+    weight = np.asarray(weight, dtype=np.float32)
+    n = np.asarray(model).shape[0]
+    n_rot, n_pat = quat.shape[0], counts.shape[0]
+    lw = np.log(weight.astype(np.float64))
+    m = np.full(n_pat, -np.inf)
+    z = np.zeros(n_pat)
+    for r0 in range(0, n_rot, n_rot_chunk):                     # sweep 1
+        sl = slice(r0, min(n_rot, r0 + n_rot_chunk))
+        w, idx = expand(model, q, quat[sl])
+        l32 = loglik(w, idx, counts, mask)[0].astype(np.float32)
+        a = l32.astype(np.float64) + lw[sl, None]
+        m, z = _merge_max_sum(m, z, a)
+    g = n * n * n
+    num, den = np.zeros(g), np.zeros(g)
+    s_all = np.zeros(n_rot)
+    for r0 in range(0, n_rot, n_rot_chunk):                     # sweep 2
+        sl = slice(r0, min(n_rot, r0 + n_rot_chunk))
+        w, idx = expand(model, q, quat[sl])
+        l32 = loglik(w, idx, counts, mask)[0].astype(np.float32)
+        a = l32.astype(np.float64) + lw[sl, None]
+        p = np.exp(a - m[None, :]) / z[None, :]
+        p[p < P_MIN] = 0.0
+        p32 = p.astype(np.float32)
+        wn, s = update(p32, counts, mask)
+        s_all[sl] = s
+        om = s.astype(np.float32) if weighted else (s > 0).astype(np.float32)
+        _, num_c, den_c = compress(wn, q, quat[sl], mask, n, slice_w=om)
+        num += num_c
+        den += den_c
+    with np.errstate(divide="ignore", invalid="ignore"):
+        new_model = np.where(den > 0, num / den, 0.0)
+    return dict(model=new_model.astype(np.float32).reshape(n, n, n), s=s_all, LL=float((m + np.log(z)).sum()), den=den)
+
+
+# ----------------------------------------------------------------------------------------------
 # Adaptive EMC, PAPER.md:205-210 (section 3.4, eq. 3.1)
 # ----------------------------------------------------------------------------------------------
 

@@ -448,3 +448,44 @@ def test_normalize_is_flush_to_zero_float32():
     big_l = np.array([[0.0, 0.0], [-95.0, -99.0]], np.float32)
     p, s, _ = o.normalize(big_l, np.full(2, 0.5, np.float32))
     assert s[1] == 0 and np.all(p[0] == 1.0)
+
+
+# ---------------------------------------------------------------------------------------------- rotation chunks (NEXT-2)
+
+@pytest.mark.parametrize("chunk", [1, 7, 64, 203, 500])
+def test_normalize_rotation_chunks_equals_unchunked(chunk):
+    """The streamed (max, sum) merge of PAPER.md:203 gives the soft-max of the whole rotation list: chunk sizes 1, ragged,
+    = R and > R; also columns whose maximum moves from chunk to chunk and a weight that is exactly 0."""
+    rng = np.random.default_rng(77)
+    n_rot, n_pat = 203, 41
+    big_l = (rng.standard_normal((n_rot, n_pat)) * 40.0 - 300.0).astype(np.float32)
+    big_l[np.arange(n_pat) * 4 % n_rot, np.arange(n_pat)] += 90.0         # maxima spread over the chunks
+    w = rng.random(n_rot).astype(np.float32) + 0.05
+    w[5] = 0.0
+    w /= w.sum()
+    with np.errstate(divide="ignore"):
+        p0, s0, ll0 = o.normalize(big_l, w)
+        p1, s1, ll1 = o.normalize_rotation_chunks(big_l, w, chunk)
+    assert np.abs(p1 - p0).max() <= 1e-13
+    assert np.abs(s1 - s0).max() <= 1e-12 and abs(ll1 - ll0) <= 1e-9 * abs(ll0)
+    assert np.abs(p1.sum(axis=0) - 1.0).max() <= 1e-12 and np.all(p1[5] == 0)
+    from scipy.special import softmax
+    with np.errstate(divide="ignore"):
+        ref = softmax(big_l.astype(np.float64) + np.log(w.astype(np.float64))[:, None], axis=0)
+    assert np.abs(p1 - ref).max() <= 1e-13
+
+
+@pytest.mark.parametrize("chunk,weighted", [(50, False), (64, True), (203, False), (1000, True)])
+def test_iterate_rotation_chunks_equals_iterate(inputs_cache, chunk, weighted):
+    """Streaming the rotation list changes nothing but the summation order: model', s and LL of the chunked iteration
+    equal those of `iterate` (itself pinned above) to float32 rounding."""
+    inp = inputs_cache("T1")
+    a = o.iterate(inp.model_init, inp.q, inp.mask, inp.quat[0], inp.weight[0], inp.counts, weighted=weighted)
+    b = o.iterate_rotation_chunks(inp.model_init, inp.q, inp.mask, inp.quat[0], inp.weight[0], inp.counts, chunk,
+                                  weighted=weighted)
+    assert np.abs(b["s"] - a["s"]).max() <= 1e-6 * max(1.0, a["s"].max())
+    assert abs(b["LL"] - a["LL"]) <= 1e-9 * abs(a["LL"])
+    cov = a["den"] >= 1e-6 * a["den"].max()
+    ma, mb = a["model"].reshape(-1)[cov], b["model"].reshape(-1)[cov]
+    assert np.abs(mb - ma).max() <= 2e-6 * np.abs(ma).max()
+    assert np.array_equal(a["den"] > 0, b["den"] > 0)
