@@ -202,6 +202,22 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
                        size_t ws_bytes, void *stream, emc_context *ctx);
 
+/* Algorithm 1 with the ROTATION list streamed in chunks of n_rot_chunk rotations, the paper's own memory scheme
+ * ("chunk C_c"; "only maximal rotational probabilities and sums are necessary", PAPER.md:203;
+ * DESIGN.md section 11 NEXT-2): nothing of size R x N or R x P is held, the workspace scales with the chunk.  Two
+ * sweeps over the chunks per iteration:
+ *   sweep 1, per chunk: Expand, log-likelihood, the chunk's per-pattern (max, sum) merged into the running ones
+ *   sweep 2, per chunk: Expand, log-likelihood (recomputed), P with the final (max, sum), s[r], update, and the
+ *                       chunk's scatter into the numerator / denominator grids of Compress; division after the last.
+ * Results are those of emc_iterate up to summation order; the log-likelihood contraction runs twice.
+ * Patterns are device-resident, in one pattern chunk.  Arguments as emc_iterate (no P_out);
+ * ws >= emc_workspace_bytes_rot_chunked(). */
+EMC_API size_t emc_workspace_bytes_rot_chunked(int n, int n_pix, int n_rot, int n_rot_chunk, int n_pat);
+EMC_API emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                                   const emc_patterns *pat, int n_iter, int n_rot_chunk, float *model_out,
+                                   double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
+                                   emc_context *ctx);
+
 /* Algorithm 1 with the paper's own likelihood: Gaussian around the slice with a fluence per (rotation, frame),
  * eqs. (2.2), (2.3), (2.5)/(2.11), (2.6), PAPER.md:70-89, 124-130 (NEXT-3, readings GA1-GA7):
  *   phi[r,d]  = sum_p K[d,p]^2 / sum_p W[r,p] K[d,p]                     (2.6), from the slices of this iteration

@@ -30,7 +30,8 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
-           "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_gaussian", "emc_refine", "emc_check",
+           "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
+           "emc_workspace_bytes_rot_chunked", "emc_iterate_gaussian", "emc_refine", "emc_check",
            "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
@@ -94,6 +95,11 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate.restype = ci
     lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                 ci, ci, vp, vp, ci, vp, cu, vp, sz, vp, vp]
+    lib.emc_workspace_bytes_rot_chunked.restype = sz
+    lib.emc_workspace_bytes_rot_chunked.argtypes = [ci, ci, ci, ci, ci]
+    lib.emc_iterate_rot_chunked.restype = ci
+    lib.emc_iterate_rot_chunked.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
+                                            ci, ci, vp, vp, cu, vp, sz, vp, vp]
     lib.emc_iterate_gaussian.restype = ci
     lib.emc_iterate_gaussian.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                          ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp, vp]
@@ -341,6 +347,26 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
                               p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream(),
                               _ctx(ctx, flags)), "emc_iterate")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
+
+
+def emc_iterate_rot_chunked(model, q, mask, quat, weight, counts, n_rot_chunk, n_iter=1, flags=0, ws=None, ctx=None):
+    """Algorithm 1 with the rotation list streamed in chunks.  Returns dict(model, loglik, ws)."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rot = _rotations(quat, weight)
+    pat = _patterns(counts, det.n_pix)
+    model_out = torch.empty_like(model)
+    loglik = torch.zeros(n_iter, dtype=torch.float64, device=model.device)
+    if ws is None:
+        nbytes = load().emc_workspace_bytes_rot_chunked(n, det.n_pix, rot.n_rot, n_rot_chunk, pat.n_pat)
+        if nbytes == 0:
+            raise EmcError(EMC_ERR_UNSUPPORTED, "emc_workspace_bytes_rot_chunked")
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=model.device)
+    _check(load().emc_iterate_rot_chunked(m, det, rot, pat, n_iter, n_rot_chunk, model_out.data_ptr(), loglik.data_ptr(),
+                                          flags, ws.data_ptr(), ws.numel(), _stream(), _ctx(ctx, flags)),
+           "emc_iterate_rot_chunked")
+    return dict(model=model_out, loglik=loglik, ws=ws)
 
 
 def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None, ctx=None):

@@ -134,7 +134,7 @@ emc_status reset_header(const Layout &l, cudaStream_t st) {
 // kernel that runs supports it (weight = prior weights or null; log_uniform = log w of every row in that case)
 emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, float *L, int ld_out,
                            unsigned flags, cudaStream_t st, const float *weight = nullptr, float log_uniform = 0.f,
-                           bool *stats_ready = nullptr, const GaussTerms *gauss = nullptr) {
+                           bool *stats_ready = nullptr, const GaussTerms *gauss = nullptr, int layout_rot = 0) {
     GemmProblem g;
     g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
     g.M = n_rot; g.N = n_pat; g.K = n_pix;
@@ -149,7 +149,7 @@ emc_status run_loglik_gemm(const Layout &l, int n_rot, int n_pix, int n_pat, flo
     g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
     const bool simt = (flags & EMC_DEBUG_SIMT) != 0;
     if (stats_ready) {
-        const size_t rows = (size_t)normalize_stat_rows(n_rot);
+        const size_t rows = (size_t)normalize_stat_rows(layout_rot > 0 ? layout_rot : n_rot);
         g.stat_m = l.scratch;
         g.stat_w = l.scratch + rows * l.ld_n;
         g.stat_z = l.scratch + 2 * rows * l.ld_n;
@@ -463,6 +463,104 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                        size_t ws_bytes, void *stream, emc_context *ctx) {
     return iterate_impl(model, det, rot, pat, n_iter, n_pat_chunk, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes,
                         stream, ctx, 0.f);
+}
+
+// Rotation chunks: the per-chunk buffers of carve() at R = chunk size, then s for the whole list
+static size_t rot_chunked_extra(int n_rot) { return round_up(sizeof(float) * (size_t)n_rot, 1024); }
+
+size_t emc_workspace_bytes_rot_chunked(int n, int n_pix, int n_rot, int n_rot_chunk, int n_pat) {
+    if (!sizes_ok(n, n_pix, n_rot, n_pat) || n_rot_chunk <= 0) return 0;
+    const int rc = n_rot_chunk < n_rot ? n_rot_chunk : n_rot;
+    return carve(nullptr, n, n_pix, rc, n_pat, 0).total + rot_chunked_extra(n_rot);
+}
+
+emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                                   const emc_patterns *pat, int n_iter, int n_rot_chunk, float *model_out,
+                                   double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
+                                   emc_context *ctx) {
+    if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_iter <= 0 || !model_out ||
+        model_out == model->model || !loglik || n_rot_chunk <= 0)
+        return EMC_ERR_ARG;
+    if (flags & EMC_PATTERNS_ON_HOST) return EMC_ERR_UNSUPPORTED;
+    if ((flags & EMC_PROFILE_STAGES) && !ctx) return EMC_ERR_ARG;
+    if (n_iter > 256) return EMC_ERR_UNSUPPORTED;
+    const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
+    if (!sizes_ok(n, n_pix, n_rot, n_pat)) return EMC_ERR_UNSUPPORTED;
+    const int rc = n_rot_chunk < n_rot ? n_rot_chunk : n_rot;
+    const size_t base_bytes = carve(nullptr, n, n_pix, rc, n_pat, 0).total;
+    EMC_TRY(check_ws(ws, ws_bytes, base_bytes + rot_chunked_extra(n_rot)));
+    const Layout l = carve(ws, n, n_pix, rc, n_pat, 0);
+    float *s_all = (float *)((uint8_t *)ws + base_bytes);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
+    const bool prof = (flags & EMC_PROFILE_STAGES) != 0;
+    const float log_uniform = log_uniform_of(n_rot);                  // log w of every row when weight == NULL
+    const int n_chunks = ceil_div(n_rot, rc);
+
+    EMC_TRY(reset_header(l, st));
+    {
+        Span sp(ctx, prof, EMC_STAGE_PACK, st);
+        EMC_TRY(launch_pack(pat->counts, pat->type, n_pat, n_pix, det->mask, l.Kc, l.ld_p, l.KT, l.ld_n, l.hdr, st));
+    }
+    const float *model_cur = model->model;
+    for (int it = 0; it < n_iter; ++it) {
+        EMC_TRY_CUDA(cudaMemsetAsync(s_all, 0, sizeof(float) * n_rot, st));
+        EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
+        for (int sweep = 1; sweep <= 2; ++sweep) {
+            for (int c = 0; c < n_chunks; ++c) {
+                const int r0 = c * rc, nr = n_rot - r0 < rc ? n_rot - r0 : rc;
+                const emc_rotations sub = {nr, rot->quat + 4 * (size_t)r0, rot->weight ? rot->weight + r0 : nullptr};
+                Geometry geo;
+                {
+                    Span sp(ctx, prof, EMC_STAGE_EXPAND, st);
+                    EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, sub.quat, nr, l.geom, &geo, st));
+                    EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * nr, st));
+                    EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, sub.quat, nr, nullptr, nullptr, l.planesL,
+                                          l.ld_p, l.S, l.blocked, &geo, st, false));
+                }
+                bool stats_ready = false;
+                {
+                    Span sp(ctx, prof, EMC_STAGE_LOGLIK, st);
+                    EMC_TRY(run_loglik_gemm(l, nr, n_pix, n_pat, l.L, l.ld_n, flags, st, sub.weight, log_uniform,
+                                            sweep == 1 ? &stats_ready : nullptr, nullptr, rc));
+                }
+                if (sweep == 1) {
+                    // the chunk's (max, sum) per pattern merged into the running ones; LL with the last chunk
+                    Span sp(ctx, prof, EMC_STAGE_NORMALIZE, st);
+                    EMC_TRY(launch_normalize(l.L, sub.weight, nr, n_pat, l.ld_n, nullptr, nullptr, 0, nullptr, nullptr,
+                                             c == n_chunks - 1 ? loglik + it : nullptr, true, l.scratch, stats_ready, st,
+                                             nullptr, 0, log_uniform, 1, c > 0, rc));
+                    continue;
+                }
+                {
+                    Span sp(ctx, prof, EMC_STAGE_NORMALIZE, st);
+                    EMC_TRY(launch_normalize(l.L, sub.weight, nr, n_pat, l.ld_n, nullptr, l.planesP, (size_t)nr * l.ld_n, l.pscale,
+                                             s_all + r0, nullptr, true, l.scratch, false, st, nullptr, 0, log_uniform, 2,
+                                             false, rc));
+                }
+                {
+                    Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
+                    GemmProblem g;
+                    g.A = l.planesP; g.B = l.KT; g.n_planes = 2;
+                    g.M = nr; g.N = n_pix; g.K = n_pat;
+                    g.lda = l.ld_n; g.ldb = l.ld_n; g.plane_stride = (size_t)nr * l.ld_n;
+                    g.a_fmt = g.b_fmt = FMT_F16;
+                    g.chunk_scale = l.pscale;
+                    g.out = l.Wnum; g.ld_out = n_pix; g.rowv = s_all + r0; g.epilogue = EPI_DIV_ROW;
+                    g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
+                    EMC_TRY(launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st));
+                }
+                {
+                    Span sp(ctx, prof, EMC_STAGE_COMPRESS, st);
+                    const int phases = COMPRESS_SCATTER | (c == 0 ? COMPRESS_CLEAR : 0) | (c == n_chunks - 1 ? COMPRESS_DIVIDE : 0);
+                    EMC_TRY(launch_compress(l.Wnum, s_all + r0, weighted, geo, n, l.acc, model_out, nullptr, st, nullptr,
+                                            phases));
+                }
+            }
+        }
+        model_cur = model_out;
+    }
+    return launch_poison(l.hdr, model_out, (size_t)n * n * n, loglik, n_iter, st);
 }
 
 emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,

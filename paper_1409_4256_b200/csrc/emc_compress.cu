@@ -175,7 +175,7 @@ compress_divide_blocked_kernel(const float *__restrict__ acc, int n, float *__re
 size_t compress_scratch_float2(int n) { return (size_t)8 * n * n * n; }
 
 emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const Geometry &geo, int n,
-                           float2 *acc, float *model_out, float *den_out, cudaStream_t st, const DenCache *cache) {
+                           float2 *acc, float *model_out, float *den_out, cudaStream_t st, const DenCache *cache, int phases) {
     const size_t g = (size_t)n * n * n;
     const int n_pix = geo.n_pix, n_rot = geo.n_rot;
     float4 *acc4 = reinterpret_cast<float4 *>(acc);          // n^3 blocks x 64 B = 8 G float2
@@ -184,6 +184,18 @@ emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighte
     const TileMap tm = make_tile_map(n_pix, geo.row_len);
     const long long items = (long long)n_rot * tm.n_bands;
     const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
+    if (phases != COMPRESS_ALL) {
+        if (phases & COMPRESS_CLEAR) EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * 8 * sizeof(float2), st));
+        if (phases & COMPRESS_SCATTER) {
+            compress_scatter_blocked_kernel<<<grid, kThreads, 0, st>>>(Wnew, slice_w, w, geo.qm, tm, n_rot, n_pix, geo.rotm, n, acc4, nullptr);
+            EMC_LAUNCHED();
+        }
+        if (phases & COMPRESS_DIVIDE) {
+            compress_divide_blocked_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(accf, n, model_out, den_out);
+            EMC_LAUNCHED();
+        }
+        return EMC_OK;
+    }
     if (cache && slice_w && !weighted) {
         // den is reused while the set of skipped slices stays the one it was accumulated for (decided on the device)
         EMC_TRY_CUDA(cudaMemsetAsync(cache->changed, 0, sizeof(int), st));

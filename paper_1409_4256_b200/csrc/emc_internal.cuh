@@ -170,7 +170,14 @@ int normalize_stat_rows(int n_rot);   // scratch = part_m, part_w, part_z [rows]
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, __half *planes, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss = nullptr, int n_store = 0, float log_uniform = 0.f);
+                            cudaStream_t st, const GaussTerms *gauss = nullptr, int n_store = 0, float log_uniform = 0.f,
+                            int chunk_mode = 0, bool carry_in = false, int layout_rot = 0);
+// chunk_mode (rotation chunks): 0 = the rows are the whole rotation list; 1 = first sweep of a
+// chunk: its column statistics are merged into the carried ones (carry_in = false for the first chunk) and nothing else is
+// written (loglik, when given, receives the total of the statistics carried so far: pass it with the last chunk only);
+// 2 = second sweep of a chunk: P / planes / s with the final statistics left by the last mode-1 call.
+// layout_rot: the rotation count the scratch was laid out for (normalize_scratch_floats); 0 = n_rot.  A ragged last chunk
+// passes the full chunk size so that the carried statistics stay where they are.
 // log_uniform: log w of every row when weight == null; 0 = log_uniform_of(n_rot) (set it when the rows are a chunk of a
 // longer rotation list)
 // n_store: columns of a row the call may write (planes padding, column arrays); 0 = ld_n.  Smaller when L, planes and
@@ -191,8 +198,10 @@ struct DenCache {
     int *changed;       // device flag, scratch
     bool force;
 };
+enum { COMPRESS_CLEAR = 1, COMPRESS_SCATTER = 2, COMPRESS_DIVIDE = 4, COMPRESS_ALL = 7 };
 emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const Geometry &geo, int n,
                            float2 *acc, float *model_out, float *den_out, cudaStream_t st,
-                           const DenCache *cache = nullptr);
+                           const DenCache *cache = nullptr, int phases = COMPRESS_ALL);
+// phases: rotation chunks scatter into the same accumulators (CLEAR with the first, DIVIDE with the last; no cache)
 
 }  // namespace emc

@@ -208,10 +208,10 @@ __device__ __forceinline__ void write_planes(float (&p)[kGroups][4], int d0, int
 // log-likelihood  LL = sum_d (m_d + log z_d).  block = 32 columns x 8 row lanes; row lane y merges the
 // partials k = y, y + 8, ... online, then the 8 are merged through shared memory.
 __global__ void __launch_bounds__(256)
-colstats_combine_kernel(const float *__restrict__ part_m, const float *__restrict__ part_w,
-                        const float *__restrict__ part_z, int n_pat, int ld_n, int n_store, int n_splits,
+colstats_combine_kernel(float *__restrict__ part_m, float *__restrict__ part_w,
+                        float *__restrict__ part_z, int n_pat, int ld_n, int n_store, int n_splits,
                         float *__restrict__ col_m, float *__restrict__ col_w, float *__restrict__ col_iz,
-                        double *__restrict__ loglik) {
+                        double *__restrict__ loglik, int carry_row, int carry_in) {
     __shared__ float sm_m[8][32], sm_w[8][32], sm_z[8][32];
     const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
     const int d = blockIdx.x * 32 + x;
@@ -238,6 +238,15 @@ colstats_combine_kernel(const float *__restrict__ part_m, const float *__restric
     if (d < n_pat) {
 #pragma unroll
         for (int k = 1; k < 8; ++k) merge(t, ColStat{sm_m[k][x], sm_w[k][x], sm_z[k][x]});
+        // rotation chunks: row `carry_row` of the partial arrays holds the statistics of the chunks seen
+        // so far; merge them in and hand the result on
+        if (carry_row >= 0) {
+            const size_t o = (size_t)carry_row * ld_n + d;
+            if (carry_in) merge(t, ColStat{part_m[o], part_w[o], part_z[o]});
+            part_m[o] = t.mL;
+            part_w[o] = t.mw;
+            part_z[o] = t.z;
+        }
         col_m[d] = t.mL;
         col_w[d] = t.mw;
         col_iz[d] = 1.f / t.z;
@@ -450,7 +459,7 @@ div_rows_kernel(float *__restrict__ Wn, const float *__restrict__ s, int n_pix) 
 // (emc_gemm.cu store_row_and_col_stats) one per 32 rotations
 int normalize_stat_rows(int n_rot) {
     const int fused = ceil_div(n_rot, 32);
-    return fused > 64 ? fused : 64;
+    return (fused > 64 ? fused : 64) + 1;              // + the carry row of rotation chunks
 }
 
 size_t normalize_scratch_floats(int n_rot, int ld_n) {
@@ -460,18 +469,22 @@ size_t normalize_scratch_floats(int n_rot, int ld_n) {
 emc_status launch_normalize(const float *L, const float *weight, int n_rot, int n_pat, int ld_n,
                             float *P, __half *planes, size_t plane_stride, float *chunk_inv_scale,
                             float *s, double *loglik, bool accumulate, float *scratch, bool stats_ready,
-                            cudaStream_t st, const GaussTerms *gauss, int n_store, float log_uniform) {
+                            cudaStream_t st, const GaussTerms *gauss, int n_store, float log_uniform, int chunk_mode,
+                            bool carry_in, int layout_rot) {
     if (n_store <= 0 || n_store > ld_n) n_store = ld_n;          // columns of a row this call may write
     if (log_uniform == 0.f) log_uniform = log_uniform_of(n_rot);
     if (gauss && !stats_ready) return EMC_ERR_UNSUPPORTED;       // the Gaussian model's statistics come from the GEMM
-    const int stat_rows = normalize_stat_rows(n_rot);
+    const int stat_rows = normalize_stat_rows(layout_rot > 0 ? layout_rot : n_rot);
     float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
     if (!accumulate) {
         if (s) EMC_TRY_CUDA(cudaMemsetAsync(s, 0, sizeof(float) * n_rot, st));
         if (loglik) EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
     }
-    int n_splits;
-    if (stats_ready) {
+    float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
+    int n_splits = 0;
+    if (chunk_mode == 2) {
+        // second sweep of a rotation chunk: the final column statistics are in place
+    } else if (stats_ready) {
         n_splits = ceil_div(n_rot, 32);               // written by the log-likelihood GEMM's epilogue
     } else {
         const int col_blocks = ceil_div(n_pat, kColsPerBlock);
@@ -482,10 +495,13 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
                                                                          rows_per_split, part_m, part_w, part_z);
         EMC_LAUNCHED();
     }
-    float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
-    colstats_combine_kernel<<<ceil_div(n_store, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_store, n_splits, col_m,
-                                                                 col_w, col_iz, loglik);
-    EMC_LAUNCHED();
+    if (chunk_mode != 2) {
+        colstats_combine_kernel<<<ceil_div(n_store, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, n_store, n_splits, col_m,
+                                                                     col_w, col_iz, chunk_mode == 2 ? nullptr : loglik,
+                                                                     chunk_mode == 1 ? stat_rows - 1 : -1, carry_in ? 1 : 0);
+        EMC_LAUNCHED();
+    }
+    if (chunk_mode == 1) return EMC_OK;                 // first sweep of a rotation chunk: statistics only
     // second sweep: 512-column chunks; row splits so that the grid is at most 6 x 148 blocks = whole waves of the 2 or 3
     // blocks per SM the kernels run at (one block more is a wave more: a quarter of the time at C2)
     const int chunks = ceil_div(n_pat, kChunkCols);

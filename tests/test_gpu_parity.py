@@ -342,3 +342,45 @@ def test_den_reuse_across_iterations(inputs_cache, name):
     rel = np.abs(ma - mo.reshape(-1))[cov] / (np.abs(mo.reshape(-1)[cov]) + 1e-6 * np.abs(mo).max())
     assert np.median(rel) <= 1e-3, np.median(rel)
     assert np.array_equal(ma[ref["den"] == 0] == 0, np.ones(int((ref["den"] == 0).sum()), bool))
+
+
+# ---------------------------------------------------------------------------------------------- rotation chunks (NEXT-2)
+
+@pytest.mark.parametrize("name,chunk,weighted,null_w", [("T1", 64, False, False), ("T1", 100, True, True), ("T2", 128, True, False),
+                                                        ("T2", 333, False, False), ("T3", 40, False, True), ("C1", 200, False, False)])
+def test_iterate_rot_chunked_matches_oracle(inputs_cache, name, chunk, weighted, null_w):
+    """emc_iterate_rot_chunked against the oracle's streamed iteration and against the GPU's own
+    unchunked emc_iterate: LL, and model' on the covered voxels, for ragged last chunks, one chunk, NULL weights."""
+    inp = inputs_cache(name)
+    c = Case(inp, stage=len(inp.quat) - 1)
+    n_rot = c.quat.shape[0]
+    w = np.full(n_rot, 1.0 / n_rot, np.float32) if null_w else c.weight
+    ref = o.iterate_rotation_chunks(inp.model_init, inp.q, inp.mask, c.quat, w, inp.counts, chunk, weighted=weighted)
+    flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
+    out = emc.emc_iterate_rot_chunked(c.d_model, c.d_q, c.d_mask, c.d_quat, None if null_w else c.d_weight, c.d_counts, chunk,
+                                      flags=flags)
+    emc.emc_check(out["ws"])
+    one = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, None if null_w else c.d_weight, c.d_counts, flags=flags)
+    ll = float(host(out["loglik"])[0])
+    assert abs(ll - ref["LL"]) <= 1e-5 * abs(ref["LL"])
+    assert abs(ll - float(host(one["loglik"])[0])) <= 1e-6 * abs(ll)
+    m, m1, m_ref = host(out["model"]).reshape(-1), host(one["model"]).reshape(-1), ref["model"].reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    scale = np.abs(m_ref).max()
+    rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
+    rel1 = np.abs(m - m1)[cov] / (np.abs(m1[cov]) + 1e-6 * scale)
+    # end to end: the same gates as test_iterate_end_to_end (P amplifies the float32 rounding of L, DESIGN.md section 4)
+    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2, (np.median(rel), rel.max())
+    assert np.median(rel1) <= 1e-5 and rel1.max() <= 2e-2, (np.median(rel1), rel1.max())
+    assert np.array_equal(m == 0, m1 == 0)
+
+
+def test_iterate_rot_chunked_two_iterations(inputs_cache):
+    inp = inputs_cache("T1")
+    c = Case(inp)
+    a = emc.emc_iterate_rot_chunked(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, 96, n_iter=2)
+    b = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=2)
+    assert np.allclose(host(a["loglik"]), host(b["loglik"]), rtol=2e-6)
+    ma, mb = host(a["model"]).reshape(-1), host(b["model"]).reshape(-1)
+    big = np.abs(mb) >= 1e-3 * np.abs(mb).max()
+    assert np.median(np.abs(ma - mb)[big] / np.abs(mb)[big]) <= 1e-5
