@@ -295,6 +295,46 @@ def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=Fal
 
 
 # ----------------------------------------------------------------------------------------------
+# Photon-list form of stages 2 and 4 for sparse frames (BASELINE.json config 4: > 99 % of the pixels hold no
+# photon; DESIGN.md section 11 NEXT-2).  Same sums as `loglik` / `update`, taken over the photons only.
+# ----------------------------------------------------------------------------------------------
+
+def photon_lists(counts, mask):
+    """Per pattern d the list of (pixel p, count K[d,p]) over unmasked pixels with K[d,p] > 0."""
+    counts = np.asarray(counts)
+    use = _use(mask, counts.shape[1])
+    out = []
+    for row in counts:
+        px = np.nonzero((row > 0) & use)[0]
+        out.append((px, row[px].astype(np.float64)))
+    return out
+
+
+def loglik_photon_list(w, idx, lists, mask):
+    """L[r,d] = sum_{(p,c) in list d} c logW[r,p] - sum_{p: mask} W[r,p]   (the zero pixels of a frame only
+    contribute -W[r,p], which is the same for every frame).  Returns L float64 [R,N]."""
+    use = _use(mask, np.asarray(w).shape[1])
+    lw = log_slices(w, idx)
+    s = np.asarray(w, dtype=np.float32).astype(np.float64)[:, use].sum(axis=1)
+    big_l = np.empty((lw.shape[0], len(lists)))
+    for d, (px, c) in enumerate(lists):
+        big_l[:, d] = lw[:, px] @ c - s
+    return big_l
+
+
+def update_photon_list(p, lists, n_pix):
+    """W'[r,p] = sum_d P[r,d] K[d,p] / sum_d P[r,d], the numerator scattered photon by photon (eq. 2.11)."""
+    pd = np.asarray(p).astype(np.float64)
+    num = np.zeros((pd.shape[0], n_pix))
+    for d, (px, c) in enumerate(lists):
+        num[:, px] += pd[:, d:d + 1] * c[None, :]
+    s = pd.sum(axis=1)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        wn = np.where(s[:, None] > 0, num / s[:, None], 0.0)
+    return wn.astype(np.float32), s
+
+
+# ----------------------------------------------------------------------------------------------
 # Rotation chunks (the paper's own streaming, PAPER.md:164-166 "chunk C_c", 203; DESIGN.md section 11 NEXT-2)
 # ----------------------------------------------------------------------------------------------
 

@@ -489,3 +489,24 @@ def test_iterate_rotation_chunks_equals_iterate(inputs_cache, chunk, weighted):
     ma, mb = a["model"].reshape(-1)[cov], b["model"].reshape(-1)[cov]
     assert np.abs(mb - ma).max() <= 2e-6 * np.abs(ma).max()
     assert np.array_equal(a["den"] > 0, b["den"] > 0)
+
+
+# ---------------------------------------------------------------------------------------------- photon lists (NEXT-2)
+
+def test_photon_list_forms_equal_the_dense_definitions(inputs_cache):
+    """Stages 2 and 4 summed over the photons only are the dense sums (the zero pixels of a frame contribute -W[r,p] to L,
+    nothing to the update); masked counts (sentinels) never enter a list."""
+    inp = inputs_cache("T1")
+    w, idx = o.expand(inp.model_init, inp.q, inp.quat[0])
+    lists = o.photon_lists(inp.counts, inp.mask)
+    use = inp.mask.astype(bool)
+    assert all(use[px].all() and (c > 0).all() for px, c in lists)
+    assert sum(len(px) for px, _ in lists) == int(((inp.counts > 0) & use[None, :]).sum())
+    big_l, big_a = o.loglik(w, idx, inp.counts, inp.mask)
+    l_sparse = o.loglik_photon_list(w, idx, lists, inp.mask)
+    assert np.abs(l_sparse - big_l).max() <= 1e-12 * big_a.max()
+    p, _, _ = o.normalize(big_l.astype(np.float32), inp.weight[0])
+    wn, s = o.update(p.astype(np.float32), inp.counts, inp.mask)
+    wn2, s2 = o.update_photon_list(p.astype(np.float32), lists, inp.counts.shape[1])
+    assert np.array_equal(s, s2)
+    assert np.abs(wn2 - wn).max() <= 1e-6 * np.abs(wn).max() and np.all(wn2[:, ~use] == 0)
