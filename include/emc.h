@@ -77,6 +77,11 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
                                       do not divide by s[r] */
 #define EMC_PROFILE_STAGES    0x20u /* emc_iterate records the context's CUDA events on `stream` around every
                                       stage; read (and reset) the sums with emc_profile_read() */
+#define EMC_SPARSE_PHOTONS    0x40u /* emc_iterate (Poisson model): stages 2 and 4 from per-frame / per-pixel photon lists on
+                                      plain CUDA cores instead of the dense tensor-core contractions; for frames that
+                                      are almost empty (DESIGN.md section 11 NEXT-2 has the measured crossover).  Needs
+                                      n_pix and the pattern chunk below 2^20; the workspace grows (pass the flag to
+                                      emc_workspace_bytes). */
 #define EMC_GEMM_1CTA         0x200u /* run the two contractions with one CTA per tile (cta_group::1)
                                         instead of CTA pairs (cta_group::2); a comparison / bisecting aid */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a

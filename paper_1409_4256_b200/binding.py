@@ -23,6 +23,7 @@ EMC_ACCUMULATE = 0x2
 EMC_UPDATE_RAW = 0x4
 EMC_PATTERNS_ON_HOST = 0x10
 EMC_PROFILE_STAGES = 0x20
+EMC_SPARSE_PHOTONS = 0x40
 EMC_DEBUG_SIMT = 0x100
 EMC_GEMM_1CTA = 0x200
 EMC_MAX_SPANS = 4096

@@ -17,7 +17,7 @@ import sys
 PKG = pathlib.Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libemc.so"
-SOURCES = ["emc_api.cu", "emc_expand.cu", "emc_pack.cu", "emc_gemm.cu", "emc_normalize.cu", "emc_compress.cu"]
+SOURCES = ["emc_api.cu", "emc_expand.cu", "emc_pack.cu", "emc_gemm.cu", "emc_normalize.cu", "emc_compress.cu", "emc_sparse.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--cudart=static", "-Xcompiler", "-fPIC,-fvisibility=hidden", "-Xptxas", "-v",

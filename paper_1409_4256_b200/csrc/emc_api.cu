@@ -76,11 +76,16 @@ struct Layout {
     float *Asq;               // [2][ld_n]     1 / (2 sigma^2 A_d) and 1 / A_d, A_d = sum_p K^2 (Gaussian model)
     uint32_t *active;         // [R/32 + 1]    slices den was accumulated for (+ the device flag), Compress
     void *stage;              // two chunks of raw counts (patterns on host, double-buffered)
-    int ld_p, ld_n;
+    // photon-list path (EMC_SPARSE_PHOTONS): everything with the rotations along the rows (pitch ld_r)
+    float *logWT;             // [P][ld_r]     log W transposed
+    float *LT;                // [Nc][ld_r]    L transposed, then P transposed
+    float *WT;                // [P][ld_r]     update numerators transposed
+    int *list_pat, *list_pix; // photon lists by frame and by pixel (sparse_list_ints)
+    int ld_p, ld_n, ld_r;
     size_t total;
 };
 
-Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_bytes) {
+Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_bytes, bool sparse = false) {
     Layout l;
     l.ld_p = (int)round_up((size_t)n_pix, 64);
     l.ld_n = (int)round_up((size_t)n_chunk, 64);
@@ -103,6 +108,18 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
     l.Asq = a.take<float>((size_t)2 * l.ld_n);
     l.active = a.take<uint32_t>((size_t)ceil_div(n_rot, 32) + 1);
     l.stage = a.take<uint8_t>(stage_bytes);
+    l.ld_r = (int)round_up((size_t)n_rot, 32);
+    if (sparse) {
+        const size_t cap = (size_t)n_chunk * n_pix;             // every count non-zero: the lists cannot overflow
+        l.logWT = a.take<float>((size_t)n_pix * l.ld_r);
+        l.LT = a.take<float>((size_t)n_chunk * l.ld_r);
+        l.WT = a.take<float>((size_t)n_pix * l.ld_r);
+        l.list_pat = a.take<int>(sparse_list_ints(n_chunk, cap));
+        l.list_pix = a.take<int>(sparse_list_ints(n_pix, cap));
+    } else {
+        l.logWT = l.LT = l.WT = nullptr;
+        l.list_pat = l.list_pix = nullptr;
+    }
     l.total = a.off;
     return l;
 }
@@ -219,7 +236,7 @@ emc_status emc_context_destroy(emc_context *c) {
 size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags) {
     if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return 0;
     const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? 2 * round_up((size_t)n_pat_chunk * n_pix * 4, 1024) : 0;
-    return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage).total;
+    return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage, (flags & EMC_SPARSE_PHOTONS) != 0).total;
 }
 
 size_t emc_workspace_bytes_geometry(int n, int n_pix, int n_rot) {
@@ -328,8 +345,11 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     const size_t csz = count_size(pat->type);
     const size_t stage_one = round_up((size_t)chunk * n_pix * 4, 1024);          // one staging buffer (4 B per count at most)
     const size_t stage_bytes = on_host ? 2 * stage_one : 0;
-    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes).total));
-    const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes);
+    const bool sparse = (flags & EMC_SPARSE_PHOTONS) != 0;
+    if (sparse && (gauss || n_pix >= (1 << 20) || chunk >= (1 << 20) || (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT))))
+        return EMC_ERR_UNSUPPORTED;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes, sparse).total));
+    const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes, sparse);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
     if (gauss && (n_chunks != 1 || (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
     const float log_uniform = log_uniform_of(n_rot);
@@ -344,7 +364,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     // copy of sub-range j + 1 crosses PCIe while sub-range j is packed (into its place in the full-size operands)
     // and goes through stages 2-4; later iterations use the resident operands in one piece.  Same arithmetic as
     // pattern chunks (G9).  Sub-ranges are multiples of 512 patterns (the update's K chunk and scale granularity).
-    const bool pipelined = on_host && n_chunks == 1 && !gauss && n_pat >= 4096;
+    const bool pipelined = on_host && n_chunks == 1 && !gauss && !sparse && n_pat >= 4096;
     const int sub = pipelined ? (int)round_up((size_t)ceil_div(n_pat, 4), 512) : chunk;
     const int n_sub = pipelined ? ceil_div(n_pat, sub) : 1;
     // pack jobs in order: every (iteration, chunk) when there are several chunks, else the resident chunk once
@@ -371,6 +391,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         EMC_TRY(issue_copy(0));
     }
     int job = 0;
+    SparseList by_frame = {nullptr, nullptr, 0}, by_pixel = {nullptr, nullptr, 0};
     const float *model_cur = model->model;
     Geometry geo;                                            // once per call: the rotation list is the same in every iteration
     EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, rot->quat, n_rot, l.geom, &geo, st));
@@ -379,8 +400,15 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
         {
             Span sp(ctx, prof, EMC_STAGE_EXPAND, st);
             EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
-            EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                                  l.planesL, l.ld_p, l.S, l.blocked, &geo, st, gauss));
+            if (sparse) {
+                // log W as float32 (into the W' buffer, free until the update), transposed: rotations along the rows
+                EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, l.Wnum, nullptr, nullptr, 0,
+                                      l.S, l.blocked, &geo, st, false, true));
+                EMC_TRY(launch_transpose(l.Wnum, n_rot, n_pix, n_pix, l.logWT, l.ld_r, st));
+            } else {
+                EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
+                                      l.planesL, l.ld_p, l.S, l.blocked, &geo, st, gauss));
+            }
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
         EMC_TRY_CUDA(cudaMemsetAsync(loglik + it, 0, sizeof(double), st));
@@ -412,11 +440,36 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                 }
                 EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, l.ld_n, l.hdr, st));
                 if (on_host) EMC_TRY_CUDA(cudaEventRecord(ctx->freed[job & 1], st));
+                if (sparse) {                       // photon lists by frame (rows of Kc) and by pixel (rows of KT)
+                    const size_t cap = (size_t)chunk * n_pix;
+                    EMC_TRY(launch_sparsify(v.Kc, nc, n_pix, l.ld_p, l.list_pat, cap, &by_frame, st));
+                    EMC_TRY(launch_sparsify(v.KT, n_pix, nc, l.ld_n, l.list_pix, cap, &by_pixel, st));
+                }
                 if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
                     EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * 2 * l.ld_n, st));
                     EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, gterms.inv2s2, l.Asq, l.Asq + l.ld_n, st));
                 }
                 ++job;
+            }
+            if (sparse) {
+                // stages 2-4 from the photon lists, in the transposed world (emc_sparse.cu)
+                float *p_buf = (P_out && it == n_iter - 1) ? P_out : reinterpret_cast<float *>(l.planesP);   // [R][ld_n] float32
+                {
+                    Span sp(ctx, prof, EMC_STAGE_LOGLIK, st);
+                    EMC_TRY(launch_spmm_rot(by_frame, l.logWT, l.LT, l.ld_r, n_rot, l.S, false, st));
+                    EMC_TRY(launch_transpose(l.LT, nc, n_rot, l.ld_r, l.L, l.ld_n, st));
+                }
+                {
+                    Span sp(ctx, prof, EMC_STAGE_NORMALIZE, st);
+                    EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_buf, nullptr, 0, nullptr, l.s, loglik + it, true,
+                                             l.scratch, false, st, nullptr, 0, log_uniform));
+                }
+                {
+                    Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
+                    EMC_TRY(launch_transpose(p_buf, n_rot, nc, l.ld_n, l.LT, l.ld_r, st));
+                    EMC_TRY(launch_spmm_rot(by_pixel, l.LT, l.WT, l.ld_r, n_rot, nullptr, c > 0, st));
+                }
+                continue;
             }
             // stage 2: L = logW K^T - S  (+ the column max / sum-exp partials of stage 3 from the same epilogue)
             bool stats_ready = false;
@@ -439,7 +492,10 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                 EMC_TRY(run_update_gemm(v, n_rot, n_pix, nc, l.Wnum, l.s, epi, flags, st));
             }
         }
-        if (n_parts > 1) {
+        if (sparse) {
+            Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
+            EMC_TRY(launch_transpose_div(l.WT, n_pix, n_rot, l.ld_r, l.Wnum, l.s, st));      // W' = numerator / s[r] (eq. 2.5)
+        } else if (n_parts > 1) {
             Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
             EMC_TRY(launch_div_rows(l.Wnum, l.s, n_rot, n_pix, st));
         }

@@ -153,7 +153,8 @@ geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, i
 // S_part [R][n_bands]: sum_{p:mask} W (or W^2) of each band, summed per rotation in a fixed order by rowsum_kernel
 // (bitwise reproducible S, no atomics).
 constexpr int kWarps = kThreads / 32;
-template <bool W_OUT, bool IDX_OUT, bool PLANES>
+// LOGW32 (photon-list path): W receives log W as float32 (0 for masked / outside samples) and S the row sums
+template <bool W_OUT, bool IDX_OUT, bool PLANES, bool LOGW32 = false>
 __global__ void __launch_bounds__(kThreads, 4)
 expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, const TileMap tm,
                       const float4 *__restrict__ rotm, int n_rot, int n_pix, float *__restrict__ W, int32_t *__restrict__ idx,
@@ -165,7 +166,7 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
         float rm[9];
         load_rotation(rotm, r, rm);
         const Band band(tm, item - r * tm.n_bands, lane);
-        float *const w_row = W_OUT ? W + (size_t)r * n_pix : nullptr;
+        float *const w_row = (W_OUT || LOGW32) ? W + (size_t)r * n_pix : nullptr;
         int32_t *const i_row = IDX_OUT ? idx + (size_t)r * n_pix : nullptr;
         __half *const hi_row = PLANES ? planes + (size_t)r * ld_p : nullptr;
         __half *const lo_row = PLANES ? hi_row + plane_stride : nullptr;
@@ -198,9 +199,14 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
                 const float c11 = hi4[j].z * z0 + hi4[j].w * tz;
                 float w = (c00 * y0 + c01 * ty) * x0 + (c10 * y0 + c11 * ty) * tx;
                 w = inside ? w : 0.f;
-                if (W_OUT && in) w_row[pc] = w;
-                if (IDX_OUT && in) i_row[pc] = s[j].base;
                 const bool use = in && g[j].w != 0.f;
+                if (LOGW32) {
+                    const float lw = (use && inside) ? __logf(fmaxf(w, 1e-30f)) : 0.f;
+                    if (in) w_row[pc] = lw;
+                } else if (W_OUT && in) {
+                    w_row[pc] = w;
+                }
+                if (IDX_OUT && in) i_row[pc] = s[j].base;
                 if (PLANES) {
                     __half hi, lo;
                     split_logw<true>(w, use && inside, hi, lo, gauss);
@@ -212,7 +218,7 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
                 part += use ? (gauss ? w * w : w) : 0.f;
             }
         }
-        if (PLANES) {                                        // S accompanies the planes (log-likelihood operands)
+        if (PLANES || LOGW32) {                              // S accompanies the log-likelihood operands
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
             if (lane == 0) S_part[item] = part;
@@ -279,7 +285,7 @@ size_t expand_scratch_floats(int n, int n_pix, int n_rot) {
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss) {
+                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss, bool logw32) {
     const int g = gauss ? 1 : 0;
     if (planes && !S) return EMC_ERR_ARG;
     if (blocked && geo) {
@@ -299,13 +305,18 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         switch (sel) {
             case 1: EMC_EXPAND_CASE(false, false, true); break;
             case 2: EMC_EXPAND_CASE(false, true, false); break;
-            case 4: EMC_EXPAND_CASE(true, false, false); break;
+            case 4:
+                if (logw32)                                      // log W and S out instead of W
+                    expand_blocked_kernel<false, false, false, true><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g);
+                else
+                    EMC_EXPAND_CASE(true, false, false);
+                break;
             case 6: EMC_EXPAND_CASE(true, true, false); break;
             default: return EMC_ERR_ARG;                         // no caller asks for slices and operand planes at once
         }
 #undef EMC_EXPAND_CASE
         EMC_LAUNCHED();
-        if (planes) {
+        if (planes || logw32) {
             rowsum_kernel<<<ceil_div(n_rot, 8), 256, 0, st>>>(S_part, n_rot, tm.n_bands, S);
             EMC_LAUNCHED();
         }

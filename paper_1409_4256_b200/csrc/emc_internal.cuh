@@ -84,7 +84,10 @@ emc_status launch_geometry(const float *q, const uint8_t *mask, int n_pix, int r
 size_t expand_scratch_floats(int n, int n_pix, int n_rot);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss = false);
+                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss = false,
+                         bool logw32 = false);
+// logw32 (blocked path, W given, no idx / planes): W receives log(max(W, 1e-30)) as float32, 0 for masked / outside samples, and
+// S the row sums (operands of the photon-list log-likelihood, emc_sparse.cu)
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
                              int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
@@ -187,6 +190,26 @@ emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);
 // rows of Wnew divided by s[r] (after the last pattern chunk).
 emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cudaStream_t st);
+
+// Photon lists and the sparse form of stages 2 and 4 (emc_sparse.cu, EMC_SPARSE_PHOTONS)
+struct SparseList {
+    const int *row_ptr;          // [rows + 1]
+    const uint32_t *entries;     // column | count << 20, in row order
+    int rows;
+};
+size_t sparse_list_ints(int rows, size_t max_entries);   // ints of scratch behind a SparseList
+// CSR of the nonzeros of A [rows][ld] fp16 (cols < 2^20)
+emc_status launch_sparsify(const __half *A, int rows, int cols, int ld, int *lists, size_t max_entries, SparseList *out,
+                           cudaStream_t st);
+// Y [rows][ld] = A X (- sub_row) (+ Y), X [K][ld], the first n_rot columns
+emc_status launch_spmm_rot(const SparseList &a, const float *X, float *Y, int ld, int n_rot, const float *sub_row,
+                           bool accumulate, cudaStream_t st);
+emc_status launch_transpose(const float *in, int rows, int cols, int ld_in, float *out, int ld_out, cudaStream_t st);
+// logW^T [P][ld_r] from W [R][P] (0 for masked / outside samples) and S[r] += sum_{p:mask} W
+emc_status launch_logw_transposed(const float *W, const int32_t *idx, const uint8_t *mask, int n_rot, int n_pix, float *logWT,
+                                  int ld_r, float *S, cudaStream_t st);
+// W' [R][P] = (W'^T [P][ld_r])^T / s[r]
+emc_status launch_transpose_div(const float *WT, int n_pix, int n_rot, int ld_r, float *Wnew, const float *s, cudaStream_t st);
 
 // Compress (emc_compress.cu).  acc = compress_scratch_float2(n) float2 of scratch (one 64-byte (num, den) corner
 // block per base corner), zeroed inside.

@@ -384,3 +384,57 @@ def test_iterate_rot_chunked_two_iterations(inputs_cache):
     ma, mb = host(a["model"]).reshape(-1), host(b["model"]).reshape(-1)
     big = np.abs(mb) >= 1e-3 * np.abs(mb).max()
     assert np.median(np.abs(ma - mb)[big] / np.abs(mb)[big]) <= 1e-5
+
+
+# ---------------------------------------------------------------------------------------------- photon lists (NEXT-2)
+
+@pytest.mark.parametrize("name,chunk,weighted,n_iter", [("T1", 0, False, 1), ("T1", 50, True, 1), ("T2", 200, False, 2), ("T3", 0, True, 1),
+                                                        ("C1", 0, False, 1), ("C1", 300, False, 2)])
+def test_iterate_sparse_photons_matches_oracle(inputs_cache, name, chunk, weighted, n_iter):
+    """EMC_SPARSE_PHOTONS: stages 2 and 4 from photon lists (emc_sparse.cu) against the oracle (whose photon-list forms are
+    pinned to the dense definitions) with the end-to-end gates of test_iterate_end_to_end, and against the dense
+    tensor-core path of the same library."""
+    inp = inputs_cache(name)
+    c = Case(inp, stage=len(inp.quat) - 1)
+    flags = (emc.EMC_COMPRESS_WEIGHTED if weighted else 0)
+    mo, ref = inp.model_init, None
+    for _ in range(n_iter):
+        ref = o.iterate(mo, inp.q, inp.mask, c.quat, c.weight, inp.counts, n_pat_chunk=chunk or None, weighted=weighted)
+        mo = ref["model"]
+    want_p = chunk == 0
+    out = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=n_iter, n_pat_chunk=chunk,
+                          flags=flags | emc.EMC_SPARSE_PHOTONS, want_p=want_p)
+    emc.emc_check(out["ws"])
+    dense = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_iter=n_iter, n_pat_chunk=chunk,
+                            flags=flags, want_p=want_p)
+    ll = host(out["loglik"])
+    assert abs(ll[-1] - ref["LL"]) <= (1e-5 if n_iter == 1 else 1e-4) * abs(ref["LL"])
+    assert np.allclose(ll, host(dense["loglik"]), rtol=1e-5 if n_iter == 1 else 1e-4)   # LL is a sum of terms that largely cancel
+    if want_p and n_iter == 1:
+        l_gpu = gpu_loglik(c)
+        p = host(out["P"])
+        assert np.all(np.abs(p - ref["P"]) <= 2 * p_bound(ref["P"], l_gpu, ref["L"]))
+        assert np.abs(p.sum(axis=0) - 1).max() <= 1e-5
+    m, md, m_ref = host(out["model"]).reshape(-1), host(dense["model"]).reshape(-1), ref["model"].reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    scale = np.abs(m_ref).max()
+    rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
+    reld = np.abs(m - md)[cov] / (np.abs(md[cov]) + 1e-6 * scale)
+    lim = (1e-4, 5e-2) if n_iter == 1 else (1e-3, 0.5)
+    assert np.median(rel) <= lim[0] and rel.max() <= lim[1], (np.median(rel), rel.max())
+    assert np.median(reld) <= lim[0] and reld.max() <= lim[1], (np.median(reld), reld.max())
+    # a voxel that is exactly 0 on one side (responsibilities below 2^-40 of their chunk's maximum vanish from the dense
+    # path's fp16 operand planes, DESIGN.md section 6) is at most a rounding error of the largest voxel on the other
+    assert np.abs(m - md)[(m == 0) | (md == 0)].max(initial=0.0) <= 1e-7 * scale
+
+
+def test_iterate_sparse_photons_host_patterns(inputs_cache):
+    inp = inputs_cache("T2")
+    c = Case(inp, stage=1)
+    pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
+    a = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, pinned, n_pat_chunk=200,
+                        flags=emc.EMC_SPARSE_PHOTONS | emc.EMC_PATTERNS_ON_HOST)
+    b = emc.emc_iterate(c.d_model, c.d_q, c.d_mask, c.d_quat, c.d_weight, c.d_counts, n_pat_chunk=200, flags=emc.EMC_SPARSE_PHOTONS)
+    emc.emc_check(a["ws"])
+    assert np.allclose(host(a["loglik"]), host(b["loglik"]), rtol=1e-7)
+    assert np.abs(host(a["model"]) - host(b["model"])).max() <= 1e-5 * np.abs(host(b["model"])).max()
