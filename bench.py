@@ -58,6 +58,12 @@ def parse():
                          "instead of the Poisson path; not the BASELINE.json metric, no cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-comparator", action="store_true", help="skip the cuBLAS fp16 GEMM on the same operands")
+    ap.add_argument("--sparse", action="store_true",
+                    help="side measurement: stages 2 and 4 from photon lists (EMC_SPARSE_PHOTONS) instead of the dense contractions")
+    ap.add_argument("--rot-chunk", type=int, default=0,
+                    help="side measurement: emc_iterate_rot_chunked with this many rotations per chunk (one pattern chunk)")
+    ap.add_argument("--photons", type=float, default=0.0, help="override the config's mean photons per pixel (density sweeps)")
+    ap.add_argument("--n-pat", type=int, default=0, help="override the config's pattern count (side measurements)")
     return ap.parse_args()
 
 
@@ -303,7 +309,13 @@ def main():
 
     from emc_inputs import CONFIGS, make_inputs
 
+    import dataclasses
+
     cfg = CONFIGS[args.config]
+    if args.photons > 0:
+        cfg = dataclasses.replace(cfg, mean_photons=args.photons)
+    if args.n_pat > 0:
+        cfg = dataclasses.replace(cfg, n_pat=args.n_pat, n_pat_chunk=min(cfg.n_pat_chunk, args.n_pat))
     inp = make_inputs(cfg)                                   # every rank: an independent replica
 
     import torch
@@ -333,9 +345,14 @@ def main():
         else:
             plan.append([dev(inp.quat[s]), None if args.null_weights else dev(inp.weight[s]), 1, inp.quat[s], inp.weight[s]])
     flags = emc.EMC_COMPRESS_WEIGHTED if args.weighted else 0
+    if args.sparse:
+        flags |= emc.EMC_SPARSE_PHOTONS
     chunk = cfg.n_pat_chunk if cfg.n_pat_chunk < cfg.n_pat else 0
-    ws_bytes = max(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, r, cfg.n_pat_chunk, emc.EMC_PATTERNS_ON_HOST)
+    ws_bytes = max(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, r, cfg.n_pat_chunk, emc.EMC_PATTERNS_ON_HOST | flags)
                    for r in cfg.n_rot)
+    if args.rot_chunk > 0:
+        ws_bytes = max(ws_bytes, max(emc.load().emc_workspace_bytes_rot_chunked(cfg.n, cfg.n_pix, r, args.rot_chunk, cfg.n_pat)
+                                     for r in cfg.n_rot))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
     ctx = emc.EmcContext()                                   # copy stream + timing events, created outside the hot path
     d_ll = torch.zeros(cfg.n_iter, dtype=torch.float64, device="cuda")
@@ -348,6 +365,12 @@ def main():
             if args.gaussian_sigma > 0:
                 out = emc.emc_iterate_gaussian(src, d_q, d_mask, quat, wgt, d_counts, args.gaussian_sigma, n_iter=n_it,
                                                flags=f | emc.EMC_COMPRESS_WEIGHTED, ws=ws, ctx=ctx)
+                d_ll[it0:it0 + n_it] = out["loglik"]
+                src, it0 = out["model"], it0 + n_it
+                continue
+            if args.rot_chunk > 0:
+                out = emc.emc_iterate_rot_chunked(src, d_q, d_mask, quat, wgt, d_counts, args.rot_chunk, n_iter=n_it, flags=f,
+                                                  ws=ws, ctx=ctx)
                 d_ll[it0:it0 + n_it] = out["loglik"]
                 src, it0 = out["model"], it0 + n_it
                 continue
@@ -381,10 +404,13 @@ def main():
     prof = emc.emc_profile_read(ctx)
     ms, value = whole_job(ms, args.steps * cfg.n_iter, world, "cuda")
 
-    if args.gaussian_sigma > 0:                  # a side measurement: device-resident only, Poisson-path JSON keys kept
+    if args.gaussian_sigma > 0 or args.sparse or args.rot_chunk > 0:
+        # a side measurement: device-resident only, per-stage CUDA-event times, no roofline / e2e / cpu legs
         prof_g = {k: v[0] / (args.steps * cfg.n_iter) for k, v in prof.items()}
+        name = ("emc_gaussian_iterations_per_s" if args.gaussian_sigma > 0 else
+                "emc_iterations_per_s[photon lists]" if args.sparse else f"emc_iterations_per_s[rotation chunks of {args.rot_chunk}]")
         if rank == 0:
-            print(json.dumps(dict(metric="emc_gaussian_iterations_per_s", value=value, unit=UNIT, n_gpus=world,
+            print(json.dumps(dict(metric=name, value=value, unit=UNIT, n_gpus=world,
                                   steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,
                                   sigma=args.gaussian_sigma, config=dict(workload=workload_name(cfg)), clocks=clk,
                                   stage_ms_per_iteration=prof_g, gpu_launches=int(launches),
