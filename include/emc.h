@@ -223,6 +223,30 @@ EMC_API emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_det
                                    double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
                                    emc_context *ctx);
 
+/* One iteration with the ROTATION list sharded over several GPUs, one process per GPU (the paper's decomposition:
+ * PAPER.md:170, 188-194 Algorithm 2, 203; DESIGN.md section 11 NEXT-4).  Every rank holds the model, the detector, all
+ * patterns and its own share of the rotations.  The library does the device work of a rank in three calls; the two
+ * exchanges between them belong to the caller (paper_1409_4256_b200/parallel.py does them with torch.distributed):
+ *   emc_shard_stats   Expand, log-likelihood and per-pattern statistics of the rank's rotations
+ *                       -> stats_out [3][ld_n] floats (reference L, reference log w, sum; ld_n = N rounded up to 64)
+ *   (all-gather of stats_out over the ranks -> stats_all [world][3][ld_n], in rank order)
+ *   emc_shard_update  merges the ranks' statistics (the same result on every rank), then P, s[r], the update and the
+ *                       Compress scatter of the rank's rotations -> numden_out [2][n^3] (numerator, denominator grids),
+ *                       loglik (device double, the total log-likelihood, identical on every rank), s_out [R_local] or NULL
+ *   (all-reduce(sum) of numden_out over the ranks)
+ *   emc_shard_finish  model_out = num / den (division as the final step).
+ * The workspace (emc_workspace_bytes for the rank's rotation count and all N patterns) carries L and the packed
+ * patterns from emc_shard_stats to emc_shard_update: same ws, same stream, nothing else in between.
+ * n_rot_total = R of the whole list (log(1/R) for weight == NULL).  world <= 64.  Poisson model, device patterns. */
+EMC_API emc_status emc_shard_stats(const emc_model *model, const emc_detector *det, const emc_rotations *rot_local,
+                           const emc_patterns *pat, int n_rot_total, float *stats_out, unsigned flags, void *ws,
+                           size_t ws_bytes, void *stream);
+EMC_API emc_status emc_shard_update(const emc_model *model, const emc_detector *det, const emc_rotations *rot_local,
+                            const emc_patterns *pat, int n_rot_total, const float *stats_all, int world,
+                            float *numden_out, double *loglik, float *s_out, unsigned flags, void *ws, size_t ws_bytes,
+                            void *stream);
+EMC_API emc_status emc_shard_finish(const float *numden, int n, float *model_out, void *stream);
+
 /* Algorithm 1 with the paper's own likelihood: Gaussian around the slice with a fluence per (rotation, frame),
  * eqs. (2.2), (2.3), (2.5)/(2.11), (2.6), PAPER.md:70-89, 124-130 (NEXT-3, readings GA1-GA7):
  *   phi[r,d]  = sum_p K[d,p]^2 / sum_p W[r,p] K[d,p]                     (2.6), from the slices of this iteration

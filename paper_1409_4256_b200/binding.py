@@ -32,7 +32,7 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
            "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
-           "emc_workspace_bytes_rot_chunked", "emc_iterate_gaussian", "emc_refine", "emc_check",
+           "emc_workspace_bytes_rot_chunked", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_refine", "emc_check",
            "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
@@ -101,6 +101,14 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate_rot_chunked.restype = ci
     lib.emc_iterate_rot_chunked.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                             ci, ci, vp, vp, cu, vp, sz, vp, vp]
+    lib.emc_shard_stats.restype = ci
+    lib.emc_shard_stats.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns), ci, vp, cu,
+                                    vp, sz, vp]
+    lib.emc_shard_update.restype = ci
+    lib.emc_shard_update.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns), ci, vp, ci,
+                                     vp, vp, vp, cu, vp, sz, vp]
+    lib.emc_shard_finish.restype = ci
+    lib.emc_shard_finish.argtypes = [vp, ci, vp, vp]
     lib.emc_iterate_gaussian.restype = ci
     lib.emc_iterate_gaussian.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                          ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp, vp]
@@ -368,6 +376,48 @@ def emc_iterate_rot_chunked(model, q, mask, quat, weight, counts, n_rot_chunk, n
                                           flags, ws.data_ptr(), ws.numel(), _stream(), _ctx(ctx, flags)),
            "emc_iterate_rot_chunked")
     return dict(model=model_out, loglik=loglik, ws=ws)
+
+
+def emc_shard_stats(model, q, mask, quat_local, weight_local, counts, n_rot_total, flags=0, ws=None):
+    """A rank's Expand, log-likelihood and per-pattern statistics (rotation shards, include/emc.h).
+    Returns (stats [3, ld_n] float32, ws): ws carries L to emc_shard_update."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rot = _rotations(quat_local, weight_local)
+    pat = _patterns(counts, det.n_pix)
+    stats = torch.empty((3, ld_for(pat.n_pat)), dtype=torch.float32, device=model.device)
+    ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, pat.n_pat, flags)
+    _check(load().emc_shard_stats(m, det, rot, pat, n_rot_total, stats.data_ptr(), flags, wp, wb, _stream()), "emc_shard_stats")
+    return stats, ws
+
+
+def emc_shard_update(model, q, mask, quat_local, weight_local, counts, n_rot_total, stats_all, ws, flags=0):
+    """Merges the ranks' statistics [world, 3, ld_n] and runs the rank's P, update and Compress scatter.
+    Returns (numden [2, n, n, n] float32, loglik 1-element float64, s [R_local])."""
+    n = model.shape[0]
+    m = _Model(n, _dev(model, torch.float32, "model"))
+    det = _detector(q, mask)
+    rot = _rotations(quat_local, weight_local)
+    pat = _patterns(counts, det.n_pix)
+    world = stats_all.shape[0]
+    if tuple(stats_all.shape[1:]) != (3, ld_for(pat.n_pat)):
+        raise ValueError("stats_all: expected [world, 3, ld_n]")
+    numden = torch.empty((2, n, n, n), dtype=torch.float32, device=model.device)
+    loglik = torch.zeros(1, dtype=torch.float64, device=model.device)
+    s = torch.empty(rot.n_rot, dtype=torch.float32, device=model.device)
+    _check(load().emc_shard_update(m, det, rot, pat, n_rot_total, _dev(stats_all, torch.float32, "stats_all"), world,
+                                   numden.data_ptr(), loglik.data_ptr(), s.data_ptr(), flags, ws.data_ptr(), ws.numel(),
+                                   _stream()), "emc_shard_update")
+    return numden, loglik, s
+
+
+def emc_shard_finish(numden):
+    """model' = num / den from the all-reduced grids."""
+    n = numden.shape[1]
+    model = torch.empty((n, n, n), dtype=torch.float32, device=numden.device)
+    _check(load().emc_shard_finish(_dev(numden, torch.float32, "numden"), n, model.data_ptr(), _stream()), "emc_shard_finish")
+    return model
 
 
 def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None, ctx=None):

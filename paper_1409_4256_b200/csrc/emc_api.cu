@@ -619,6 +619,87 @@ emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_detector *d
     return launch_poison(l.hdr, model_out, (size_t)n * n * n, loglik, n_iter, st);
 }
 
+// ---- rotation shards (NEXT-4): a rank's device work between the caller's collectives
+static emc_status shard_args(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                             const emc_patterns *pat, int n_rot_total, unsigned flags, void *ws, size_t ws_bytes, Layout *l) {
+    if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_rot_total < rot->n_rot) return EMC_ERR_ARG;
+    if (flags & (EMC_PATTERNS_ON_HOST | EMC_SPARSE_PHOTONS | EMC_PROFILE_STAGES)) return EMC_ERR_UNSUPPORTED;
+    if (!sizes_ok(model->n, det->n_pix, rot->n_rot, pat->n_pat)) return EMC_ERR_UNSUPPORTED;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, model->n, det->n_pix, rot->n_rot, pat->n_pat, 0).total));
+    *l = carve(ws, model->n, det->n_pix, rot->n_rot, pat->n_pat, 0);
+    return EMC_OK;
+}
+
+emc_status emc_shard_stats(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                           const emc_patterns *pat, int n_rot_total, float *stats_out, unsigned flags, void *ws,
+                           size_t ws_bytes, void *stream) {
+    Layout l;
+    EMC_TRY(shard_args(model, det, rot, pat, n_rot_total, flags, ws, ws_bytes, &l));
+    if (!stats_out) return EMC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
+    const float log_uniform = log_uniform_of(n_rot_total);
+    EMC_TRY(reset_header(l, st));
+    EMC_TRY(launch_pack(pat->counts, pat->type, n_pat, n_pix, det->mask, l.Kc, l.ld_p, l.KT, l.ld_n, l.hdr, st));
+    Geometry geo;
+    EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, rot->quat, n_rot, l.geom, &geo, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
+    EMC_TRY(launch_expand(model->model, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr, l.planesL, l.ld_p, l.S,
+                          l.blocked, &geo, st, false));
+    bool stats_ready = false;
+    EMC_TRY(run_loglik_gemm(l, n_rot, n_pix, n_pat, l.L, l.ld_n, flags, st, rot->weight, log_uniform, &stats_ready));
+    // the rank's statistics = the carry row after a first-sweep merge with nothing carried in
+    EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, n_pat, l.ld_n, nullptr, nullptr, 0, nullptr, nullptr, nullptr, true, l.scratch,
+                             stats_ready, st, nullptr, 0, log_uniform, 1, false));
+    float *m, *w, *z;
+    normalize_stat_row(l.scratch, n_rot, l.ld_n, -1, &m, &w, &z);
+    const size_t row = sizeof(float) * (size_t)l.ld_n;
+    EMC_TRY_CUDA(cudaMemcpyAsync(stats_out, m, row, cudaMemcpyDeviceToDevice, st));
+    EMC_TRY_CUDA(cudaMemcpyAsync(stats_out + l.ld_n, w, row, cudaMemcpyDeviceToDevice, st));
+    EMC_TRY_CUDA(cudaMemcpyAsync(stats_out + 2 * (size_t)l.ld_n, z, row, cudaMemcpyDeviceToDevice, st));
+    return launch_poison(l.hdr, stats_out, 3 * (size_t)l.ld_n, nullptr, 0, st);
+}
+
+emc_status emc_shard_update(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
+                            const emc_patterns *pat, int n_rot_total, const float *stats_all, int world,
+                            float *numden_out, double *loglik, float *s_out, unsigned flags, void *ws, size_t ws_bytes,
+                            void *stream) {
+    Layout l;
+    EMC_TRY(shard_args(model, det, rot, pat, n_rot_total, flags, ws, ws_bytes, &l));
+    if (!stats_all || world <= 0 || world > 64 || !numden_out || !loglik) return EMC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
+    const float log_uniform = log_uniform_of(n_rot_total);
+    const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
+    // the ranks' statistics become partial rows 0 .. world-1 (merged in rank order: the same result on every rank)
+    const size_t row = sizeof(float) * (size_t)l.ld_n;
+    for (int k = 0; k < world; ++k) {
+        float *m, *w, *z;
+        normalize_stat_row(l.scratch, n_rot, l.ld_n, k, &m, &w, &z);
+        const float *src = stats_all + (size_t)k * 3 * l.ld_n;
+        EMC_TRY_CUDA(cudaMemcpyAsync(m, src, row, cudaMemcpyDeviceToDevice, st));
+        EMC_TRY_CUDA(cudaMemcpyAsync(w, src + l.ld_n, row, cudaMemcpyDeviceToDevice, st));
+        EMC_TRY_CUDA(cudaMemcpyAsync(z, src + 2 * (size_t)l.ld_n, row, cudaMemcpyDeviceToDevice, st));
+    }
+    EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
+    EMC_TRY(launch_colstats_combine_rows(l.scratch, n_rot, world, n_pat, l.ld_n, loglik, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
+    EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, n_pat, l.ld_n, nullptr, l.planesP, (size_t)n_rot * l.ld_n, l.pscale, l.s, nullptr,
+                             true, l.scratch, false, st, nullptr, 0, log_uniform, 2, false));
+    EMC_TRY(run_update_gemm(l, n_rot, n_pix, n_pat, l.Wnum, l.s, EPI_DIV_ROW, flags, st));
+    Geometry geo;
+    EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, rot->quat, n_rot, l.geom, &geo, st));
+    EMC_TRY(launch_compress(l.Wnum, l.s, weighted, geo, n, l.acc, nullptr, nullptr, st, nullptr, COMPRESS_CLEAR | COMPRESS_SCATTER));
+    EMC_TRY(launch_compress_export(l.acc, n, numden_out, st));
+    if (s_out) EMC_TRY_CUDA(cudaMemcpyAsync(s_out, l.s, sizeof(float) * n_rot, cudaMemcpyDeviceToDevice, st));
+    return launch_poison(l.hdr, numden_out, 2 * (size_t)n * n * n, loglik, 1, st);
+}
+
+emc_status emc_shard_finish(const float *numden, int n, float *model_out, void *stream) {
+    if (!numden || !model_out || n < 2 || n > 1024) return EMC_ERR_ARG;
+    return launch_numden_divide(numden, n, model_out, (cudaStream_t)stream);
+}
+
 emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
                                 const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
                                 int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,

@@ -170,7 +170,49 @@ compress_divide_blocked_kernel(const float *__restrict__ acc, int n, float *__re
     if (den_out) den_out[l] = den;
 }
 
+// num and den of every voxel, gathered from the corner blocks, undivided
+__global__ void __launch_bounds__(256)
+compress_export_kernel(const float *__restrict__ acc, int n, float *__restrict__ numden) {
+    const size_t l = (size_t)blockIdx.x * 256 + threadIdx.x;
+    const size_t g = (size_t)n * n * n;
+    if (l >= g) return;
+    const int z = (int)(l % n), y = (int)((l / n) % n), x = (int)(l / ((size_t)n * n));
+    float num = 0.f, den = 0.f;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        const int bx = x - (d >> 2), by = y - ((d >> 1) & 1), bz = z - (d & 1);
+        if (bx < 0 || by < 0 || bz < 0 || bx > n - 2 || by > n - 2 || bz > n - 2) continue;
+        const size_t blk = ((size_t)bx * n + by) * n + bz;
+        num += acc[16 * blk + d];
+        den += acc[16 * blk + 8 + d];
+    }
+    numden[l] = num;
+    numden[g + l] = den;
+}
+
+__global__ void __launch_bounds__(256)
+numden_divide_kernel(const float *__restrict__ numden, size_t g, float *__restrict__ model_out) {
+    const size_t l = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (l >= g) return;
+    const float num = numden[l], den = numden[g + l];
+    model_out[l] = den > 0.f ? num / den : 0.f;
+}
+
 }  // namespace
+
+emc_status launch_compress_export(const float2 *acc, int n, float *numden, cudaStream_t st) {
+    const size_t g = (size_t)n * n * n;
+    compress_export_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float *>(acc), n, numden);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+emc_status launch_numden_divide(const float *numden, int n, float *model_out, cudaStream_t st) {
+    const size_t g = (size_t)n * n * n;
+    numden_divide_kernel<<<(unsigned)((g + 255) / 256), 256, 0, st>>>(numden, g, model_out);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
 
 size_t compress_scratch_float2(int n) { return (size_t)8 * n * n * n; }
 

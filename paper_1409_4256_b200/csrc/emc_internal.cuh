@@ -185,6 +185,12 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
 // longer rotation list)
 // n_store: columns of a row the call may write (planes padding, column arrays); 0 = ld_n.  Smaller when L, planes and
 // scratch are views that start inside a row (emc_api.cu, pipelined first iteration).
+// Rotation shards (one process per GPU, DESIGN.md section 11 NEXT-4): (m, w, z) pointers of partial row `row` of the statistics
+// scratch (row < 0: the carry row), and the merge of the first n_rows partial rows (one per rank, in rank order) into the
+// final column statistics (+ the total log-likelihood); launch_normalize(chunk_mode = 2) then writes P.
+void normalize_stat_row(float *scratch, int layout_rot, int ld_n, int row, float **m, float **w, float **z);
+emc_status launch_colstats_combine_rows(float *scratch, int layout_rot, int n_rows, int n_pat, int ld_n, double *loglik,
+                                        cudaStream_t st);
 // operand planes of a given P (stage API of emc_update).
 emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half *planes, int ld_pl,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st);
@@ -222,6 +228,10 @@ struct DenCache {
     bool force;
 };
 enum { COMPRESS_CLEAR = 1, COMPRESS_SCATTER = 2, COMPRESS_DIVIDE = 4, COMPRESS_ALL = 7 };
+// numden [2][n^3] = the numerator and denominator grids gathered from the corner blocks (what rotation shards all-reduce)
+emc_status launch_compress_export(const float2 *acc, int n, float *numden, cudaStream_t st);
+// model' = num / den from such grids (division as the final step)
+emc_status launch_numden_divide(const float *numden, int n, float *model_out, cudaStream_t st);
 emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighted, const Geometry &geo, int n,
                            float2 *acc, float *model_out, float *den_out, cudaStream_t st,
                            const DenCache *cache = nullptr, int phases = COMPRESS_ALL);

@@ -525,6 +525,26 @@ emc_status launch_normalize(const float *L, const float *weight, int n_rot, int 
     return EMC_OK;
 }
 
+void normalize_stat_row(float *scratch, int layout_rot, int ld_n, int row, float **m, float **w, float **z) {
+    const size_t stat_rows = (size_t)normalize_stat_rows(layout_rot);
+    if (row < 0) row = (int)stat_rows - 1;                       // the carry row
+    *m = scratch + (size_t)row * ld_n;
+    *w = *m + stat_rows * ld_n;
+    *z = *w + stat_rows * ld_n;
+}
+
+emc_status launch_colstats_combine_rows(float *scratch, int layout_rot, int n_rows, int n_pat, int ld_n, double *loglik,
+                                        cudaStream_t st) {
+    const int stat_rows = normalize_stat_rows(layout_rot);
+    if (n_rows > stat_rows) return EMC_ERR_UNSUPPORTED;
+    float *part_m = scratch, *part_w = part_m + (size_t)stat_rows * ld_n, *part_z = part_w + (size_t)stat_rows * ld_n;
+    float *col_m = scratch + (size_t)3 * stat_rows * ld_n, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
+    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, ld_n, n_rows, col_m, col_w, col_iz,
+                                                               loglik, -1, 0);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
 emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half *planes, int ld_pl,
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st) {
     dim3 grid(ceil_div(n_pat, kChunkCols), ceil_div(n_rot, kWarps));

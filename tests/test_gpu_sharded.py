@@ -1,0 +1,117 @@
+"""Rotation shards on the GPU (`-m gpu`): the three libemc phases of every rank run one after the other on cuda:0 with the
+two exchanges done in the test (no process group), against the oracle and against the unsharded emc_iterate; then the
+real thing, two processes and paper_1409_4256_b200.parallel.iterate_sharded, with gloo moving the two small messages
+(the ranks' kernels never wait on one another: the collectives are host-side)."""
+import os
+import pathlib
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.multiprocessing as mp
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+emc = pytest.importorskip("paper_1409_4256_b200")
+ROOT = pathlib.Path(__file__).resolve().parents[1]
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+@pytest.mark.parametrize("name,world,weighted,null_w", [("T1", 2, False, False), ("T1", 3, True, True), ("T2", 4, False, False),
+                                                        ("C1", 2, False, False)])
+def test_shard_phases_match_oracle_and_unsharded(inputs_cache, name, world, weighted, null_w):
+    from paper_1409_4256_b200.parallel import shard_bounds
+
+    inp = inputs_cache(name)
+    cfg = inp.cfg
+    stage = len(inp.quat) - 1
+    quat, weight = inp.quat[stage], inp.weight[stage]
+    n_rot = quat.shape[0]
+    w_np = np.full(n_rot, 1.0 / n_rot, np.float32) if null_w else weight
+    d_model, d_q, d_mask = dev(inp.model_init), dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask)
+    d_quat, d_w, d_k = dev(quat), (None if null_w else dev(weight)), dev(inp.counts)
+    flags = emc.EMC_COMPRESS_WEIGHTED if weighted else 0
+    shares = [shard_bounds(n_rot, world, r) for r in range(world)]
+    stats, wss = [], []
+    for r0, r1 in shares:                                           # phase 1 of every rank
+        st, ws = emc.emc_shard_stats(d_model, d_q, d_mask, d_quat[r0:r1].contiguous(), None if null_w else d_w[r0:r1].contiguous(),
+                                     d_k, n_rot, flags=flags)
+        stats.append(st)
+        wss.append(ws)
+    stats_all = torch.stack(stats)                                  # the all-gather
+    numden, lls, s_parts = None, [], []
+    for (r0, r1), ws in zip(shares, wss):                           # phase 2 of every rank
+        nd, ll, s = emc.emc_shard_update(d_model, d_q, d_mask, d_quat[r0:r1].contiguous(),
+                                         None if null_w else d_w[r0:r1].contiguous(), d_k, n_rot, stats_all, ws, flags=flags)
+        emc.emc_check(ws)
+        numden = nd if numden is None else numden + nd              # the all-reduce
+        lls.append(float(host(ll)[0]))
+        s_parts.append(host(s))
+    model = host(emc.emc_shard_finish(numden)).reshape(-1)
+    assert max(lls) - min(lls) <= 1e-9 * abs(lls[0])                # every rank computes the same total
+    ref = o.iterate(inp.model_init, inp.q, inp.mask, quat, w_np, inp.counts, weighted=weighted)
+    one = emc.emc_iterate(d_model, d_q, d_mask, d_quat, d_w, d_k, flags=flags)
+    assert abs(lls[0] - ref["LL"]) <= 1e-5 * abs(ref["LL"])
+    assert abs(lls[0] - float(host(one["loglik"])[0])) <= 1e-6 * abs(lls[0])
+    s_all = np.concatenate(s_parts)
+    assert np.abs(s_all - ref["s"]).max() <= 2e-4 * max(1.0, ref["s"].max())
+    m_ref, m_one = ref["model"].reshape(-1), host(one["model"]).reshape(-1)
+    cov = ref["den"] >= 1e-3 * ref["den"].max()
+    scale = np.abs(m_ref).max()
+    rel = np.abs(model - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
+    rel1 = np.abs(model - m_one)[cov] / (np.abs(m_one[cov]) + 1e-6 * scale)
+    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2, (np.median(rel), rel.max())
+    assert np.median(rel1) <= 1e-5 and rel1.max() <= 2e-2, (np.median(rel1), rel1.max())
+
+
+def _worker(rank, world, port, out):
+    import torch.distributed as dist
+
+    sys.path.insert(0, str(ROOT))
+    from emc_inputs import make_inputs
+    from paper_1409_4256_b200 import parallel
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    inp = make_inputs("T1")
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    res = parallel.iterate_sharded(t(inp.model_init), t(inp.q), t(inp.mask), t(inp.quat[0]), t(inp.weight[0]), t(inp.counts),
+                                   n_iter=2)
+    torch.cuda.synchronize()
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, res["model"].cpu().numpy(), res["loglik"].cpu().numpy()))
+
+
+def test_two_processes_iterate_sharded(inputs_cache):
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((out.get(timeout=600) for _ in procs), key=lambda x: x[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    (_, m0, ll0), (_, m1, ll1) = got
+    assert np.array_equal(ll0, ll1)
+    assert np.abs(m0 - m1).max() <= 1e-6 * np.abs(m0).max()          # the float32 atomics of each rank's own scatter
+    inp = inputs_cache("T1")
+    d = [dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]), dev(inp.counts)]
+    one = emc.emc_iterate(*d, n_iter=2)
+    assert np.allclose(ll0, host(one["loglik"]), rtol=2e-6)
+    mo = host(one["model"])
+    big = np.abs(mo) >= 1e-3 * np.abs(mo).max()
+    assert np.median(np.abs(m0 - mo)[big] / np.abs(mo)[big]) <= 1e-5
