@@ -62,6 +62,9 @@ def parse():
                     help="side measurement: stages 2 and 4 from photon lists (EMC_SPARSE_PHOTONS) instead of the dense contractions")
     ap.add_argument("--rot-chunk", type=int, default=0,
                     help="side measurement: emc_iterate_rot_chunked with this many rotations per chunk (one pattern chunk)")
+    ap.add_argument("--shard-rotations", action="store_true",
+                    help="side measurement (N > 1): ONE job with the rotation list sharded over the ranks "
+                         "(paper_1409_4256_b200.parallel, NCCL all-gather + all-reduce) instead of N replicas; strong scaling")
     ap.add_argument("--photons", type=float, default=0.0, help="override the config's mean photons per pixel (density sweeps)")
     ap.add_argument("--n-pat", type=int, default=0, help="override the config's pattern count (side measurements)")
     return ap.parse_args()
@@ -368,6 +371,13 @@ def main():
                 d_ll[it0:it0 + n_it] = out["loglik"]
                 src, it0 = out["model"], it0 + n_it
                 continue
+            if args.shard_rotations and world > 1:
+                from paper_1409_4256_b200 import parallel
+
+                out = parallel.iterate_sharded(src, d_q, d_mask, quat, wgt, d_counts, n_iter=n_it, flags=f & ~emc.EMC_PROFILE_STAGES)
+                d_ll[it0:it0 + n_it] = out["loglik"]
+                src, it0 = out["model"], it0 + n_it
+                continue
             if args.rot_chunk > 0:
                 out = emc.emc_iterate_rot_chunked(src, d_q, d_mask, quat, wgt, d_counts, args.rot_chunk, n_iter=n_it, flags=f,
                                                   ws=ws, ctx=ctx)
@@ -404,11 +414,16 @@ def main():
     prof = emc.emc_profile_read(ctx)
     ms, value = whole_job(ms, args.steps * cfg.n_iter, world, "cuda")
 
-    if args.gaussian_sigma > 0 or args.sparse or args.rot_chunk > 0:
+    sharded = args.shard_rotations and world > 1
+    if sharded:
+        value /= world                       # one job, not N replicas: iterations of THE job per second
+    if args.gaussian_sigma > 0 or args.sparse or args.rot_chunk > 0 or sharded:
         # a side measurement: device-resident only, per-stage CUDA-event times, no roofline / e2e / cpu legs
         prof_g = {k: v[0] / (args.steps * cfg.n_iter) for k, v in prof.items()}
         name = ("emc_gaussian_iterations_per_s" if args.gaussian_sigma > 0 else
-                "emc_iterations_per_s[photon lists]" if args.sparse else f"emc_iterations_per_s[rotation chunks of {args.rot_chunk}]")
+                "emc_iterations_per_s[photon lists]" if args.sparse else
+                f"emc_iterations_per_s[rotations sharded over {world} ranks, strong scaling]" if sharded else
+                f"emc_iterations_per_s[rotation chunks of {args.rot_chunk}]")
         if rank == 0:
             print(json.dumps(dict(metric=name, value=value, unit=UNIT, n_gpus=world,
                                   steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,

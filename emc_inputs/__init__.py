@@ -13,6 +13,7 @@ from .synth import (  # noqa: F401
     detector_geometry,
     detector_mask,
     intensity_model,
+    ladder_rotations,
     make_inputs,
     random_rotations,
     rotation_ladder,

@@ -149,6 +149,22 @@ def random_rotations(n_rot: int, seed: int) -> np.ndarray:
     return v.astype(np.float32)
 
 
+def ladder_rotations(d: int, seed: int):
+    """A rotation list of the size eq. (2.7) gives for discretisation level d, M_rot(d) = 10 (5 d^3 + d) (PAPER.md:95-98:
+    6 300 for d = 5 ... 86 520 for d = 12), WITH non-uniform prior weights w_j.  The paper refines the
+    600-cell (ref. [11] App. C, not in the container); the stand-in is seeded uniform random quaternions, each weighted by
+    the volume it represents: w_j ~ (distance to its nearest neighbour on the 3-sphere, antipodes identified)^3,
+    normalised to sum 1 (a library nearest-neighbour query, scipy cKDTree).  Returns (quat [M,4] float32, weight [M] float32)."""
+    from scipy.spatial import cKDTree
+
+    m = int(rotation_ladder(d))
+    quat = random_rotations(m, seed)
+    both = np.concatenate([quat, -quat]).astype(np.float64)       # q and -q are the same rotation
+    dist, _ = cKDTree(both).query(quat.astype(np.float64), k=2)
+    w = dist[:, 1] ** 3
+    return quat, (w / w.sum()).astype(np.float32)
+
+
 def _slices_library(model64: np.ndarray, q: np.ndarray, quat: np.ndarray) -> np.ndarray:
     """Mean intensities of the simulated experiment: the model read at R q + n/2 by the library's
     own linear interpolation.  scipy's quaternions are scalar-last."""

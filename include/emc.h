@@ -256,12 +256,22 @@ EMC_API emc_status emc_shard_finish(const float *numden, int n, float *model_out
  * over unmasked pixels, then Compress by eq. (2.12) with EMC_COMPRESS_WEIGHTED (what the paper runs) or (2.10).
  * With phi of (2.6), Q collapses to (B^2 / A_d - C_r) / (2 sigma^2), B = sum_p W K (one plane GEMM), A_d = sum_p K^2,
  * C_r = sum_p W^2; float32 evaluation of that form carries an absolute error of about 1e-7 C_r / (2 sigma^2).
- * One pattern chunk, device-resident or host-resident patterns; slices must stay below 65504 (fp16 operand planes).
+ * Pattern chunks as in emc_iterate (the fluence and the E-step are per frame, so chunks are independent; s[r] and the
+ * numerators add up), device-resident or host-resident patterns; slices must stay below 65504 (fp16 operand planes).
  * Arguments as emc_iterate; sigma > 0 in the units of the model. */
 EMC_API emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
-                                const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
-                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
-                                emc_context *ctx);
+                                const emc_patterns *pat, int n_iter, int n_pat_chunk, float sigma, float *model_out,
+                                float *P_out, int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
+                                void *stream, emc_context *ctx);
+
+/* The E-step of the Gaussian model as a stage of its own (eqs. 2.2, 2.3, 2.6):
+ *   phi[r,d] = sum_p K[d,p]^2 / sum_p W[r,p] K[d,p],   Q[r,d] = -sum_p (K[d,p] / phi[r,d] - W[r,p])^2 / (2 sigma^2)
+ * over unmasked pixels, evaluated in the collapsed form (B^2 / A_d - C_r) / (2 sigma^2) that emc_iterate_gaussian uses
+ * (same kernels), so that the exponent itself can be checked, not only the responsibilities that come out of it.
+ *   W [R][P] float in (as written by emc_expand);  Q, phi [R][ld_n] float out, either may be NULL. */
+EMC_API emc_status emc_loglik_gaussian(const float *W, const emc_detector *det, const emc_patterns *pat, int n_rot,
+                               float sigma, float *Q, float *phi, int ld_n, unsigned flags, void *ws, size_t ws_bytes,
+                               void *stream);
 
 /* Adaptive EMC, section 3.4 and eq. (3.1): `n_iter` iterations that start on the coarsest
  * rotation list levels[0] and move on to the next list after an iteration n >= 1 whose total log-likelihood

@@ -32,7 +32,7 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
            "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
-           "emc_workspace_bytes_rot_chunked", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_refine", "emc_check",
+           "emc_workspace_bytes_rot_chunked", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_loglik_gaussian", "emc_refine", "emc_check",
            "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
@@ -101,6 +101,8 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate_rot_chunked.restype = ci
     lib.emc_iterate_rot_chunked.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                             ci, ci, vp, vp, cu, vp, sz, vp, vp]
+    lib.emc_loglik_gaussian.restype = ci
+    lib.emc_loglik_gaussian.argtypes = [vp, POINTER(_Detector), POINTER(_Patterns), ci, ctypes.c_float, vp, vp, ci, cu, vp, sz, vp]
     lib.emc_shard_stats.restype = ci
     lib.emc_shard_stats.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns), ci, vp, cu,
                                     vp, sz, vp]
@@ -111,7 +113,7 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_shard_finish.argtypes = [vp, ci, vp, vp]
     lib.emc_iterate_gaussian.restype = ci
     lib.emc_iterate_gaussian.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
-                                         ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp, vp]
+                                         ci, ci, ctypes.c_float, vp, vp, ci, vp, cu, vp, sz, vp, vp]
     lib.emc_refine.restype = ci
     lib.emc_refine.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), ci, POINTER(_Patterns), ci,
                                c_double, ci, vp, vp, vp, POINTER(ctypes.c_int32), cu, vp, sz, vp, vp]
@@ -378,6 +380,20 @@ def emc_iterate_rot_chunked(model, q, mask, quat, weight, counts, n_rot_chunk, n
     return dict(model=model_out, loglik=loglik, ws=ws)
 
 
+def emc_loglik_gaussian(w, q, mask, counts, sigma, flags=0, ws=None):
+    """E-step exponent and fluence of the Gaussian model (eqs. 2.2, 2.3, 2.6).  Returns (Q, phi) as [R, N] views."""
+    n_rot, n_pix = w.shape
+    det = _detector(q, mask)
+    pat = _patterns(counts, n_pix)
+    ld = ld_for(pat.n_pat)
+    big_q = torch.empty((n_rot, ld), dtype=torch.float32, device=w.device)
+    phi = torch.empty((n_rot, ld), dtype=torch.float32, device=w.device)
+    ws, wp, wb = _ws(ws, 2, n_pix, n_rot, pat.n_pat)
+    _check(load().emc_loglik_gaussian(_dev(w, torch.float32, "W"), det, pat, n_rot, float(sigma), big_q.data_ptr(), phi.data_ptr(),
+                                      ld, flags, wp, wb, _stream()), "emc_loglik_gaussian")
+    return big_q[:, :pat.n_pat], phi[:, :pat.n_pat]
+
+
 def emc_shard_stats(model, q, mask, quat_local, weight_local, counts, n_rot_total, flags=0, ws=None):
     """A rank's Expand, log-likelihood and per-pattern statistics (rotation shards, include/emc.h).
     Returns (stats [3, ld_n] float32, ws): ws carries L to emc_shard_update."""
@@ -420,7 +436,8 @@ def emc_shard_finish(numden):
     return model
 
 
-def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, flags=0, want_p=False, ws=None, ctx=None):
+def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, n_pat_chunk=0, flags=0, want_p=False, ws=None,
+                         ctx=None):
     """Algorithm 1 with the paper's Gaussian likelihood and fluence (eqs. 2.2-2.6).  Returns dict(model, loglik, P)."""
     n = model.shape[0]
     m = _Model(n, _dev(model, torch.float32, "model"))
@@ -432,8 +449,9 @@ def emc_iterate_gaussian(model, q, mask, quat, weight, counts, sigma, n_iter=1, 
     loglik = torch.zeros(n_iter, dtype=torch.float64, device=dev)
     ld = ld_for(pat.n_pat)
     p = torch.empty((rot.n_rot, ld), dtype=torch.float32, device=dev) if want_p else None
-    ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, pat.n_pat, flags)
-    _check(load().emc_iterate_gaussian(m, det, rot, pat, n_iter, float(sigma), model_out.data_ptr(),
+    chunk = pat.n_pat if (n_pat_chunk == 0 or n_pat_chunk > pat.n_pat) else n_pat_chunk
+    ws, wp, wb = _ws(ws, n, det.n_pix, rot.n_rot, chunk, flags)
+    _check(load().emc_iterate_gaussian(m, det, rot, pat, n_iter, n_pat_chunk, float(sigma), model_out.data_ptr(),
                                        p.data_ptr() if want_p else None, ld, loglik.data_ptr(), flags, wp, wb, _stream(),
                                        _ctx(ctx, flags)), "emc_iterate_gaussian")
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)

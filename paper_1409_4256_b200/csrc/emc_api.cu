@@ -282,6 +282,35 @@ emc_status emc_loglik(const float *W, const int32_t *idx, const emc_detector *de
     return launch_poison(l.hdr, L, (size_t)n_rot * ld_n, nullptr, 0, st);
 }
 
+emc_status emc_loglik_gaussian(const float *W, const emc_detector *det, const emc_patterns *pat, int n_rot,
+                               float sigma, float *Q, float *phi, int ld_n, unsigned flags, void *ws, size_t ws_bytes,
+                               void *stream) {
+    if (!W || !det_ok(det) || !pat_ok(pat) || n_rot <= 0 || (!Q && !phi) || ld_n < pat->n_pat || !(sigma > 0.f)) return EMC_ERR_ARG;
+    if (!sizes_ok(2, det->n_pix, n_rot, pat->n_pat)) return EMC_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, 0, det->n_pix, n_rot, pat->n_pat, 0).total));
+    const Layout l = carve(ws, 0, det->n_pix, n_rot, pat->n_pat, 0);
+    const float inv2s2 = 1.f / (2.f * sigma * sigma);
+    EMC_TRY(reset_header(l, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(l.S, 0, sizeof(float) * n_rot, st));
+    EMC_TRY(launch_logw_split(W, nullptr, det->mask, det->n_pix, n_rot, l.planesL, l.ld_p, l.S, st, true));   // planes of W, C_r
+    EMC_TRY(launch_pack(pat->counts, pat->type, pat->n_pat, det->n_pix, det->mask, l.Kc, l.ld_p, nullptr, 0, l.hdr, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * 2 * l.ld_n, st));
+    EMC_TRY(launch_rowsq(l.Kc, pat->n_pat, det->n_pix, l.ld_p, inv2s2, l.Asq, l.Asq + l.ld_n, st));
+    GemmProblem g;                                              // B = W K^T, the same plane GEMM, no epilogue
+    g.A = l.planesL; g.B = l.Kc; g.n_planes = 2;
+    g.M = n_rot; g.N = pat->n_pat; g.K = det->n_pix;
+    g.lda = l.ld_p; g.ldb = l.ld_p; g.plane_stride = (size_t)n_rot * l.ld_p;
+    g.a_fmt = g.b_fmt = FMT_F16;
+    g.out = l.L; g.ld_out = l.ld_n; g.rowv = nullptr; g.epilogue = EPI_STORE;
+    g.one_cta = (flags & EMC_GEMM_1CTA) != 0;
+    EMC_TRY(launch_plane_gemm(g, (flags & EMC_DEBUG_SIMT) != 0, st));
+    EMC_TRY(launch_gauss_q(l.L, l.S, l.Asq, l.Asq + l.ld_n, inv2s2, n_rot, pat->n_pat, l.ld_n, Q, phi, ld_n, st));
+    if (Q) EMC_TRY(launch_poison(l.hdr, Q, (size_t)n_rot * ld_n, nullptr, 0, st));
+    if (phi) EMC_TRY(launch_poison(l.hdr, phi, (size_t)n_rot * ld_n, nullptr, 0, st));
+    return EMC_OK;
+}
+
 emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
                          float *s, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
                          void *stream) {
@@ -351,7 +380,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes, sparse).total));
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes, sparse);
     if (P_out && (n_chunks != 1 || ld_n != l.ld_n)) return EMC_ERR_ARG;
-    if (gauss && (n_chunks != 1 || (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT)))) return EMC_ERR_UNSUPPORTED;
+    if (gauss && (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT))) return EMC_ERR_UNSUPPORTED;
     const float log_uniform = log_uniform_of(n_rot);
     const GaussTerms gterms = {l.S, l.Asq, l.Asq + l.ld_n, gauss ? 1.f / (2.f * sigma * sigma) : 0.f, log_uniform};
     const GaussTerms *gt = gauss ? &gterms : nullptr;
@@ -701,11 +730,11 @@ emc_status emc_shard_finish(const float *numden, int n, float *model_out, void *
 }
 
 emc_status emc_iterate_gaussian(const emc_model *model, const emc_detector *det, const emc_rotations *rot,
-                                const emc_patterns *pat, int n_iter, float sigma, float *model_out, float *P_out,
-                                int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes, void *stream,
-                                emc_context *ctx) {
+                                const emc_patterns *pat, int n_iter, int n_pat_chunk, float sigma, float *model_out,
+                                float *P_out, int ld_n, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
+                                void *stream, emc_context *ctx) {
     if (!(sigma > 0.f)) return EMC_ERR_ARG;
-    return iterate_impl(model, det, rot, pat, n_iter, 0, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes, stream,
+    return iterate_impl(model, det, rot, pat, n_iter, n_pat_chunk, model_out, P_out, ld_n, loglik, flags, ws, ws_bytes, stream,
                         ctx, sigma);
 }
 

@@ -241,7 +241,7 @@ rowsum_kernel(const float *__restrict__ S_part, int n_rot, int n_bands, float *_
 __global__ void __launch_bounds__(kThreads)
 logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
                   const uint8_t *__restrict__ mask, int n_pix, __half *__restrict__ planes, int ld_p,
-                  size_t plane_stride, float *__restrict__ S) {
+                  size_t plane_stride, float *__restrict__ S, int gauss) {
     __shared__ float red[kThreads / 32];
     const int r = blockIdx.x;
     float part = 0.f;
@@ -254,11 +254,11 @@ logw_split_kernel(const float *__restrict__ W, const int32_t *__restrict__ idx,
         const bool inside = idx ? (idx[o] >= 0) : true;
         const bool use = mask ? (mask[p] != 0) : true;
         __half hi, lo;
-        split_logw(w, use && inside, hi, lo);
+        split_logw(w, use && inside, hi, lo, gauss);
         const size_t po = (size_t)r * ld_p + p;
         planes[po] = hi;
         planes[plane_stride + po] = lo;
-        if (use) part += w;
+        if (use) part += gauss ? w * w : w;
     }
     const float t = block_sum(part, red);
     if (threadIdx.x == 0) atomicAdd(S + r, t);
@@ -330,10 +330,10 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
 }
 
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
-                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st) {
+                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st, bool gauss) {
     dim3 grid(n_rot, ceil_div(n_pix, kPixPerBlock));
     logw_split_kernel<<<grid, kThreads, 0, st>>>(W, idx, mask, n_pix, planes, ld_p,
-                                                 (size_t)n_rot * ld_p, S);
+                                                 (size_t)n_rot * ld_p, S, gauss ? 1 : 0);
     EMC_LAUNCHED();
     return EMC_OK;
 }

@@ -90,7 +90,11 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
 // S the row sums (operands of the photon-list log-likelihood, emc_sparse.cu)
 // logW planes + S from a given W (stage API of emc_loglik).
 emc_status launch_logw_split(const float *W, const int32_t *idx, const uint8_t *mask, int n_pix,
-                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st);
+                             int n_rot, __half *planes, int ld_p, float *S, cudaStream_t st, bool gauss = false);
+// gauss: the planes hold W itself and S[r] += sum_{p:mask} W^2 (stage API of the Gaussian model)
+// Q[r,d] = B^2 g_d - C_r / (2 sigma^2) and phi[r,d] = A_d / B[r,d] (inf where B = 0) from B = W K^T (eqs. 2.2, 2.3, 2.6 collapsed)
+emc_status launch_gauss_q(const float *B, const float *c_row, const float *g_col, const float *ia_col, float inv2s2, int n_rot,
+                          int n_pat, int ld_b, float *Q, float *phi, int ld_out, cudaStream_t st);
 
 // Pack photon counts (emc_pack.cu): Kc [Nc][ld_p] fp16 (row = pattern) and/or KT [P][ld_n] fp16
 // (row = pixel), masked pixels zeroed, an unmasked count above EMC_MAX_COUNT recorded in hdr->max_count.

@@ -444,6 +444,22 @@ p_split_kernel(const float *__restrict__ P, int n_rot, int n_pat, int ld_n, __ha
                  chunk_inv_scale + (size_t)blockIdx.x * n_rot + r);
 }
 
+// stage API of the Gaussian model: the E-step's exponent and the fluence themselves
+__global__ void __launch_bounds__(256)
+gauss_q_kernel(const float *__restrict__ B, const float *__restrict__ c_row, const float *__restrict__ g_col,
+               const float *__restrict__ ia_col, float inv2s2, int n_pat, int ld_b, float *__restrict__ Q,
+               float *__restrict__ phi, int ld_out) {
+    const int d = blockIdx.y * 256 + threadIdx.x, r = blockIdx.x;
+    if (d >= n_pat) return;
+    const float b = B[(size_t)r * ld_b + d];
+    // the same two terms, formed the same way, as the GEMM epilogue's statistics and the second sweep (emc_internal.cuh)
+    if (Q) Q[(size_t)r * ld_out + d] = __fadd_rn(gauss_elem_term(b, g_col[d]), gauss_row_term(0.f, c_row[r], inv2s2));
+    if (phi) {
+        const float ia = ia_col[d];
+        phi[(size_t)r * ld_out + d] = (b > 0.f && ia > 0.f) ? 1.f / (b * ia) : INFINITY;      // GA3: K / phi = 0
+    }
+}
+
 __global__ void __launch_bounds__(256)
 div_rows_kernel(float *__restrict__ Wn, const float *__restrict__ s, int n_pix) {
     const int p = blockIdx.y * 256 + threadIdx.x;
@@ -549,6 +565,13 @@ emc_status launch_p_split(const float *P, int n_rot, int n_pat, int ld_n, __half
                           size_t plane_stride, float *chunk_inv_scale, cudaStream_t st) {
     dim3 grid(ceil_div(n_pat, kChunkCols), ceil_div(n_rot, kWarps));
     p_split_kernel<<<grid, kThreads, 0, st>>>(P, n_rot, n_pat, ld_n, planes, ld_pl, plane_stride, chunk_inv_scale);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+emc_status launch_gauss_q(const float *B, const float *c_row, const float *g_col, const float *ia_col, float inv2s2, int n_rot,
+                          int n_pat, int ld_b, float *Q, float *phi, int ld_out, cudaStream_t st) {
+    gauss_q_kernel<<<dim3(n_rot, ceil_div(n_pat, 256)), 256, 0, st>>>(B, c_row, g_col, ia_col, inv2s2, n_pat, ld_b, Q, phi, ld_out);
     EMC_LAUNCHED();
     return EMC_OK;
 }

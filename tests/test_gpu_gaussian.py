@@ -67,3 +67,44 @@ def test_gaussian_multi_iteration_and_arguments(inputs_cache):
     pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
     h = emc.emc_iterate_gaussian(*args[:5], pinned, 10.0, n_iter=2, flags=emc.EMC_PATTERNS_ON_HOST)
     assert np.allclose(h["loglik"].cpu().numpy(), lls, rtol=1e-6)
+
+
+@pytest.mark.parametrize("name,sigma", [("T1", 20.0), ("T2", 6.0), ("T3", 10.0), ("C1", 30.0)])
+def test_loglik_gaussian_stage_q_and_phi(inputs_cache, name, sigma):
+    """The E-step of the Gaussian model on its own (eqs. 2.2, 2.3, 2.6): the exponent Q against the oracle's term-by-term
+    sum within 1e-5 of its scale A[r,d] = sum((K/phi)^2 + W^2) / (2 sigma^2) (the tolerance DESIGN.md section 11 states for the
+    collapsed form), and the fluence phi to relative 1e-5."""
+    inp = inputs_cache(name)
+    stage = len(inp.quat) - 1
+    w_ref, idx = o.expand(inp.model_init, inp.q, inp.quat[stage])
+    phi_ref = o.fluence(w_ref, inp.counts, inp.mask)
+    q_ref, a_ref = o.gaussian_loglik(w_ref, inp.counts, inp.mask, phi_ref, sigma)
+    big_q, phi = emc.emc_loglik_gaussian(dev(w_ref), dev(inp.q), dev(inp.mask), dev(inp.counts), sigma)
+    big_q, phi = big_q.cpu().numpy().astype(np.float64), phi.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(big_q - q_ref) <= 1e-5 * a_ref + 1e-30), f"max dQ/A {np.max(np.abs(big_q - q_ref) / (a_ref + 1e-30)):.3e}"
+    fin = np.isfinite(phi_ref)
+    assert np.array_equal(np.isfinite(phi), fin)
+    assert np.all(np.abs(phi[fin] - phi_ref[fin]) <= 1e-5 * np.abs(phi_ref[fin]))
+
+
+@pytest.mark.parametrize("name,chunk", [("T1", 50), ("T2", 200)])
+def test_iterate_gaussian_pattern_chunks(inputs_cache, name, chunk):
+    """Pattern chunks of the Gaussian model: fluence and E-step are per frame, so the chunked run equals the one-chunk run
+    (and through it the oracle) up to summation order; host-resident chunks go through the staging buffers."""
+    inp = inputs_cache(name)
+    stage = len(inp.quat) - 1
+    args = (dev(inp.model_init), dev(inp.q), dev(inp.mask), dev(inp.quat[stage]), dev(inp.weight[stage]), dev(inp.counts))
+    ref = o.iterate_gaussian(inp.model_init, inp.q, inp.mask, inp.quat[stage], inp.weight[stage], inp.counts, 15.0)
+    one = emc.emc_iterate_gaussian(*args, 15.0, flags=emc.EMC_COMPRESS_WEIGHTED)
+    pinned = torch.from_numpy(inp.counts.copy()).pin_memory()
+    for counts, extra in ((args[5], 0), (pinned, emc.EMC_PATTERNS_ON_HOST)):
+        out = emc.emc_iterate_gaussian(*args[:5], counts, 15.0, n_pat_chunk=chunk, flags=emc.EMC_COMPRESS_WEIGHTED | extra)
+        emc.emc_check(out["ws"])
+        ll, ll1 = float(out["loglik"].cpu()[0]), float(one["loglik"].cpu()[0])
+        assert abs(ll - ll1) <= 1e-6 * abs(ll1) and abs(ll - ref["LL"]) <= 1e-5 * ref["A"].max(axis=0).sum()
+        m, m1, m_ref = (x.reshape(-1) for x in (out["model"].cpu().numpy(), one["model"].cpu().numpy(), ref["model"]))
+        cov = ref["den"] >= 1e-3 * ref["den"].max()
+        scale = np.abs(m_ref).max()
+        assert np.median(np.abs(m - m1)[cov] / (np.abs(m1[cov]) + 1e-6 * scale)) <= 1e-5
+        rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
+        assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2

@@ -510,3 +510,16 @@ def test_photon_list_forms_equal_the_dense_definitions(inputs_cache):
     wn2, s2 = o.update_photon_list(p.astype(np.float32), lists, inp.counts.shape[1])
     assert np.array_equal(s, s2)
     assert np.abs(wn2 - wn).max() <= 1e-6 * np.abs(wn).max() and np.all(wn2[:, ~use] == 0)
+
+
+def test_ladder_rotations_sizes_and_weights():
+    """Input generator of NEXT-1: list sizes are eq. (2.7)'s (golden ladder), quaternions are unit with w >= 0,
+    the weights are positive, non-uniform and sum to 1."""
+    from emc_inputs import ladder_rotations, rotation_ladder
+
+    for d in (1, 2, 5):
+        quat, w = ladder_rotations(d, 99)
+        assert len(quat) == len(w) == int(rotation_ladder(d)) == 10 * (5 * d ** 3 + d)
+        assert np.allclose(np.linalg.norm(quat.astype(np.float64), axis=1), 1.0, atol=1e-6) and (quat[:, 0] >= 0).all()
+        assert (w > 0).all() and abs(float(w.astype(np.float64).sum()) - 1.0) <= 1e-5 and w.max() > 1.5 * w.min()
+    assert int(rotation_ladder(5)) == 6300 and int(rotation_ladder(12)) == 86520

@@ -63,7 +63,11 @@ def test_emc_refine_matches_oracle(threshold):
 
     emc = pytest.importorskip("paper_1409_4256_b200")
     inp = make_inputs("T2")
-    levels = make_levels((60, 150, 333))
+    # the ladder of eq. (2.7) at d = 1, 2, 3 (60, 420, 1380 rotations) with non-uniform prior weights
+    from emc_inputs import ladder_rotations
+
+    levels = [ladder_rotations(d, 7100 + d) for d in (1, 2, 3)]
+    assert [len(w) for _, w in levels] == [60, 420, 1380] and all(w.std() > 0.1 * w.mean() for _, w in levels)
     ref = o.refine(inp.model_init, inp.q, inp.mask, levels, inp.counts, 10, threshold)
     assert ref["level"].max() == 2                                      # the case does refine twice
     dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
