@@ -41,7 +41,7 @@ METRIC = "emc_iterations_per_s"
 UNIT = "iterations/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels, from the committed `ncu --set full`
 # captures (profiles/*.md name the commands); keyed "<config>:<stage>"
-TRAFFIC_FILE = ROOT / "profiles" / "ncu_dram_bytes_per_launch.json"
+TRAFFIC_FILE = ROOT / "profiles" / "r02_dram_traffic.csv"       # from the committed ncu capture (profiles/r02_full_ncu.md)
 
 
 def parse():
@@ -513,9 +513,10 @@ def main():
     dom = "update" if stage_ms["update"] >= stage_ms["loglik"] else "loglik"
     traffic, traffic_src = None, None
     if TRAFFIC_FILE.exists():
-        rec = json.loads(TRAFFIC_FILE.read_text()).get(f"{cfg.name}:{dom}")
-        if rec:
-            traffic, traffic_src = rec["bytes"], rec["source"]
+        for ln in TRAFFIC_FILE.read_text().splitlines()[1:]:
+            c_, s_, b_ = ln.split(",")
+            if c_ == cfg.name and s_ == dom:
+                traffic, traffic_src = float(b_), "profiles/r02_full_ncu.md (ncu --set full, dram read + write bytes per launch)"
     # tensor-core peak the chip has at the clock it held during this run (148 SMs x 8192 dense fp16 flops per clock)
     clock_peak = 148 * 8192 * clk["sm_mhz"] * 1e6 / 1e12 if clk.get("sm_mhz") else None
     roofline = dict(bound="tensor", kernel=f"plane_gemm_pair_kernel ({dom}, {stages[dom]['dtype']})",
