@@ -1,0 +1,52 @@
+"""emc_iterate inside a CUDA graph (`-m gpu`): the library creates no CUDA objects and never synchronises inside a hot call
+(include/emc.h, conventions), so a caller can capture the whole iteration -- every kernel and memset -- once and replay it.
+The replayed result must equal the eager one (bitwise up to the float32 atomics of Compress) and the oracle's."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import emc_oracle as o
+
+pytestmark = pytest.mark.gpu
+emc = pytest.importorskip("paper_1409_4256_b200")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+@pytest.mark.parametrize("name,n_iter", [("T1", 1), ("C1", 2)])
+def test_graph_replay_equals_eager(inputs_cache, name, n_iter):
+    inp = inputs_cache(name)
+    cfg = inp.cfg
+    d = [dev(inp.model_init), dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask), dev(inp.quat[0]), dev(inp.weight[0]),
+         dev(inp.counts)]
+    ws = emc.make_workspace(cfg.n, cfg.n_pix, inp.quat[0].shape[0], cfg.n_pat)
+    out_buf, ll = torch.empty_like(d[0]), torch.zeros(n_iter, dtype=torch.float64, device="cuda")
+    eager = emc.emc_iterate(*d, n_iter=n_iter, ws=ws)
+    m_eager, ll_eager = eager["model"].clone(), eager["loglik"].clone()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        emc.emc_iterate(*d, n_iter=n_iter, ws=ws, model_out=out_buf, loglik=ll)          # warm-up on the capture stream
+        with torch.cuda.graph(graph, stream=side):
+            emc.emc_iterate(*d, n_iter=n_iter, ws=ws, model_out=out_buf, loglik=ll)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        out_buf.zero_()
+        ll.zero_()
+        graph.replay()
+    torch.cuda.synchronize()
+    emc.emc_check(ws)
+    lg, le = ll.cpu().numpy(), ll_eager.cpu().numpy()
+    assert abs(lg[0] - le[0]) <= 1e-12 * abs(le[0])          # same kernels, same inputs, reproducible stages 1-3
+    assert np.allclose(lg, le, rtol=1e-6)                      # later iterations inherit the order of Compress's float32 atomics
+    m, me = out_buf.cpu().numpy().reshape(-1), m_eager.cpu().numpy().reshape(-1)
+    big = np.abs(me) >= 1e-3 * np.abs(me).max()
+    assert np.median(np.abs(m - me)[big] / np.abs(me)[big]) <= 1e-6 and np.array_equal(m == 0, me == 0)
+    ref = None
+    mo = inp.model_init
+    for _ in range(n_iter):
+        ref = o.iterate(mo, inp.q, inp.mask, inp.quat[0], inp.weight[0], inp.counts)
+        mo = ref["model"]
+    assert abs(float(ll.cpu()[-1]) - ref["LL"]) <= (1e-5 if n_iter == 1 else 1e-4) * abs(ref["LL"])
