@@ -52,7 +52,8 @@ typedef enum {
     EMC_ERR_UNSUPPORTED = -2,  /* a size outside what the kernels index (see each call) */
     EMC_ERR_WORKSPACE = -3,    /* ws is NULL, misaligned or smaller than emc_workspace_bytes() */
     EMC_ERR_CUDA = -4,         /* a CUDA runtime/driver call failed (emc_last_cuda_error()) */
-    EMC_ERR_COUNT_RANGE = -5   /* an unmasked photon count exceeds EMC_MAX_COUNT (emc_check) */
+    EMC_ERR_COUNT_RANGE = -5,  /* an unmasked photon count exceeds EMC_MAX_COUNT (emc_check) */
+    EMC_ERR_VALUE_RANGE = -6   /* emc_iterate_gaussian: an unmasked slice value >= 65504 (fp16 planes of W; emc_check) */
 } emc_status;
 
 typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
@@ -292,6 +293,7 @@ EMC_API emc_status emc_refine(const emc_model *model, const emc_detector *det, c
 
 /* Synchronises `stream` and reports what only the device saw during calls that used `ws`:
  * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (the results of that call are NaN),
+ * EMC_ERR_VALUE_RANGE if a slice of the Gaussian model left the fp16 range (its results hold inf / NaN),
  * EMC_ERR_CUDA if the stream is in error.  Clears the record. */
 EMC_API emc_status emc_check(void *ws, void *stream);
 

@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 EMC_OK = 0
-EMC_ERR_ARG, EMC_ERR_UNSUPPORTED, EMC_ERR_WORKSPACE, EMC_ERR_CUDA, EMC_ERR_COUNT_RANGE = -1, -2, -3, -4, -5
+EMC_ERR_ARG, EMC_ERR_UNSUPPORTED, EMC_ERR_WORKSPACE, EMC_ERR_CUDA, EMC_ERR_COUNT_RANGE, EMC_ERR_VALUE_RANGE = -1, -2, -3, -4, -5, -6
 EMC_I32, EMC_U16, EMC_U8 = 0, 1, 2
 EMC_MAX_COUNT = 2048
 EMC_COMPRESS_WEIGHTED = 0x1

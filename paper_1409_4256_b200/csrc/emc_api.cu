@@ -436,7 +436,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                 EMC_TRY(launch_transpose(l.Wnum, n_rot, n_pix, n_pix, l.logWT, l.ld_r, st));
             } else {
                 EMC_TRY(launch_expand(model_cur, n, det->q, det->mask, n_pix, rot->quat, n_rot, nullptr, nullptr,
-                                      l.planesL, l.ld_p, l.S, l.blocked, &geo, st, gauss));
+                                      l.planesL, l.ld_p, l.S, l.blocked, &geo, st, gauss, false, gauss ? &l.hdr->w_range : nullptr));
             }
         }
         EMC_TRY_CUDA(cudaMemsetAsync(l.s, 0, sizeof(float) * n_rot, st));
@@ -776,7 +776,8 @@ emc_status emc_check(void *ws, void *stream) {
     EMC_TRY_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
     EMC_TRY_CUDA(cudaMemcpy(&h, ws, sizeof(h), cudaMemcpyDeviceToHost));
     EMC_TRY_CUDA(cudaMemset(ws, 0, sizeof(h)));
-    return h.max_count > 0 ? EMC_ERR_COUNT_RANGE : EMC_OK;      // the pack kernel records only counts over its limit
+    if (h.max_count > 0) return EMC_ERR_COUNT_RANGE;            // the pack kernel records only counts over its limit
+    return h.w_range ? EMC_ERR_VALUE_RANGE : EMC_OK;
 }
 
 emc_status emc_profile_read(emc_context *c, double *ms, int *spans) {
@@ -805,6 +806,7 @@ const char *emc_strerror(emc_status s) {
         case EMC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case EMC_ERR_CUDA: return "CUDA error";
         case EMC_ERR_COUNT_RANGE: return "unmasked photon count above EMC_MAX_COUNT";
+        case EMC_ERR_VALUE_RANGE: return "slice value at or above 65504 in the Gaussian model (fp16 operand planes)";
     }
     return "unknown status";
 }

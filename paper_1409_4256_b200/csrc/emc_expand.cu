@@ -158,7 +158,8 @@ template <bool W_OUT, bool IDX_OUT, bool PLANES, bool LOGW32 = false>
 __global__ void __launch_bounds__(kThreads, 4)
 expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, const TileMap tm,
                       const float4 *__restrict__ rotm, int n_rot, int n_pix, float *__restrict__ W, int32_t *__restrict__ idx,
-                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S_part, int gauss) {
+                      __half *__restrict__ planes, int ld_p, size_t plane_stride, float *__restrict__ S_part, int gauss,
+                      int *__restrict__ w_range) {
     const int lane = threadIdx.x & 31;
     const int n_items = n_rot * tm.n_bands;
     for (int item = blockIdx.x * kWarps + (threadIdx.x >> 5); item < n_items; item += gridDim.x * kWarps) {
@@ -209,6 +210,7 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
                 if (IDX_OUT && in) i_row[pc] = s[j].base;
                 if (PLANES) {
                     __half hi, lo;
+                    if (gauss && use && w >= 65504.f && w_range) *w_range = 1;       // fp16 planes of W itself would hold inf
                     split_logw<true>(w, use && inside, hi, lo, gauss);
                     if (in) {
                         hi_row[pc] = hi;
@@ -285,7 +287,7 @@ size_t expand_scratch_floats(int n, int n_pix, int n_rot) {
 
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
-                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss, bool logw32) {
+                         int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss, bool logw32, int *w_range) {
     const int g = gauss ? 1 : 0;
     if (planes && !S) return EMC_ERR_ARG;
     if (blocked && geo) {
@@ -300,14 +302,14 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         const long long items = (long long)n_rot * tm.n_bands;
         const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
 #define EMC_EXPAND_CASE(w_, i_, p_)                                                                                   \
-    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g)
+    expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g, w_range)
         const int sel = (W ? 4 : 0) | (idx ? 2 : 0) | (planes ? 1 : 0);
         switch (sel) {
             case 1: EMC_EXPAND_CASE(false, false, true); break;
             case 2: EMC_EXPAND_CASE(false, true, false); break;
             case 4:
                 if (logw32)                                      // log W and S out instead of W
-                    expand_blocked_kernel<false, false, false, true><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g);
+                    expand_blocked_kernel<false, false, false, true><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g, w_range);
                 else
                     EMC_EXPAND_CASE(true, false, false);
                 break;

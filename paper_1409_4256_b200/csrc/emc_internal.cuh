@@ -41,7 +41,8 @@ static inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 // First 256 bytes of every workspace: what only the device can see (emc_check()).
 struct WsHeader {
     int max_count;   // largest unmasked photon count seen by the pack kernel
-    int pad[63];
+    int w_range;     // 1 if a slice value left the fp16 range of the Gaussian model's operand planes (>= 65504)
+    int pad[62];
 };
 static_assert(sizeof(WsHeader) == 256, "header is one 256-byte line");
 
@@ -85,7 +86,8 @@ size_t expand_scratch_floats(int n, int n_pix, int n_rot);
 emc_status launch_expand(const float *model, int n, const float *q, const uint8_t *mask, int n_pix,
                          const float *quat, int n_rot, float *W, int32_t *idx, __half *planes,
                          int ld_p, float *S, float *blocked, const Geometry *geo, cudaStream_t st, bool gauss = false,
-                         bool logw32 = false);
+                         bool logw32 = false, int *w_range = nullptr);
+// w_range (gauss): set to 1 if an unmasked slice value is >= 65504 (it would become inf in the fp16 planes of W)
 // logw32 (blocked path, W given, no idx / planes): W receives log(max(W, 1e-30)) as float32, 0 for masked / outside samples, and
 // S the row sums (operands of the photon-list log-likelihood, emc_sparse.cu)
 // logW planes + S from a given W (stage API of emc_loglik).

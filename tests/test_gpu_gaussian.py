@@ -108,3 +108,16 @@ def test_iterate_gaussian_pattern_chunks(inputs_cache, name, chunk):
         assert np.median(np.abs(m - m1)[cov] / (np.abs(m1[cov]) + 1e-6 * scale)) <= 1e-5
         rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
         assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2
+
+
+def test_gaussian_slice_range_is_reported(inputs_cache):
+    """Slices at or above 65504 do not fit the fp16 planes of W: emc_check says so instead of letting inf / NaN pass."""
+    inp = inputs_cache("T1")
+    args = [dev(inp.model_init * np.float32(1e9 / inp.model_init.max())), dev(inp.q), dev(inp.mask), dev(inp.quat[0]),
+            dev(inp.weight[0]), dev(inp.counts)]
+    out = emc.emc_iterate_gaussian(*args, 10.0)
+    with pytest.raises(emc.EmcError) as e:
+        emc.emc_check(out["ws"])
+    assert e.value.status == emc.EMC_ERR_VALUE_RANGE
+    ok = emc.emc_iterate_gaussian(dev(inp.model_init), *args[1:], 10.0, ws=out["ws"])
+    emc.emc_check(ok["ws"])                                   # the record is cleared by the check and by the next call
