@@ -80,6 +80,7 @@ struct Layout {
     float *logWT;             // [P][ld_r]     log W transposed
     float *LT;                // [Nc][ld_r]    L transposed, then P transposed
     float *WT;                // [P][ld_r]     update numerators transposed
+    float *logw;              // [ld_r]        log of the prior weights
     int *list_pat, *list_pix; // photon lists by frame and by pixel (sparse_list_ints)
     int ld_p, ld_n, ld_r;
     size_t total;
@@ -114,10 +115,11 @@ Layout carve(void *ws, int n, int n_pix, int n_rot, int n_chunk, size_t stage_by
         l.logWT = a.take<float>((size_t)n_pix * l.ld_r);
         l.LT = a.take<float>((size_t)n_chunk * l.ld_r);
         l.WT = a.take<float>((size_t)n_pix * l.ld_r);
+        l.logw = a.take<float>((size_t)l.ld_r);
         l.list_pat = a.take<int>(sparse_list_ints(n_chunk, cap));
         l.list_pix = a.take<int>(sparse_list_ints(n_pix, cap));
     } else {
-        l.logWT = l.LT = l.WT = nullptr;
+        l.logWT = l.LT = l.WT = l.logw = nullptr;
         l.list_pat = l.list_pix = nullptr;
     }
     l.total = a.off;
@@ -424,6 +426,7 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     const float *model_cur = model->model;
     Geometry geo;                                            // once per call: the rotation list is the same in every iteration
     EMC_TRY(launch_geometry(det->q, det->mask, n_pix, det->row_len, rot->quat, n_rot, l.geom, &geo, st));
+    if (sparse && rot->weight) EMC_TRY(launch_logw(rot->weight, n_rot, l.logw, st));
     for (int it = 0; it < n_iter; ++it) {
         // stage 1: Expand, with logW planes and S fused in
         {
@@ -467,13 +470,11 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                     EMC_TRY_CUDA(cudaStreamWaitEvent(st, ctx->ready[b], 0));
                     src = (const uint8_t *)l.stage + b * stage_one;
                 }
-                EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, l.ld_n, l.hdr, st));
+                if (sparse)                         // photon lists by frame and by pixel, straight from the raw counts
+                    EMC_TRY(launch_lists_raw(src, pat->type, nc, n_pix, det->mask, l.list_pat, l.list_pix, l.hdr, &by_frame, &by_pixel, st));
+                else
+                    EMC_TRY(launch_pack(src, pat->type, nc, n_pix, det->mask, v.Kc, l.ld_p, v.KT, l.ld_n, l.hdr, st));
                 if (on_host) EMC_TRY_CUDA(cudaEventRecord(ctx->freed[job & 1], st));
-                if (sparse) {                       // photon lists by frame (rows of Kc) and by pixel (rows of KT)
-                    const size_t cap = (size_t)chunk * n_pix;
-                    EMC_TRY(launch_sparsify(v.Kc, nc, n_pix, l.ld_p, l.list_pat, cap, &by_frame, st));
-                    EMC_TRY(launch_sparsify(v.KT, n_pix, nc, l.ld_n, l.list_pix, cap, &by_pixel, st));
-                }
                 if (gauss) {                        // A_d = sum_p K^2, the numerators of the fluence (eq. 2.6)
                     EMC_TRY_CUDA(cudaMemsetAsync(l.Asq, 0, sizeof(float) * 2 * l.ld_n, st));
                     EMC_TRY(launch_rowsq(l.Kc, nc, n_pix, l.ld_p, gterms.inv2s2, l.Asq, l.Asq + l.ld_n, st));
@@ -481,21 +482,18 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
                 ++job;
             }
             if (sparse) {
-                // stages 2-4 from the photon lists, in the transposed world (emc_sparse.cu)
-                float *p_buf = (P_out && it == n_iter - 1) ? P_out : reinterpret_cast<float *>(l.planesP);   // [R][ld_n] float32
+                // stages 2-4 from the photon lists, in the transposed world (emc_sparse.cu): L^T, P^T, W'^T
                 {
                     Span sp(ctx, prof, EMC_STAGE_LOGLIK, st);
                     EMC_TRY(launch_spmm_rot(by_frame, l.logWT, l.LT, l.ld_r, n_rot, l.S, false, st));
-                    EMC_TRY(launch_transpose(l.LT, nc, n_rot, l.ld_r, l.L, l.ld_n, st));
                 }
                 {
                     Span sp(ctx, prof, EMC_STAGE_NORMALIZE, st);
-                    EMC_TRY(launch_normalize(l.L, rot->weight, n_rot, nc, l.ld_n, p_buf, nullptr, 0, nullptr, l.s, loglik + it, true,
-                                             l.scratch, false, st, nullptr, 0, log_uniform));
+                    EMC_TRY(launch_softmax_rows(l.LT, nc, n_rot, l.ld_r, rot->weight ? l.logw : nullptr, log_uniform, l.s, loglik + it, st));
+                    if (P_out && it == n_iter - 1) EMC_TRY(launch_transpose(l.LT, nc, n_rot, l.ld_r, P_out, l.ld_n, st));
                 }
                 {
                     Span sp(ctx, prof, EMC_STAGE_UPDATE, st);
-                    EMC_TRY(launch_transpose(p_buf, n_rot, nc, l.ld_n, l.LT, l.ld_r, st));
                     EMC_TRY(launch_spmm_rot(by_pixel, l.LT, l.WT, l.ld_r, n_rot, nullptr, c > 0, st));
                 }
                 continue;

@@ -210,9 +210,15 @@ struct SparseList {
     int rows;
 };
 size_t sparse_list_ints(int rows, size_t max_entries);   // ints of scratch behind a SparseList
-// CSR of the nonzeros of A [rows][ld] fp16 (cols < 2^20)
-emc_status launch_sparsify(const __half *A, int rows, int cols, int ld, int *lists, size_t max_entries, SparseList *out,
-                           cudaStream_t st);
+// both lists straight from the raw counts [rows = frames][cols = pixels] (masked pixels skipped; an unmasked count above
+// EMC_MAX_COUNT recorded in hdr); list_pat / list_pix = sparse_list_ints(rows, rows x cols) / (cols, rows x cols) ints
+emc_status launch_lists_raw(const void *counts, emc_count_type type, int rows, int cols, const uint8_t *mask, int *list_pat,
+                            int *list_pix, WsHeader *hdr, SparseList *by_frame, SparseList *by_pixel, cudaStream_t st);
+// rows of L^T [rows][ld] -> rows of P^T in place (soft-max over the n_rot rotations of a row with log weights logw [n_rot] or
+// null = uniform, every log w = log_uniform); s[r] += column sums; loglik += total
+emc_status launch_softmax_rows(float *LT, int rows, int n_rot, int ld, const float *logw, float log_uniform, float *s,
+                               double *loglik, cudaStream_t st);
+emc_status launch_logw(const float *weight, int n_rot, float *out, cudaStream_t st);
 // Y [rows][ld] = A X (- sub_row) (+ Y), X [K][ld], the first n_rot columns
 emc_status launch_spmm_rot(const SparseList &a, const float *X, float *Y, int ld, int n_rot, const float *sub_row,
                            bool accumulate, cudaStream_t st);
