@@ -407,6 +407,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if args.cuda_graph:
         # the library creates nothing and never synchronises inside emc_iterate: the step is capturable as it is
+        torch.cuda.synchronize()        # the workspace moves to another stream: the warm-up steps are over first
         side = torch.cuda.Stream()
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.stream(side):

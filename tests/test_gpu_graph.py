@@ -25,6 +25,7 @@ def test_graph_replay_equals_eager(inputs_cache, name, n_iter):
     out_buf, ll = torch.empty_like(d[0]), torch.zeros(n_iter, dtype=torch.float64, device="cuda")
     eager = emc.emc_iterate(*d, n_iter=n_iter, ws=ws)
     m_eager, ll_eager = eager["model"].clone(), eager["loglik"].clone()
+    torch.cuda.synchronize()            # one workspace serves one stream at a time: the eager run is over before `side` starts
     side = torch.cuda.Stream()
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.stream(side):
