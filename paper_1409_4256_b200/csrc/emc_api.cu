@@ -811,6 +811,6 @@ const char *emc_strerror(emc_status s) {
 
 const char *emc_last_cuda_error(void) { return g_err; }
 
-const char *emc_version(void) { return "libemc 0.2 (sm_100a)"; }
+const char *emc_version(void) { return "libemc 0.3 (sm_100a)"; }
 
 }  // extern "C"

@@ -225,6 +225,7 @@ emc_status launch_compress(const float *Wnew, const float *slice_w, bool weighte
     const int w = weighted ? 1 : 0;
     const TileMap tm = make_tile_map(n_pix, geo.row_len);
     const long long items = (long long)n_rot * tm.n_bands;
+    if (items > 0x7fffffffLL) return EMC_ERR_UNSUPPORTED;          // the kernel counts work items in 32 bits
     const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
     if (phases != COMPRESS_ALL) {
         if (phases & COMPRESS_CLEAR) EMC_TRY_CUDA(cudaMemsetAsync(acc4, 0, g * 8 * sizeof(float2), st));

@@ -300,6 +300,7 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
         // band partials of S live behind the corner blocks (expand_scratch_floats)
         float *S_part = blocked + (size_t)8 * n * n * n;
         const long long items = (long long)n_rot * tm.n_bands;
+        if (items > 0x7fffffffLL) return EMC_ERR_UNSUPPORTED;      // the kernels count work items in 32 bits
         const int grid = (int)std::min<long long>((items + kWarps - 1) / kWarps, (long long)1 << 30);
 #define EMC_EXPAND_CASE(w_, i_, p_)                                                                                   \
     expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g, w_range)
