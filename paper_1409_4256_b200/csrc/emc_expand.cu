@@ -154,7 +154,8 @@ geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, i
 // (bitwise reproducible S, no atomics).
 constexpr int kWarps = kThreads / 32;
 // LOGW32 (photon-list path): W receives log W as float32 (0 for masked / outside samples) and S the row sums
-template <bool W_OUT, bool IDX_OUT, bool PLANES, bool LOGW32 = false>
+// GAUSS: the planes hold W itself (Gaussian model); a compile-time switch so that the Poisson path pays nothing for it
+template <bool W_OUT, bool IDX_OUT, bool PLANES, bool LOGW32 = false, bool GAUSS = false>
 __global__ void __launch_bounds__(kThreads, 4)
 expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *__restrict__ qm, const TileMap tm,
                       const float4 *__restrict__ rotm, int n_rot, int n_pix, float *__restrict__ W, int32_t *__restrict__ idx,
@@ -210,14 +211,14 @@ expand_blocked_kernel(const float4 *__restrict__ blocked, int n, const float4 *_
                 if (IDX_OUT && in) i_row[pc] = s[j].base;
                 if (PLANES) {
                     __half hi, lo;
-                    if (gauss && use && w >= 65504.f && w_range) *w_range = 1;       // fp16 planes of W itself would hold inf
-                    split_logw<true>(w, use && inside, hi, lo, gauss);
+                    if (GAUSS && use && w >= 65504.f && w_range) *w_range = 1;       // fp16 planes of W itself would hold inf
+                    split_logw<true>(w, use && inside, hi, lo, GAUSS ? 1 : 0);
                     if (in) {
                         hi_row[pc] = hi;
                         lo_row[pc] = lo;
                     }
                 }
-                part += use ? (gauss ? w * w : w) : 0.f;
+                part += use ? (GAUSS ? w * w : w) : 0.f;
             }
         }
         if (PLANES || LOGW32) {                              // S accompanies the log-likelihood operands
@@ -306,7 +307,12 @@ emc_status launch_expand(const float *model, int n, const float *q, const uint8_
     expand_blocked_kernel<w_, i_, p_><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g, w_range)
         const int sel = (W ? 4 : 0) | (idx ? 2 : 0) | (planes ? 1 : 0);
         switch (sel) {
-            case 1: EMC_EXPAND_CASE(false, false, true); break;
+            case 1:
+                if (gauss)
+                    expand_blocked_kernel<false, false, true, false, true><<<grid, kThreads, 0, st>>>(b4, n, geo->qm, tm, geo->rotm, n_rot, n_pix, W, idx, planes, ld_p, ps, S_part, g, w_range);
+                else
+                    EMC_EXPAND_CASE(false, false, true);
+                break;
             case 2: EMC_EXPAND_CASE(false, true, false); break;
             case 4:
                 if (logw32)                                      // log W and S out instead of W

@@ -85,8 +85,8 @@ __device__ __forceinline__ Sample locate(const float *__restrict__ m, float qx, 
 // length is known, 1 x 32 otherwise), so that its 32 samples cover a compact patch of the slice.  Work is handed out
 // to warps in BANDS: one tile row (TH detector rows), cut into segments of at most kMaxTilesPerBand tiles; a warp walks
 // along its band kTilesPerStep tiles at a time.  Any row_len gives the same results; only locality changes.
-constexpr int kTilesPerStep = 4;
-constexpr int kMaxTilesPerBand = 4;       // measured at C2: 4 (one step per item) 127 us, 8: 207 us, 32 with 6 blocks per SM: 258 us
+constexpr int kTilesPerStep = 4;           // measured at C2: 4 tiles per step (64 registers) 130 us, 2 (40-48 registers) 137-139 us, 1: 178 us
+constexpr int kMaxTilesPerBand = 4;        // measured at C2: 4 (one step per item) 127-130 us, 8: 207 us, 32 with 6 blocks per SM: 258 us
 struct TileMap {
     int row_len, n_rows, n_tx, n_seg, n_bands, tw_shift, th;
 };
