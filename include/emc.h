@@ -53,7 +53,8 @@ typedef enum {
     EMC_ERR_WORKSPACE = -3,    /* ws is NULL, misaligned or smaller than emc_workspace_bytes() */
     EMC_ERR_CUDA = -4,         /* a CUDA runtime/driver call failed (emc_last_cuda_error()) */
     EMC_ERR_COUNT_RANGE = -5,  /* an unmasked photon count exceeds EMC_MAX_COUNT (emc_check) */
-    EMC_ERR_VALUE_RANGE = -6   /* emc_iterate_gaussian: an unmasked slice value >= 65504 (fp16 planes of W; emc_check) */
+    EMC_ERR_VALUE_RANGE = -6,  /* emc_iterate_gaussian: an unmasked slice value >= 65504 (fp16 planes of W; emc_check) */
+    EMC_ERR_STATIC_SCRATCH = -7 /* emc_normalize_static: these sizes need more than EMC_STATIC_SCRATCH_BYTES */
 } emc_status;
 
 typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
@@ -168,6 +169,39 @@ EMC_API emc_status emc_loglik(const float *W, const int32_t *idx, const emc_dete
 EMC_API emc_status emc_normalize(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
                          float *s, double *loglik, unsigned flags, void *ws, size_t ws_bytes,
                          void *stream);
+
+/* Stage 3 again, for callers that have no device memory to hand over as a workspace and no way to get any.
+ *
+ * Who that is: code that runs where cudaMalloc is off limits or already spent -- a plug-in inside a host
+ * application that gave it fixed input / output buffers and nothing else, a real-time acquisition loop at the
+ * beamline that must not touch the allocator (cudaMalloc takes a device-wide lock and can stall every stream for
+ * milliseconds), a process whose memory pool has been handed out in full to the experiment's frames.  Every other
+ * call of this header takes its scratch from the caller's `ws`; this one brings its own.
+ *
+ * Same arithmetic, same kernels, same results as emc_normalize (P bit for bit; s and loglik up to the order of
+ * their atomic additions).  The per-pattern partial statistics of the first sweep live in ONE array of
+ * EMC_STATIC_SCRATCH_BYTES that is compiled into the library as a `static __device__` object: every GPU that
+ * loads libemc holds these 4 MiB from then until the process exits, whether this call is ever used or not.
+ *
+ *   Arguments as emc_normalize, without ws / ws_bytes.  L, P, s, loglik are the caller's device buffers.
+ *   Limit: emc_normalize_static_bytes(n_rot, n_pat, ld_n) <= EMC_STATIC_SCRATCH_BYTES, else the call returns
+ *     EMC_ERR_STATIC_SCRATCH and enqueues nothing.  The need is (3 * row_splits + 3) * ld_n floats with
+ *     row_splits <= 64 shrinking as n_pat grows; every n_pat up to 100 000 fits for any n_rot (all of
+ *     Table 4.1's pattern counts per chunk).
+ *   The call itself never calls cudaMalloc, cudaFree or any library routine that allocates.
+ *   First call on a device: looks up the device address of the array (cudaGetSymbolAddress, with the device that
+ *     owns `stream` current -- the caller makes it current, as for every other call) and keeps it for later calls on
+ *     that device.  Make that first call outside any stream capture.
+ *   One array per device, shared by every call in the process: two emc_normalize_static calls whose kernels can
+ *     overlap on the GPU (different streams, or different host threads on different streams) race on it and
+ *     produce garbage.  Keep them on one stream, or order them with events.  The array keeps whatever the last
+ *     call left; nothing in it has to start at zero, because every value a call reads it has written itself
+ *     earlier in the same call (s and loglik are cleared by the call unless EMC_ACCUMULATE is set). */
+#define EMC_STATIC_SCRATCH_BYTES (4u << 20)
+/* bytes of the built-in array a call at these sizes uses; 0 on invalid sizes */
+EMC_API size_t emc_normalize_static_bytes(int n_rot, int n_pat, int ld_n);
+EMC_API emc_status emc_normalize_static(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P,
+                                float *s, double *loglik, unsigned flags, void *stream);
 
 /* Stage 4, slice update (M-step), eq. (2.5) with phi == 1 / eq. (2.11), PAPER.md:84-85, 124-125:
  *   Wnew[r,p] = sum_d P[r,d] K[d,p] / s[r]   for unmasked p, 0 for masked p and where s[r] = 0.

@@ -16,6 +16,8 @@ from . import build as _build
 
 EMC_OK = 0
 EMC_ERR_ARG, EMC_ERR_UNSUPPORTED, EMC_ERR_WORKSPACE, EMC_ERR_CUDA, EMC_ERR_COUNT_RANGE, EMC_ERR_VALUE_RANGE = -1, -2, -3, -4, -5, -6
+EMC_ERR_STATIC_SCRATCH = -7
+EMC_STATIC_SCRATCH_BYTES = 4 << 20
 EMC_I32, EMC_U16, EMC_U8 = 0, 1, 2
 EMC_MAX_COUNT = 2048
 EMC_COMPRESS_WEIGHTED = 0x1
@@ -31,7 +33,7 @@ STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
-           "emc_normalize", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
+           "emc_normalize", "emc_normalize_static", "emc_normalize_static_bytes", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
            "emc_workspace_bytes_rot_chunked", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_loglik_gaussian", "emc_refine", "emc_check",
            "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
@@ -89,6 +91,10 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_loglik.argtypes = [vp, vp, POINTER(_Detector), POINTER(_Patterns), ci, vp, ci, cu, vp, sz, vp]
     lib.emc_normalize.restype = ci
     lib.emc_normalize.argtypes = [vp, POINTER(_Rotations), ci, ci, vp, vp, vp, cu, vp, sz, vp]
+    lib.emc_normalize_static_bytes.restype = sz
+    lib.emc_normalize_static_bytes.argtypes = [ci, ci, ci]
+    lib.emc_normalize_static.restype = ci
+    lib.emc_normalize_static.argtypes = [vp, POINTER(_Rotations), ci, ci, vp, vp, vp, cu, vp]
     lib.emc_update.restype = ci
     lib.emc_update.argtypes = [vp, ci, vp, POINTER(_Detector), POINTER(_Patterns), ci, vp, cu, vp, sz, vp]
     lib.emc_compress.restype = ci
@@ -302,6 +308,23 @@ def emc_normalize(big_l, quat, weight, flags=0, s=None, loglik=None, ws=None):
     _check(load().emc_normalize(lp, rot, n_pat, ld, p.data_ptr(), s.data_ptr(), loglik.data_ptr(), flags, wp, wb,
                                 _stream()), "emc_normalize")
     return p[:, :n_pat], s, loglik
+
+
+def emc_normalize_static(big_l, quat, weight, p_out, s_out=None, loglik_out=None, flags=0):
+    """Stage 3 without a workspace, for callers that cannot allocate device memory (include/emc.h,
+    emc_normalize_static): the scratch is an array built into libemc.  Unlike the other wrappers this one creates no
+    tensor: the caller passes L and every output -- p_out a [R, N] float32 view with the row pitch of L, s_out [R]
+    float32 or None, loglik_out one float64 or None -- and gets nothing back.  Raises EmcError
+    (EMC_ERR_STATIC_SCRATCH) when the sizes exceed the built-in array.  Calls that may overlap on the GPU race on
+    that array: keep them on one stream."""
+    n_rot, n_pat = big_l.shape
+    lp, ld = _pitched(big_l, "L")
+    pp, ldp = _pitched(p_out, "P")
+    if tuple(p_out.shape) != (n_rot, n_pat) or ldp != ld:
+        raise ValueError("p_out: expected the shape and row pitch of L")
+    rot = _rotations(quat, weight)
+    _check(load().emc_normalize_static(lp, rot, n_pat, ld, pp, _opt(s_out, torch.float32, "s"),
+                                       _opt(loglik_out, torch.float64, "loglik"), flags, _stream()), "emc_normalize_static")
 
 
 def emc_update(p, s, q, mask, counts, flags=0, wnew=None, ws=None):

@@ -805,6 +805,9 @@ const char *emc_strerror(emc_status s) {
         case EMC_ERR_CUDA: return "CUDA error";
         case EMC_ERR_COUNT_RANGE: return "unmasked photon count above EMC_MAX_COUNT";
         case EMC_ERR_VALUE_RANGE: return "slice value at or above 65504 in the Gaussian model (fp16 operand planes)";
+        case EMC_ERR_STATIC_SCRATCH:
+            return "emc_normalize_static: these sizes need more than the EMC_STATIC_SCRATCH_BYTES built into the library "
+                   "(see emc_normalize_static_bytes); use emc_normalize with a workspace";
     }
     return "unknown status";
 }

@@ -11,6 +11,8 @@
 //     partials per column and adds up the total log-likelihood.
 // (2) normalize_kernel reads L once and writes P, its operand planes for the update GEMM and s[r] = sum_d P[r,d].
 // HBM-bound: 8 algorithmic bytes per (r,d).
+#include <atomic>
+
 #include "emc_internal.cuh"
 
 namespace emc {
@@ -584,3 +586,112 @@ emc_status launch_div_rows(float *Wnew, const float *s, int n_rot, int n_pix, cu
 }
 
 }  // namespace emc
+
+// ---------------------------------------------------------------- emc_normalize_static (include/emc.h)
+// Stage 3 for callers that cannot allocate device memory (a plug-in with fixed buffers, an acquisition loop that must
+// stay off the allocator's device-wide lock, a process whose pool is spent): the partial column statistics of the
+// first sweep live in an array that is part of the library image instead of the caller's workspace.  The array costs
+// EMC_STATIC_SCRATCH_BYTES on every GPU that loads libemc, for the life of the process.  The kernels are the ones
+// emc_normalize runs (colstats_kernel, colstats_combine_kernel, normalize_kernel), with the same row splits.
+//
+// `emc_static_scratch` below is a device object.  On the host its name is only a handle for the runtime's symbol
+// table -- passing it to a kernel would hand the kernel a host address -- so the host asks the runtime once per device
+// where the object lives (cudaGetSymbolAddress, that device current) and passes THAT pointer.
+static __device__ __align__(256) float emc_static_scratch[EMC_STATIC_SCRATCH_BYTES / sizeof(float)];
+
+namespace emc {
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::atomic<float *> g_static_scratch_addr[kMaxDevices];   // device address of emc_static_scratch, per device ordinal
+
+// Address of the array on the current device.  The first call on a device does the look-up (the documented set-up
+// step: outside stream capture); two threads racing here both obtain the same address, so a plain store suffices.
+emc_status static_scratch_on_current_device(float **out) {
+    int dev = -1;
+    EMC_TRY_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return EMC_ERR_UNSUPPORTED;
+    float *p = g_static_scratch_addr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        void *sym = nullptr;
+        EMC_TRY_CUDA(cudaGetSymbolAddress(&sym, emc_static_scratch));
+        if (!sym || ((uintptr_t)sym & 255)) return EMC_ERR_CUDA;
+        p = (float *)sym;
+        g_static_scratch_addr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return EMC_OK;
+}
+
+// the row splits launch_normalize takes when the statistics do not come from the GEMM, and the floats they need:
+// three partial arrays [n_splits][ld_n] and the three combined column arrays [ld_n]
+struct StaticPlan {
+    int col_blocks, rows_per_split, n_splits;
+    size_t floats;
+};
+bool static_plan(int n_rot, int n_pat, int ld_n, StaticPlan *pl) {
+    if (n_rot <= 0 || n_pat <= 0 || ld_n < n_pat || (ld_n & 3)) return false;
+    pl->col_blocks = ceil_div(n_pat, kColsPerBlock);
+    const int splits = row_splits_for(n_rot, pl->col_blocks);
+    pl->rows_per_split = ceil_div(n_rot, splits);
+    pl->n_splits = ceil_div(n_rot, pl->rows_per_split);
+    pl->floats = (size_t)(3 * pl->n_splits + 3) * (size_t)ld_n;
+    return true;
+}
+
+}  // namespace
+}  // namespace emc
+
+extern "C" {
+
+size_t emc_normalize_static_bytes(int n_rot, int n_pat, int ld_n) {
+    emc::StaticPlan pl;
+    return emc::static_plan(n_rot, n_pat, ld_n, &pl) ? pl.floats * sizeof(float) : 0;
+}
+
+emc_status emc_normalize_static(const float *L, const emc_rotations *rot, int n_pat, int ld_n, float *P, float *s,
+                                double *loglik, unsigned flags, void *stream) {
+    using namespace emc;
+    StaticPlan pl;
+    if (!L || !rot || !P || ((uintptr_t)L & 15) || ((uintptr_t)P & 15) || !static_plan(rot->n_rot, n_pat, ld_n, &pl))
+        return EMC_ERR_ARG;
+    if (pl.floats * sizeof(float) > EMC_STATIC_SCRATCH_BYTES) return EMC_ERR_STATIC_SCRATCH;   // nothing enqueued
+    float *scratch = nullptr;
+    EMC_TRY(static_scratch_on_current_device(&scratch));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n_rot = rot->n_rot;
+    const float *weight = rot->weight;
+    const size_t plane = (size_t)pl.n_splits * ld_n;
+    float *part_m = scratch, *part_w = part_m + plane, *part_z = part_w + plane;
+    float *col_m = part_z + plane, *col_w = col_m + ld_n, *col_iz = col_w + ld_n;
+    // results the kernels add into start at zero; the scratch needs no clearing (every element read below is written
+    // by the kernel before it: partials for d < n_pat and k < n_splits, column arrays up to ld_n)
+    if (!(flags & EMC_ACCUMULATE)) {
+        if (s) EMC_TRY_CUDA(cudaMemsetAsync(s, 0, sizeof(float) * n_rot, st));
+        if (loglik) EMC_TRY_CUDA(cudaMemsetAsync(loglik, 0, sizeof(double), st));
+    }
+    colstats_kernel<<<dim3(pl.col_blocks, pl.n_splits), kThreads, 0, st>>>(L, weight, log_uniform_of(n_rot), n_rot, n_pat, ld_n,
+                                                                           pl.rows_per_split, part_m, part_w, part_z);
+    EMC_LAUNCHED();
+    colstats_combine_kernel<<<ceil_div(ld_n, 32), 256, 0, st>>>(part_m, part_w, part_z, n_pat, ld_n, ld_n, pl.n_splits, col_m, col_w,
+                                                               col_iz, loglik, -1, 0);
+    EMC_LAUNCHED();
+    // second sweep: the grid emc_normalize uses (512-column chunks, at most 6 x 148 blocks)
+    const int chunks = ceil_div(n_pat, kChunkCols);
+    int splits2 = (6 * 148) / chunks;
+    const int cap2 = ceil_div(n_rot, 4 * kWarps);
+    if (splits2 > cap2) splits2 = cap2;
+    if (splits2 < 1) splits2 = 1;
+    const int rows2 = ceil_div(n_rot, splits2);
+    const dim3 grid2(chunks, ceil_div(n_rot, rows2));
+    if (weight)
+        normalize_kernel<false><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, ld_n, rows2, col_m, col_w, col_iz, P,
+                                                            nullptr, 0, nullptr, s);
+    else
+        normalize_kernel<true><<<grid2, kThreads, 0, st>>>(L, weight, n_rot, n_pat, ld_n, ld_n, rows2, col_m, col_w, col_iz, P,
+                                                           nullptr, 0, nullptr, s);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
+
+}  // extern "C"
