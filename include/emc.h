@@ -82,8 +82,9 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
 #define EMC_SPARSE_PHOTONS    0x40u /* emc_iterate (Poisson model): stages 2 and 4 from per-frame / per-pixel photon lists on
                                       plain CUDA cores instead of the dense tensor-core contractions; for frames that
                                       are almost empty (DESIGN.md section 11 NEXT-2 has the measured crossover).  Needs
-                                      n_pix and the pattern chunk below 2^20; the workspace grows (pass the flag to
-                                      emc_workspace_bytes). */
+                                      n_pix and the pattern chunk below 2^20 and their product below 2^31 (32-bit list
+                                      offsets), else EMC_ERR_UNSUPPORTED; the workspace grows (pass the flag to
+                                      emc_workspace_bytes).  Not taken by emc_iterate_rot_chunked (EMC_ERR_UNSUPPORTED). */
 #define EMC_GEMM_1CTA         0x200u /* run the two contractions with one CTA per tile (cta_group::1)
                                         instead of CTA pairs (cta_group::2); a comparison / bisecting aid */
 #define EMC_DEBUG_SIMT        0x100u /* run the two contractions on plain CUDA cores (slow; a
@@ -242,6 +243,19 @@ EMC_API emc_status emc_iterate(const emc_model *model, const emc_detector *det, 
                        float *P_out, int ld_n, double *loglik, unsigned flags, void *ws,
                        size_t ws_bytes, void *stream, emc_context *ctx);
 
+/* Where emc_iterate / emc_iterate_gaussian left its intermediate results inside the caller's workspace: pointer
+ * arithmetic on the host, nothing is enqueued.  For checking the product path itself (tests/): the log-likelihood matrix
+ * that the fused Expand (logW operand planes formed in registers) and the contraction produced, which no stage call
+ * returns, and the slices W' and their weights s that went into Compress.  Sizes and flags as passed to the emc_iterate
+ * call that used `ws`.  Valid after that call's work on its stream has finished and until the next call that uses `ws`;
+ * with several pattern chunks the per-chunk buffers hold the LAST chunk of the last iteration.
+ *   what = EMC_VIEW_LOGLIK: *ptr = L [R][*ld] float (Gaussian model: B = W K^T); not with EMC_SPARSE_PHOTONS
+ *          EMC_VIEW_S:      *ptr = s [R] float, *ld = 0
+ *          EMC_VIEW_WNEW:   *ptr = W' [R][*ld] float, *ld = n_pix */
+enum { EMC_VIEW_LOGLIK = 0, EMC_VIEW_S = 1, EMC_VIEW_WNEW = 2 };
+EMC_API emc_status emc_workspace_view(void *ws, int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags, int what,
+                              void **ptr, int *ld);
+
 /* Algorithm 1 with the ROTATION list streamed in chunks of n_rot_chunk rotations, the paper's own memory scheme
  * ("chunk C_c"; "only maximal rotational probabilities and sums are necessary", PAPER.md:203;
  * DESIGN.md section 11 NEXT-2): nothing of size R x N or R x P is held, the workspace scales with the chunk.  Two
@@ -271,7 +285,9 @@ EMC_API emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_det
  *   (all-reduce(sum) of numden_out over the ranks)
  *   emc_shard_finish  model_out = num / den (division as the final step).
  * The workspace (emc_workspace_bytes for the rank's rotation count and all N patterns) carries L and the packed
- * patterns from emc_shard_stats to emc_shard_update: same ws, same stream, nothing else in between.
+ * patterns from emc_shard_stats to emc_shard_update: same ws, same stream, nothing else in between.  emc_shard_stats
+ * stamps the workspace header with its sizes and emc_shard_update checks the stamp on the device: with a workspace that
+ * does not come from a matching emc_shard_stats its results are NaN and emc_check returns EMC_ERR_WORKSPACE.
  * n_rot_total = R of the whole list (log(1/R) for weight == NULL).  world <= 64.  Poisson model, device patterns. */
 EMC_API emc_status emc_shard_stats(const emc_model *model, const emc_detector *det, const emc_rotations *rot_local,
                            const emc_patterns *pat, int n_rot_total, float *stats_out, unsigned flags, void *ws,
@@ -328,7 +344,8 @@ EMC_API emc_status emc_refine(const emc_model *model, const emc_detector *det, c
 /* Synchronises `stream` and reports what only the device saw during calls that used `ws`:
  * EMC_ERR_COUNT_RANGE if an unmasked count exceeded EMC_MAX_COUNT (the results of that call are NaN),
  * EMC_ERR_VALUE_RANGE if a slice of the Gaussian model left the fp16 range (its results hold inf / NaN),
- * EMC_ERR_CUDA if the stream is in error.  Clears the record. */
+ * EMC_ERR_WORKSPACE if emc_shard_update found a workspace that no matching emc_shard_stats had prepared (results NaN),
+ * EMC_ERR_CUDA if the stream is in error.  Reads and clears the record on `stream` itself. */
 EMC_API emc_status emc_check(void *ws, void *stream);
 
 /* Stages timed under EMC_PROFILE_STAGES (at most EMC_MAX_SPANS spans between reads; later ones are dropped). */
@@ -338,6 +355,9 @@ enum { EMC_STAGE_EXPAND = 0, EMC_STAGE_PACK = 1, EMC_STAGE_LOGLIK = 2, EMC_STAGE
 /* Waits for the recorded events, returns per stage the summed device time in milliseconds (HOST
  * array ms[EMC_N_STAGES]) and the number of spans (HOST array spans[EMC_N_STAGES]), and resets. */
 EMC_API emc_status emc_profile_read(emc_context *ctx, double *ms, int *spans);
+/* Spans that found the pool of EMC_MAX_SPANS event pairs exhausted since the last call of this function (their time is
+ * missing from emc_profile_read's sums: read more often, e.g. once per emc_iterate_rot_chunked iteration); resets the count. */
+EMC_API int emc_profile_dropped(emc_context *ctx);
 
 /* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
 EMC_API uint64_t emc_launch_count(void);

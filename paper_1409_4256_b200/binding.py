@@ -29,13 +29,14 @@ EMC_SPARSE_PHOTONS = 0x40
 EMC_DEBUG_SIMT = 0x100
 EMC_GEMM_1CTA = 0x200
 EMC_MAX_SPANS = 4096
+EMC_VIEW_LOGLIK, EMC_VIEW_S, EMC_VIEW_WNEW = 0, 1, 2
 STAGES = ("expand", "pack", "loglik", "normalize", "update", "compress")
 
 # every symbol include/emc.h declares (tests check the library exports all of them)
 SYMBOLS = ("emc_context_create", "emc_context_destroy", "emc_workspace_bytes", "emc_workspace_bytes_geometry", "emc_expand", "emc_loglik",
            "emc_normalize", "emc_normalize_static", "emc_normalize_static_bytes", "emc_update", "emc_compress", "emc_iterate", "emc_iterate_rot_chunked",
-           "emc_workspace_bytes_rot_chunked", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_loglik_gaussian", "emc_refine", "emc_check",
-           "emc_profile_read", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
+           "emc_workspace_bytes_rot_chunked", "emc_workspace_view", "emc_shard_stats", "emc_shard_update", "emc_shard_finish", "emc_iterate_gaussian", "emc_loglik_gaussian", "emc_refine", "emc_check",
+           "emc_profile_read", "emc_profile_dropped", "emc_launch_count", "emc_strerror", "emc_last_cuda_error", "emc_version")
 
 
 class EmcError(RuntimeError):
@@ -102,6 +103,8 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_iterate.restype = ci
     lib.emc_iterate.argtypes = [POINTER(_Model), POINTER(_Detector), POINTER(_Rotations), POINTER(_Patterns),
                                 ci, ci, vp, vp, ci, vp, cu, vp, sz, vp, vp]
+    lib.emc_workspace_view.restype = ci
+    lib.emc_workspace_view.argtypes = [vp, ci, ci, ci, ci, cu, ci, POINTER(vp), POINTER(c_int)]
     lib.emc_workspace_bytes_rot_chunked.restype = sz
     lib.emc_workspace_bytes_rot_chunked.argtypes = [ci, ci, ci, ci, ci]
     lib.emc_iterate_rot_chunked.restype = ci
@@ -127,6 +130,8 @@ def load(path: str | pathlib.Path | None = None) -> ctypes.CDLL:
     lib.emc_check.argtypes = [vp, vp]
     lib.emc_profile_read.restype = ci
     lib.emc_profile_read.argtypes = [vp, POINTER(c_double), POINTER(c_int)]
+    lib.emc_profile_dropped.restype = ci
+    lib.emc_profile_dropped.argtypes = [vp]
     lib.emc_launch_count.restype = c_uint64
     lib.emc_launch_count.argtypes = []
     for name in ("emc_strerror", "emc_last_cuda_error", "emc_version"):
@@ -383,6 +388,23 @@ def emc_iterate(model, q, mask, quat, weight, counts, n_iter=1, n_pat_chunk=0, f
     return dict(model=model_out, loglik=loglik, P=p[:, :pat.n_pat] if want_p else None, ws=ws)
 
 
+def emc_workspace_view(ws, n, n_pix, n_rot, n_pat_chunk, what, flags=0):
+    """A tensor view (no copy) of what the emc_iterate call that used `ws` left in it (include/emc.h, emc_workspace_view):
+    EMC_VIEW_LOGLIK -> L [R, n_pat_chunk] float32 (rows ld_n apart), EMC_VIEW_S -> s [R], EMC_VIEW_WNEW -> W' [R, P].
+    Synchronise the stream of that call first."""
+    ptr, ld = c_void_p(), c_int()
+    _check(load().emc_workspace_view(ws.data_ptr(), n, n_pix, n_rot, n_pat_chunk, flags, what, ctypes.byref(ptr), ctypes.byref(ld)),
+           "emc_workspace_view")
+    off = ptr.value - ws.data_ptr()
+    pitch = ld.value if what != EMC_VIEW_S else 1
+    rows = n_rot if what != EMC_VIEW_S else 1
+    cols = {EMC_VIEW_LOGLIK: n_pat_chunk, EMC_VIEW_S: n_rot, EMC_VIEW_WNEW: n_pix}[what]
+    flat = ws[off: off + 4 * ((rows - 1) * pitch + cols)].view(torch.float32)
+    if what == EMC_VIEW_S:
+        return flat
+    return flat.as_strided((rows, cols), (pitch, 1))
+
+
 def emc_iterate_rot_chunked(model, q, mask, quat, weight, counts, n_rot_chunk, n_iter=1, flags=0, ws=None, ctx=None):
     """Algorithm 1 with the rotation list streamed in chunks.  Returns dict(model, loglik, ws)."""
     n = model.shape[0]
@@ -511,6 +533,11 @@ def emc_profile_read(ctx=None) -> dict:
     spans = (c_int * len(STAGES))()
     _check(load().emc_profile_read((ctx or default_context()).handle, ms, spans), "emc_profile_read")
     return {name: (ms[i], spans[i]) for i, name in enumerate(STAGES)}
+
+
+def emc_profile_dropped(ctx=None) -> int:
+    """Spans dropped because the context's pool of EMC_MAX_SPANS event pairs was exhausted; resets the count."""
+    return load().emc_profile_dropped((ctx or default_context()).handle)
 
 
 def emc_launch_count() -> int:

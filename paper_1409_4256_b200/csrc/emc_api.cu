@@ -32,7 +32,7 @@ struct emc_context {
     cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, entry = nullptr;
     cudaEvent_t beg[EMC_MAX_SPANS], end[EMC_MAX_SPANS];
     int stage[EMC_MAX_SPANS];
-    int created = 0, used = 0;
+    int created = 0, used = 0, dropped = 0;
 };
 
 namespace emc {
@@ -44,7 +44,8 @@ struct Span {
     int slot = -1;
     cudaStream_t st;
     Span(emc_context *ctx, bool on, int stage, cudaStream_t stream) : st(stream) {
-        if (!on || !ctx || ctx->used >= ctx->created) return;
+        if (!on || !ctx) return;
+        if (ctx->used >= ctx->created) { ++ctx->dropped; return; }   // emc_profile_dropped()
         c = ctx;
         slot = c->used++;
         c->stage[slot] = stage;
@@ -237,6 +238,8 @@ emc_status emc_context_destroy(emc_context *c) {
 
 size_t emc_workspace_bytes(int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags) {
     if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return 0;
+    if ((flags & EMC_SPARSE_PHOTONS) && (n_pix >= (1 << 20) || n_pat_chunk >= (1 << 20) || (size_t)n_pat_chunk * n_pix >= ((size_t)1 << 31)))
+        return 0;                                               // what emc_iterate refuses for the photon-list path
     const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? 2 * round_up((size_t)n_pat_chunk * n_pix * 4, 1024) : 0;
     return carve(nullptr, n, n_pix, n_rot, n_pat_chunk, stage, (flags & EMC_SPARSE_PHOTONS) != 0).total;
 }
@@ -377,7 +380,9 @@ static emc_status iterate_impl(const emc_model *model, const emc_detector *det, 
     const size_t stage_one = round_up((size_t)chunk * n_pix * 4, 1024);          // one staging buffer (4 B per count at most)
     const size_t stage_bytes = on_host ? 2 * stage_one : 0;
     const bool sparse = (flags & EMC_SPARSE_PHOTONS) != 0;
-    if (sparse && (gauss || n_pix >= (1 << 20) || chunk >= (1 << 20) || (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT))))
+    // photon lists: 20-bit column indices, and 32-bit offsets into lists sized for a chunk in which every count is non-zero
+    if (sparse && (gauss || n_pix >= (1 << 20) || chunk >= (1 << 20) || (size_t)chunk * n_pix >= ((size_t)1 << 31) ||
+                   (flags & (EMC_GEMM_1CTA | EMC_DEBUG_SIMT))))
         return EMC_ERR_UNSUPPORTED;
     EMC_TRY(check_ws(ws, ws_bytes, carve(nullptr, n, n_pix, n_rot, chunk, stage_bytes, sparse).total));
     const Layout l = carve(ws, n, n_pix, n_rot, chunk, stage_bytes, sparse);
@@ -548,6 +553,24 @@ emc_status emc_iterate(const emc_model *model, const emc_detector *det, const em
                         stream, ctx, 0.f);
 }
 
+emc_status emc_workspace_view(void *ws, int n, int n_pix, int n_rot, int n_pat_chunk, unsigned flags, int what, void **ptr,
+                              int *ld) {
+    if (!ws || ((uintptr_t)ws & 255) || !ptr || !ld) return EMC_ERR_ARG;
+    if (!sizes_ok(n, n_pix, n_rot, n_pat_chunk)) return EMC_ERR_UNSUPPORTED;
+    const bool sparse = (flags & EMC_SPARSE_PHOTONS) != 0;
+    const size_t stage = (flags & EMC_PATTERNS_ON_HOST) ? 2 * round_up((size_t)n_pat_chunk * n_pix * 4, 1024) : 0;
+    const Layout l = carve(ws, n, n_pix, n_rot, n_pat_chunk, stage, sparse);      // the layout iterate_impl uses
+    switch (what) {
+        case EMC_VIEW_LOGLIK:
+            if (sparse) return EMC_ERR_UNSUPPORTED;                                // the photon-list path forms L^T only
+            *ptr = l.L; *ld = l.ld_n;
+            return EMC_OK;
+        case EMC_VIEW_S: *ptr = l.s; *ld = 0; return EMC_OK;
+        case EMC_VIEW_WNEW: *ptr = l.Wnum; *ld = n_pix; return EMC_OK;
+    }
+    return EMC_ERR_ARG;
+}
+
 // Rotation chunks: the per-chunk buffers of carve() at R = chunk size, then s for the whole list
 static size_t rot_chunked_extra(int n_rot) { return round_up(sizeof(float) * (size_t)n_rot, 1024); }
 
@@ -564,7 +587,7 @@ emc_status emc_iterate_rot_chunked(const emc_model *model, const emc_detector *d
     if (!model || !model->model || !det_ok(det) || !rot_ok(rot) || !pat_ok(pat) || n_iter <= 0 || !model_out ||
         model_out == model->model || !loglik || n_rot_chunk <= 0)
         return EMC_ERR_ARG;
-    if (flags & EMC_PATTERNS_ON_HOST) return EMC_ERR_UNSUPPORTED;
+    if (flags & (EMC_PATTERNS_ON_HOST | EMC_SPARSE_PHOTONS)) return EMC_ERR_UNSUPPORTED;   // dense, device-resident only
     if ((flags & EMC_PROFILE_STAGES) && !ctx) return EMC_ERR_ARG;
     if (n_iter > 256) return EMC_ERR_UNSUPPORTED;
     const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
@@ -684,6 +707,7 @@ emc_status emc_shard_stats(const emc_model *model, const emc_detector *det, cons
     EMC_TRY_CUDA(cudaMemcpyAsync(stats_out, m, row, cudaMemcpyDeviceToDevice, st));
     EMC_TRY_CUDA(cudaMemcpyAsync(stats_out + l.ld_n, w, row, cudaMemcpyDeviceToDevice, st));
     EMC_TRY_CUDA(cudaMemcpyAsync(stats_out + 2 * (size_t)l.ld_n, z, row, cudaMemcpyDeviceToDevice, st));
+    EMC_TRY(launch_shard_stamp(l.hdr, n_rot, n_pat, n_pix, false, st));      // what the workspace now carries
     return launch_poison(l.hdr, stats_out, 3 * (size_t)l.ld_n, nullptr, 0, st);
 }
 
@@ -698,6 +722,9 @@ emc_status emc_shard_update(const emc_model *model, const emc_detector *det, con
     const int n = model->n, n_pix = det->n_pix, n_rot = rot->n_rot, n_pat = pat->n_pat;
     const float log_uniform = log_uniform_of(n_rot_total);
     const bool weighted = (flags & EMC_COMPRESS_WEIGHTED) != 0;
+    // L, the packed counts and the header must be those of an emc_shard_stats call with these sizes: checked on the
+    // device; a mismatch turns the results into NaN and emc_check reports EMC_ERR_WORKSPACE
+    EMC_TRY(launch_shard_stamp(l.hdr, n_rot, n_pat, n_pix, true, st));
     // the ranks' statistics become partial rows 0 .. world-1 (merged in rank order: the same result on every rank)
     const size_t row = sizeof(float) * (size_t)l.ld_n;
     for (int k = 0; k < world; ++k) {
@@ -771,10 +798,14 @@ emc_status emc_refine(const emc_model *model, const emc_detector *det, const emc
 emc_status emc_check(void *ws, void *stream) {
     if (!ws) return EMC_ERR_ARG;
     WsHeader h;
-    EMC_TRY_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
-    EMC_TRY_CUDA(cudaMemcpy(&h, ws, sizeof(h), cudaMemcpyDeviceToHost));
-    EMC_TRY_CUDA(cudaMemset(ws, 0, sizeof(h)));
+    cudaStream_t st = (cudaStream_t)stream;
+    // read and clear ON the caller's stream (ordered after the calls that used ws, before whatever the caller enqueues
+    // next on it); the legacy default stream would not be ordered against a non-blocking stream
+    EMC_TRY_CUDA(cudaMemcpyAsync(&h, ws, sizeof(h), cudaMemcpyDeviceToHost, st));
+    EMC_TRY_CUDA(cudaMemsetAsync(ws, 0, sizeof(h), st));
+    EMC_TRY_CUDA(cudaStreamSynchronize(st));
     if (h.max_count > 0) return EMC_ERR_COUNT_RANGE;            // the pack kernel records only counts over its limit
+    if (h.shard_mismatch) return EMC_ERR_WORKSPACE;             // emc_shard_update without the matching emc_shard_stats
     return h.w_range ? EMC_ERR_VALUE_RANGE : EMC_OK;
 }
 
@@ -792,6 +823,13 @@ emc_status emc_profile_read(emc_context *c, double *ms, int *spans) {
     }
     c->used = 0;
     return rc;
+}
+
+int emc_profile_dropped(emc_context *c) {
+    if (!c) return 0;
+    const int d = c->dropped;
+    c->dropped = 0;
+    return d;
 }
 
 uint64_t emc_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -147,7 +147,7 @@ geometry_kernel(const float *__restrict__ q, const uint8_t *__restrict__ mask, i
 // blocks per gather against 25 for 32 pixels of a detector row), four tiles per step in PHASES so that the loads of
 // a phase are all in flight together: geometry loads; coordinates; gathers; interpolation and outputs.  The kernel
 // is specialised on the outputs it has to write and has no divergent control flow: a lane without a pixel repeats
-// pixel 0 and only its stores are predicated.  What bounds it (ncu, profiles/r02_expand_compress.md): the issue
+// pixel 0 and only its stores are predicated.  What bounds it (ncu, profiles/r02_full_ncu.md): the issue
 // slots (125 warp instructions per 32 samples, 62 % of the slots used) with the waits for the gather exposed; capping
 // registers for more warps per SM (spills) or making the warps persistent over long bands were both slower.
 // S_part [R][n_bands]: sum_{p:mask} W (or W^2) of each band, summed per rotation in a fixed order by rowsum_kernel

@@ -42,8 +42,11 @@ static inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 struct WsHeader {
     int max_count;   // largest unmasked photon count seen by the pack kernel
     int w_range;     // 1 if a slice value left the fp16 range of the Gaussian model's operand planes (>= 65504)
-    int pad[62];
+    int shard_stamp[4];   // written by emc_shard_stats: (R_local, N, P, kShardTag) of the L / packed patterns the workspace carries
+    int shard_mismatch;   // set by emc_shard_update when the stamp is not the one its own arguments give
+    int pad[57];
 };
+constexpr int kShardTag = 0x53484152;   // "SHAR"
 static_assert(sizeof(WsHeader) == 256, "header is one 256-byte line");
 
 // Bump allocator over the caller's workspace.
@@ -106,6 +109,10 @@ emc_status launch_pack(const void *counts, emc_count_type type, int n_pat, int n
 // fills out[0..n) (floats) with NaN if hdr->max_count != 0: a result computed from clamped counts must not be
 // consumed unnoticed (emc.h, conventions)
 emc_status launch_poison(const WsHeader *hdr, float *out, size_t n, double *out64, int n64, cudaStream_t st);
+// rotation shards: emc_shard_stats stamps the header with the sizes of what it leaves in the workspace; emc_shard_update
+// verifies the stamp on the device (no host round trip) and records a mismatch, which poisons its results like a count out
+// of range does and is reported by emc_check
+emc_status launch_shard_stamp(WsHeader *hdr, int n_rot, int n_pat, int n_pix, bool verify, cudaStream_t st);
 
 // A[d] = sum_p Kc[d][p]^2 (fluence numerators of the Gaussian model, eq. 2.6) as g_col[d] = 1 / (2 sigma^2 A_d) and
 // ia_col[d] = 1 / A_d (both 0 where A_d = 0)

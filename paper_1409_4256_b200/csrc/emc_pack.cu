@@ -129,13 +129,33 @@ rowsq_kernel(const __half *__restrict__ Kc, int n_pat, int n_pix, int ld_p, floa
 // out[i] = NaN for every i if a count was out of range (grid-stride; a no-op launch otherwise)
 __global__ void __launch_bounds__(256)
 poison_kernel(const WsHeader *__restrict__ hdr, float *__restrict__ out, size_t n, double *__restrict__ out64, int n64) {
-    if (hdr->max_count == 0) return;
+    if (hdr->max_count == 0 && hdr->shard_mismatch == 0) return;
     const float nan = __int_as_float(0x7fc00000);
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) out[i] = nan;
     if (blockIdx.x == 0 && (int)threadIdx.x < n64) out64[threadIdx.x] = (double)nan;
 }
 
+__global__ void shard_stamp_kernel(WsHeader *__restrict__ hdr, int n_rot, int n_pat, int n_pix, int verify) {
+    if (threadIdx.x != 0) return;
+    if (verify) {
+        if (hdr->shard_stamp[0] != n_rot || hdr->shard_stamp[1] != n_pat || hdr->shard_stamp[2] != n_pix ||
+            hdr->shard_stamp[3] != kShardTag)
+            hdr->shard_mismatch = 1;
+    } else {
+        hdr->shard_stamp[0] = n_rot;
+        hdr->shard_stamp[1] = n_pat;
+        hdr->shard_stamp[2] = n_pix;
+        hdr->shard_stamp[3] = kShardTag;
+    }
+}
+
 }  // namespace
+
+emc_status launch_shard_stamp(WsHeader *hdr, int n_rot, int n_pat, int n_pix, bool verify, cudaStream_t st) {
+    shard_stamp_kernel<<<1, 32, 0, st>>>(hdr, n_rot, n_pat, n_pix, verify ? 1 : 0);
+    EMC_LAUNCHED();
+    return EMC_OK;
+}
 
 emc_status launch_poison(const WsHeader *hdr, float *out, size_t n, double *out64, int n64, cudaStream_t st) {
     if (n64 > 256) return EMC_ERR_UNSUPPORTED;

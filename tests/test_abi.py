@@ -72,6 +72,22 @@ def test_null_arguments_are_rejected_synchronously():
     assert lib.emc_context_create(None) == emc.EMC_ERR_ARG
     assert lib.emc_context_destroy(None) == emc.EMC_OK
     assert lib.emc_profile_read(None, None, None) == emc.EMC_ERR_ARG
+    assert lib.emc_profile_dropped(None) == 0
+    # flags a call does not implement are refused, not ignored (rotation chunks run the dense, device-resident path)
+    for flag in (emc.EMC_SPARSE_PHOTONS, emc.EMC_PATTERNS_ON_HOST):
+        assert lib.emc_iterate_rot_chunked(m, det, rot, pat, 1, 2, 16, 8, flag, 256, 1 << 30, None, None) == emc.EMC_ERR_UNSUPPORTED
+    # photon lists index a chunk with 32 bits: chunk x pixels must stay below 2^31
+    assert emc.emc_workspace_bytes(32, 65536, 100, 32768, emc.EMC_SPARSE_PHOTONS) == 0
+    assert emc.emc_workspace_bytes(32, 65536, 100, 32767, emc.EMC_SPARSE_PHOTONS) > 0
+    big = binding._Patterns(40000, 8, emc.binding.EMC_U16)
+    det_big = binding._Detector(65536, 8, None, 0)
+    assert lib.emc_iterate(m, det_big, rot, big, 1, 0, 16, None, 64, 8, emc.EMC_SPARSE_PHOTONS, 256, 1 << 40, None, None) == emc.EMC_ERR_UNSUPPORTED
+    # emc_workspace_view: host-side pointer arithmetic
+    ptr, ld = ctypes.c_void_p(), ctypes.c_int()
+    assert lib.emc_workspace_view(4096, 16, 16, 4, 4, 0, emc.EMC_VIEW_LOGLIK, ctypes.byref(ptr), ctypes.byref(ld)) == emc.EMC_OK
+    assert ptr.value > 4096 and ld.value == 64
+    assert lib.emc_workspace_view(4096, 16, 16, 4, 4, emc.EMC_SPARSE_PHOTONS, emc.EMC_VIEW_LOGLIK, ctypes.byref(ptr), ctypes.byref(ld)) == emc.EMC_ERR_UNSUPPORTED
+    assert lib.emc_workspace_view(4096, 16, 16, 4, 4, 0, 99, ctypes.byref(ptr), ctypes.byref(ld)) == emc.EMC_ERR_ARG
 
 
 def test_binding_refuses_cpu_tensors():

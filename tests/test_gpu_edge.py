@@ -28,9 +28,11 @@ def run_both(model, q, mask, quat, weight, counts, weighted=False, null_weight=F
     d = [dev(model), dev(q), dev(mask), dev(quat), None if null_weight else dev(weight), dev(counts)]
     out = emc.emc_iterate(*d, want_p=True, flags=emc.EMC_COMPRESS_WEIGHTED if weighted else 0)
     emc.emc_check(out["ws"])
-    # the float32 L the GPU path forms (stage API: the same kernels as inside emc_iterate), for the measured P bound
-    w, idx = emc.emc_expand(d[0], d[1], d[3])
-    out["L"] = host(emc.emc_loglik(w, idx, d[1], d[2], d[5]))
+    # the float32 L this emc_iterate call itself formed, read from its workspace, for the measured P bound
+    torch.cuda.synchronize()
+    n, n_pix, n_rot, n_pat = model.shape[0], q.shape[0], quat.shape[0], counts.shape[0]
+    out["L"] = host(emc.emc_workspace_view(out["ws"], n, n_pix, n_rot, n_pat, emc.EMC_VIEW_LOGLIK,
+                                           emc.EMC_COMPRESS_WEIGHTED if weighted else 0))
     return ref, out
 
 

@@ -3,9 +3,13 @@
   C4  128^3 / 128x128 / R = 10 000, pattern chunks of 25 000 streamed from pinned host memory: the config's own chunk
       size and route, N cut to 2 chunks + a ragged third (60 000 of 200 000 patterns);
   C5  last stage, 256^3 / 256x256 / R = 50 000, the full 20 000 patterns (EMC_TEST_LARGE=0 cuts them to 1024).
+At C3 and C5 Compress runs over ALL rotations against oracle.compress (float64, thread pool), and emc_iterate itself -- the
+path bench.py times -- is checked at size: T1 on the L it formed (read from its workspace), T2 on its P, its s, LL, W' rows
+and model' against the oracle / the stage chain.
 Model, detector, mask and rotation list are the configs' own.  What these sizes exercise beyond C2: linear indices
 past 2^31 (R x P = 3.3e9), accumulators that do not fit L2, hundreds of K chunks, ragged last pair tiles."""
 import os
+from concurrent.futures import ThreadPoolExecutor
 
 import numpy as np
 import pytest
@@ -37,7 +41,29 @@ def sampled_rows(n_rot, k, seed):
     return np.array(sorted(rows), dtype=np.int64)
 
 
-def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
+def oracle_compress(wn, q, quat, mask, n, slice_w):
+    """oracle.compress over ALL the rotations given: the definition evaluated on disjoint blocks of the rotation list by a
+    pool of threads (numpy releases the GIL in the arithmetic), the float64 numerator / denominator grids of the blocks
+    added up in float64, division last.  3.2e9 (C3) / 2.6e10 (C5) float64 additions."""
+    n_rot = wn.shape[0]
+    workers = min(32, os.cpu_count() or 1)
+    bounds = np.linspace(0, n_rot, 4 * workers + 1).astype(int)
+
+    def block(i):
+        sl = slice(bounds[i], bounds[i + 1])
+        _, num, den = o.compress(wn[sl], q, quat[sl], mask, n, slice_w=slice_w[sl])
+        return num, den
+
+    num, den = np.zeros(n ** 3), np.zeros(n ** 3)
+    with ThreadPoolExecutor(workers) as ex:
+        for nb, db in ex.map(block, range(len(bounds) - 1)):
+            num += nb
+            den += db
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return np.where(den > 0, num / den, 0.0), den
+
+
+def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols):
     inp = inputs_cache(name, n_pat=n_pat)
     cfg = inp.cfg
     quat, weight = inp.quat[stage], inp.weight[stage]
@@ -96,21 +122,61 @@ def run_case(inputs_cache, name, n_pat, stage, n_rows, n_cols, n_compress):
     use = inp.mask.astype(bool)
     assert np.abs(tot[use] - k_tot[use]).max() <= 1e-4 * max(1.0, k_tot[use].max())
 
-    # ---- stage 5 on the first n_compress rotations of the GPU's W' (the oracle scatters them in float64)
-    sub = slice(0, n_compress)
-    sw = (host(s[sub]) > 0).astype(np.float32)
-    m, den = emc.emc_compress(wn[sub].contiguous(), dev(sw), d_q, d_mask, d_quat[sub].contiguous(), cfg.n, want_den=True,
-                              ws=ws)
-    m_ref, _, den_ref = o.compress(host(wn[sub]), inp.q, quat[sub], inp.mask, cfg.n, slice_w=sw)
+    # ---- stage 5 over ALL rotations of the GPU's W' (the oracle scatters them in float64): the longest chains of float32
+    # reductions per voxel that the config produces (T3, eq. 2.10; "division as a final step" :166)
+    sw = (host(s) > 0).astype(np.float32)
+    d_sw = dev(sw)
+    m, den = emc.emc_compress(wn, d_sw, d_q, d_mask, d_quat, cfg.n, want_den=True, ws=ws)
+    m_ref, den_ref = oracle_compress(host(wn), inp.q, quat, inp.mask, cfg.n, sw)
     m, den, m_ref = host(m).reshape(-1), host(den), m_ref.reshape(-1)
     cov = den_ref >= 1e-6 * den_ref.max()
-    assert np.all(np.abs(den[cov] - den_ref[cov]) <= 1e-5 * den_ref[cov])
-    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12)
+    rel_den = np.abs(den[cov] - den_ref[cov]) / den_ref[cov]
+    rel_m = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-12)
+    print(f"{name}: Compress over all {n_rot} rotations: max rel den {rel_den.max():.2e}, model {rel_m.max():.2e} "
+          f"(most hits on a voxel {den_ref.max():.3g})")
+    assert rel_den.max() <= 1e-5
+    assert np.all(np.abs(m[cov] - m_ref[cov]) <= 1e-5 * np.abs(m_ref[cov]) + 1e-12), f"max rel {rel_m.max():.3e}"
     assert np.all(m[den_ref == 0] == 0)
+    model_chain, ll_chain, s_chain = m, float(host(ll)[0]), host(s)
+    del m_ref, den_ref
+
+    # ---- the product path at this size: emc_iterate as bench.py times it (fused Expand with __logf planes, column
+    # statistics from the contraction's epilogue, planes-only normalisation) against the oracle on the L it formed itself
+    # and against the stage chain above (Algorithm 1)
+    del p, wn, big_l
+    torch.cuda.empty_cache()
+    out = emc.emc_iterate(dev(inp.model_init), d_q, d_mask, d_quat, dev(weight), d_k, want_p=True, ws=ws)
+    emc.emc_check(ws)
+    torch.cuda.synchronize()
+    l_it = emc.emc_workspace_view(ws, cfg.n, n_pix, n_rot, n_pat, emc.EMC_VIEW_LOGLIK)
+    err = np.abs(host(l_it[t_rows]) - l_ref) / a_ref
+    assert err.max() <= 1e-5, f"emc_iterate's own L: max |dL|/A = {err.max():.3e}"          # T1 on the product path's L
+    p_ref, _, _ = o.normalize(host(l_it[:, t_cols]), weight)
+    assert np.abs(host(out["P"][:, t_cols]) - p_ref).max() <= 1e-6                          # T2 on its P, stage-wise
+    s_it = host(emc.emc_workspace_view(ws, cfg.n, n_pix, n_rot, n_pat, emc.EMC_VIEW_S))
+    s_sum = host(out["P"].sum(dim=1, dtype=torch.float64))
+    assert np.abs(s_it - s_sum).max() <= 1e-5 * max(1.0, s_sum.max())
+    ll_it = float(host(out["loglik"])[0])
+    assert abs(ll_it - ll_chain) <= 1e-6 * abs(ll_chain)
+    # its W' rows from its own P (eq. 2.11), as for the stage call
+    wn_it = host(emc.emc_workspace_view(ws, cfg.n, n_pix, n_rot, n_pat, emc.EMC_VIEW_WNEW)[t_rows])
+    wn_ref2, _ = o.update(host(out["P"][t_rows]), inp.counts, inp.mask)
+    keep = s_it[rows] > 1e-20
+    scale = np.abs(wn_ref2[keep]).max()
+    rel = np.abs(wn_it[keep] - wn_ref2[keep]) / (np.abs(wn_ref2[keep]) + 1e-7 * scale)
+    assert rel.max() <= 2e-5, f"emc_iterate's own W': max rel {rel.max():.3e}"
+    # model' of the two routes: the same arithmetic from L onwards, L itself differs by logf / __logf in the planes
+    m_it = host(out["model"]).reshape(-1)
+    big = np.abs(model_chain) >= 1e-6 * np.abs(model_chain).max()
+    rel = np.abs(m_it - model_chain)[big] / np.abs(model_chain)[big]
+    flips = int(((s_it > 0) != (s_chain > 0)).sum())
+    print(f"{name}: emc_iterate vs stage chain: model' rel median {np.median(rel):.2e} max {rel.max():.2e}, "
+          f"slices with s > 0 on one route only: {flips}")
+    assert np.median(rel) <= 1e-5 and rel.max() <= 1e-2, (np.median(rel), rel.max())
 
 
 def test_c3_full_config_sampled(inputs_cache):
-    run_case(inputs_cache, "C3", n_pat=50000, stage=0, n_rows=24, n_cols=48, n_compress=1500)
+    run_case(inputs_cache, "C3", n_pat=50000, stage=0, n_rows=24, n_cols=48)
 
 
 def test_c4_route_pattern_chunks_from_host(inputs_cache):
@@ -186,4 +252,4 @@ def test_c4_route_pattern_chunks_from_host(inputs_cache):
 
 
 def test_c5_last_stage_geometry_sampled(inputs_cache):
-    run_case(inputs_cache, "C5", n_pat=20000 if FULL else 1024, stage=4, n_rows=12, n_cols=32, n_compress=400)
+    run_case(inputs_cache, "C5", n_pat=20000 if FULL else 1024, stage=4, n_rows=12, n_cols=32)

@@ -36,10 +36,18 @@ def p_bound(p_ref, l_gpu, l_ref):
 
 
 def gpu_loglik(case, model=None):
-    """The float32 L the GPU path forms for this case (stage API: Expand, then the log-likelihood contraction; the
-    same kernels and arithmetic as inside emc_iterate)."""
+    """The float32 L of the STAGE calls for this case (emc_expand, then emc_loglik: W stored as float32, logW planes by
+    logw_split_kernel with logf).  Not the arithmetic of emc_iterate, whose Expand forms the planes in registers with
+    __logf and whose contraction also writes the column statistics: for that L see iterate_loglik()."""
     w, idx = emc.emc_expand(case.d_model if model is None else model, case.d_q, case.d_quat)
     return host(emc.emc_loglik(w, idx, case.d_q, case.d_mask, case.d_counts))
+
+
+def iterate_loglik(out, n, n_pix, n_rot, n_pat, flags=0):
+    """The float32 L that the emc_iterate call behind `out` itself formed (one pattern chunk, dense path), read from where
+    it lies in that call's workspace (emc_workspace_view): the product path's own L, not a stage call's."""
+    torch.cuda.synchronize()
+    return host(emc.emc_workspace_view(out["ws"], n, n_pix, n_rot, n_pat, emc.EMC_VIEW_LOGLIK, flags))
 
 
 class Case:
@@ -175,9 +183,17 @@ def test_iterate_end_to_end(case, weighted, uniform_null):
     out = emc.emc_iterate(case.d_model, case.d_q, case.d_mask, case.d_quat, None if uniform_null else dev(weight),
                           case.d_counts, flags=flags, want_p=True)
     emc.emc_check(out["ws"])
+    # T1 on the L this very call formed (fused Expand with __logf planes, statistics in the contraction's epilogue)
+    l_it = iterate_loglik(out, case.cfg.n, inp.q.shape[0], n_rot, inp.counts.shape[0], flags)
+    l64, big_a = o.loglik(r["W"], r["idx"], inp.counts, inp.mask)
+    err = np.abs(l_it.astype(np.float64) - l64) / big_a
+    assert err.max() <= 1e-5, f"emc_iterate's own L: max |dL|/A = {err.max():.3e}"
     p = host(out["P"])
-    bound = p_bound(r["P"], gpu_loglik(case), r["L"])
+    bound = p_bound(r["P"], l_it, r["L"])                      # the bound on P from the dL of the same call
     assert np.all(np.abs(p - r["P"]) <= bound), f"max dP {np.abs(p - r['P']).max():.3e}"
+    # the slices and weights that went into Compress, on the same footing as the stage tests
+    s_it = host(emc.emc_workspace_view(out["ws"], case.cfg.n, inp.q.shape[0], n_rot, inp.counts.shape[0], emc.EMC_VIEW_S, flags))
+    assert np.abs(s_it - p.sum(axis=1)).max() <= 1e-5 * max(1.0, float(s_it.max()))
     assert np.abs(p.sum(axis=0) - 1).max() <= 1e-5
     ll = float(host(out["loglik"])[0])
     assert abs(ll - r["LL"]) <= 1e-5 * abs(r["LL"])

@@ -73,6 +73,42 @@ def test_shard_phases_match_oracle_and_unsharded(inputs_cache, name, world, weig
     assert np.median(rel1) <= 1e-5 and rel1.max() <= 2e-2, (np.median(rel1), rel1.max())
 
 
+def test_shard_update_refuses_a_workspace_without_matching_stats(inputs_cache):
+    """emc_shard_update trusts L and the packed patterns in the workspace.  emc_shard_stats stamps the header with its sizes;
+    a workspace that no matching call prepared (fresh, or prepared for another share) gives NaN results and emc_check says so,
+    instead of a silently wrong P."""
+    inp = inputs_cache("T1")
+    cfg = inp.cfg
+    quat = inp.quat[0]
+    n_rot = quat.shape[0]
+    d_model, d_q, d_mask = dev(inp.model_init), dev(inp.q.reshape(cfg.n_det, cfg.n_det, 3)), dev(inp.mask)
+    d_quat, d_k = dev(quat), dev(inp.counts)
+    half = n_rot // 2
+    st_a, ws_a = emc.emc_shard_stats(d_model, d_q, d_mask, d_quat[:half].contiguous(), None, d_k, n_rot)
+    st_b, ws_b = emc.emc_shard_stats(d_model, d_q, d_mask, d_quat[half:].contiguous(), None, d_k, n_rot)
+    stats_all = torch.stack([st_a, st_b])
+    # the matching pair works and leaves nothing to report
+    nd, ll, _ = emc.emc_shard_update(d_model, d_q, d_mask, d_quat[:half].contiguous(), None, d_k, n_rot, stats_all, ws_a)
+    emc.emc_check(ws_a)
+    assert torch.isfinite(nd).all() and torch.isfinite(ll).all()
+    # a workspace nobody prepared
+    fresh = torch.zeros_like(ws_a)
+    nd, ll, _ = emc.emc_shard_update(d_model, d_q, d_mask, d_quat[:half].contiguous(), None, d_k, n_rot, stats_all, fresh)
+    with pytest.raises(emc.EmcError) as e:
+        emc.emc_check(fresh)
+    assert e.value.status == emc.EMC_ERR_WORKSPACE
+    assert torch.isnan(nd).all() and torch.isnan(ll).all()
+    # a workspace prepared for another share of the rotations (one rotation fewer: the same layout would not even be needed)
+    if n_rot - half != half - 1:
+        other = d_quat[: half - 1].contiguous()
+        ws_c = torch.zeros(emc.emc_workspace_bytes(cfg.n, cfg.n_pix, half - 1, inp.counts.shape[0]), dtype=torch.uint8, device="cuda")
+        ws_c[: min(ws_c.numel(), ws_a.numel())] = ws_a[: min(ws_c.numel(), ws_a.numel())]      # header stamped for `half` rotations
+        nd, ll, _ = emc.emc_shard_update(d_model, d_q, d_mask, other, None, d_k, n_rot, stats_all, ws_c)
+        with pytest.raises(emc.EmcError):
+            emc.emc_check(ws_c)
+        assert torch.isnan(nd).all()
+
+
 def _worker(rank, world, port, out):
     import torch.distributed as dist
 
