@@ -42,6 +42,7 @@ UNIT = "iterations/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels, from the committed `ncu --set full`
 # captures (profiles/*.md name the commands); keyed "<config>:<stage>"
 TRAFFIC_FILE = ROOT / "profiles" / "r02_dram_traffic.csv"       # from the committed ncu capture (profiles/r02_full_ncu.md)
+TRAFFIC_COMMIT = "ca8073a"                                      # the commit that capture was taken at (emc_gemm.cu unchanged since)
 
 
 def parse():
@@ -86,14 +87,18 @@ def measured_peaks():
 # ------------------------------------------------------------------------------ CPU oracle leg
 
 def oracle_sample(inp, stage, n_rot_s, n_pat_s):
-    """Times the oracle's five stages on a bounded sample and extrapolates one full iteration
-    (stages 1, 5 are linear in R; stages 2-4 bilinear in R x N).  Returns (seconds_full, dict)."""
+    """Times the oracle's five stages on a bounded sample and extrapolates one full iteration.  Stages 1 and 5 are linear in
+    R.  Stages 2-4 are timed at TWO rotation counts (R_s and R_s / 2) on the same patterns and fitted as
+    t = a N P + b R N P: oracle.loglik and oracle.update convert the whole count sample to float64 on every call, a cost that
+    does not depend on R and that a purely bilinear extrapolation would multiply by R / R_s (the two arms of bench.py, which
+    sample different R_s, then disagree by up to 2x).  Returns (seconds_full, dict)."""
     from oracle import emc_oracle as o
 
     cfg = inp.cfg
     quat, wgt = inp.quat[stage], inp.weight[stage]
     n_rot, n_pat = len(quat), cfg.n_pat
     rs, ns = min(n_rot, n_rot_s), min(n_pat, n_pat_s, inp.counts.shape[0])
+    r2 = max(1, rs // 2)
     qs = quat[:rs]
     ws = (wgt[:rs] / wgt[:rs].sum()).astype(np.float32)
     ks = inp.counts[:ns]
@@ -101,22 +106,35 @@ def oracle_sample(inp, stage, n_rot_s, n_pat_s):
     t0 = time.perf_counter()
     w, idx = o.expand(inp.model_init, inp.q, qs)
     t["expand"] = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    big_l, _ = o.loglik(w, idx, ks, inp.mask)
-    t["loglik"] = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    p, _, _ = o.normalize(big_l.astype(np.float32), ws)
-    t["normalize"] = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    wn, s = o.update(p.astype(np.float32), ks, inp.mask)
-    t["update"] = time.perf_counter() - t0
+
+    def stages_2_to_4(rows):
+        tt = {}
+        t0 = time.perf_counter()
+        big_l, _ = o.loglik(w[:rows], idx[:rows], ks, inp.mask)
+        tt["loglik"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        p, _, _ = o.normalize(big_l.astype(np.float32), (ws[:rows] / ws[:rows].sum()).astype(np.float32))
+        tt["normalize"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        wn, s = o.update(p.astype(np.float32), ks, inp.mask)
+        tt["update"] = time.perf_counter() - t0
+        return tt, wn, s
+
+    half, _, _ = stages_2_to_4(r2)
+    whole, wn, s = stages_2_to_4(rs)
+    t.update(whole)
     t0 = time.perf_counter()
     o.compress(wn, inp.q, qs, inp.mask, cfg.n, slice_w=(s > 0).astype(np.float32))
     t["compress"] = time.perf_counter() - t0
-    lin = n_rot / rs
-    bil = (n_rot * n_pat) / (rs * ns)
-    full = (t["expand"] + t["compress"]) * lin + (t["loglik"] + t["normalize"] + t["update"]) * bil
-    return full, dict(times=t, sample_seconds=sum(t.values()), n_rot_sample=rs, n_pat_sample=ns)
+    full = (t["expand"] + t["compress"]) * n_rot / rs
+    fit = {}
+    for k in ("loglik", "normalize", "update"):
+        slope = max(0.0, (whole[k] - half[k]) / max(1, rs - r2)) if rs > r2 else whole[k] / rs     # seconds per rotation
+        fixed = max(0.0, whole[k] - slope * rs)                                                   # R-independent part
+        fit[k] = dict(per_rotation=slope, fixed=fixed)
+        full += (fixed + slope * n_rot) * n_pat / ns
+    return full, dict(times=t, times_half=half, fit=fit, sample_seconds=sum(t.values()) + sum(half.values()),
+                      n_rot_sample=rs, n_pat_sample=ns)
 
 
 def sample_sizes(cfg, scale=1.0):
@@ -153,7 +171,8 @@ def cpu_baseline(inp, scale=1.0):
     sample = (f"oracle/emc_oracle.py stage by stage on the first {parts[0]['n_rot_sample']} rotations x "
               f"{parts[0]['n_pat_sample']} patterns x all {cfg.n_pix} pixels of {cfg.name} "
               f"({sum(p['sample_seconds'] for p in parts):.1f} s of CPU work), extrapolated linearly in R "
-              f"(expand, compress) and bilinearly in R x N (loglik, normalize, update) to the full workload")
+              f"(expand, compress) and as (a + b R) N (loglik, normalize, update; a, b fitted from the sample and its first "
+              f"half of the rotations) to the full workload")
     return dict(value=value, unit=UNIT, cores=host_threads(), kind="oracle", sample=sample)
 
 
@@ -184,13 +203,25 @@ def run_reference(args):
     line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=warm, ms_per_step=1e3 * statistics.mean(times), higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=workload_name(cfg),
-                            note="every step times the CPU oracle on one bounded sample (cpu_baseline.sample); ms_per_step is "
-                                 "the wall time of such a step, value the extrapolation to the full workload",
-                            ms_per_full_step_extrapolated=1e3 * cfg.n_iter / value),
+                config=bench_config(cfg, int(os.environ.get("WORLD_SIZE", "1")), args.weighted, args.null_weights,
+                                    int(np.count_nonzero(inp.mask))),
+                note="every step times the CPU oracle on one bounded sample (cpu_baseline.sample); ms_per_step is the wall "
+                     "time of such a step, value the extrapolation to the full workload (eq. (2.10), explicit weights: the "
+                     "oracle has one code path)",
+                ms_per_full_step_extrapolated=1e3 * cfg.n_iter / value,
                 cpu_baseline=base,
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
+
+
+def bench_config(cfg, world, weighted, null_weights, p_eff):
+    """`config` of the JSON line: the same keys and values in both arms (--impl reference times the oracle on this workload)."""
+    return dict(workload=workload_name(cfg), parallelism="replicas only" if world > 1 else "1 GPU",
+                l2="per-iteration working set exceeds the 126 MB L2, no flush" if cfg.name != "C1"
+                else "working set fits L2 (launch-latency-bound config), no flush",
+                compress="eq. (2.12)" if weighted else "eq. (2.10)", p_eff=p_eff,
+                weights="NULL (1/R): uniform branches, normalize_kernel<true>" if null_weights
+                else "explicit equal weights: general branches, normalize_kernel<false>")
 
 
 def workload_name(cfg):
@@ -545,7 +576,8 @@ def main():
         for ln in TRAFFIC_FILE.read_text().splitlines()[1:]:
             c_, s_, b_ = ln.split(",")
             if c_ == cfg.name and s_ == dom:
-                traffic, traffic_src = float(b_), "profiles/r02_full_ncu.md (ncu --set full, dram read + write bytes per launch)"
+                traffic, traffic_src = float(b_), ("NOT measured in this run: read from the committed capture profiles/r02_full_ncu.md "
+                                                   f"of commit {TRAFFIC_COMMIT} (ncu --set full, dram read + write bytes per launch)")
     # tensor-core peak the chip has at the clock it held during this run (148 SMs x 8192 dense fp16 flops per clock)
     clock_peak = 148 * 8192 * clk["sm_mhz"] * 1e6 / 1e12 if clk.get("sm_mhz") else None
     roofline = dict(bound="tensor", kernel=f"plane_gemm_pair_kernel ({dom}, {stages[dom]['dtype']})",
@@ -566,12 +598,7 @@ def main():
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warmup,
                 ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="fp16x2 operand planes, f32 accumulate", data="synthetic",
-                config=dict(workload=workload_name(cfg), parallelism="replicas only" if world > 1 else "1 GPU",
-                            l2="per-iteration working set exceeds the 126 MB L2, no flush" if cfg.name != "C1"
-                            else "working set fits L2 (launch-latency-bound config), no flush",
-                            compress="eq. (2.12)" if args.weighted else "eq. (2.10)", p_eff=p_eff,
-                            weights="NULL (1/R): uniform branches, normalize_kernel<true>" if args.null_weights
-                            else "explicit equal weights: general branches, normalize_kernel<false>"),
+                config=bench_config(cfg, world, args.weighted, args.null_weights, p_eff),
                 clocks=clk,
                 e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                          ms_per_step=ms_e2e / args.steps),

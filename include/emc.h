@@ -64,10 +64,14 @@ typedef enum { EMC_I32 = 0, EMC_U16 = 1, EMC_U8 = 2 } emc_count_type;
  * expected to be masked. */
 #define EMC_MAX_COUNT 2048
 
-/* Responsibilities are float32 (the paper works in single precision).  Below the smallest
- * normal float32, 2^-126, a value has no relative precision left, so P is stored flush-to-zero: values
- * below 2^-126 are 0 (DESIGN.md §3 G20).  A rotation whose whole row is 0 has s[r] = 0: W'[r,:] = 0 and
- * the slice is skipped by Compress (G17).  Which slices that is matters under eq. (2.10) only. */
+/* Responsibilities are float32 (the paper works in single precision).  libemc stores them flush-to-zero:
+ * a value below the smallest normal float32, 2^-126, is 0, on output (emc_normalize, P_out) and on input (emc_update)
+ * (DESIGN.md §3 G20).  The paper is silent on underflow; the plain IEEE cast would keep subnormals down to 2^-149.  Why
+ * the library flushes: a subnormal P has lost its 24 significant bits, so a slice whose weights are all subnormal gets a
+ * W' (eq. 2.11) that no float32 pipeline can form to 1e-5 -- and the B200's own float32 reduction units (RED.ADD.F32 to
+ * global memory, which accumulates s[r]) flush subnormal operands anyway.  A rotation whose whole row is 0 has
+ * s[r] = 0: W'[r,:] = 0 and the slice is skipped by Compress (G17).  Which slices that is matters under eq. (2.10)
+ * only; the tests gate the difference to the plain cast slice by slice (tests/gates.py). */
 #define EMC_P_MIN 1.1754943508222875e-38f
 
 /* flags */

@@ -25,7 +25,13 @@ from __future__ import annotations
 import numpy as np
 
 LOGW_FLOOR = np.float32(1e-30)      # DESIGN.md §3 G8: log(max(W, 1e-30))
-P_MIN = float(np.finfo(np.float32).tiny)   # DESIGN.md §3 G20: float32 P is stored flush-to-zero (below 2^-126 -> 0)
+# DESIGN.md §3 G20.  P is a float32 quantity and the paper says nothing about its underflow, so
+# the oracle does nothing about it either: P_MIN = 0 leaves P to the plain float32 cast at the stage boundary (IEEE
+# gradual underflow: subnormals kept, 0 below 2^-150).  P_MIN_FLUSH = 2^-126 names the other float32 convention,
+# flush-to-zero below the smallest normal number, which is what libemc's storage does (EMC_P_MIN in include/emc.h);
+# tests select it with the `p_min` argument where they examine that convention.  The default is the plain cast.
+P_MIN = 0.0
+P_MIN_FLUSH = float(np.finfo(np.float32).tiny)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -176,13 +182,13 @@ def _use(mask, n_pix):
 # Stage 3: normalisation over rotations (reconstructed eq. 2.4)
 # ----------------------------------------------------------------------------------------------
 
-def normalize(big_l, weight):
+def normalize(big_l, weight, p_min=None):
     """P[r,d] = w_r T_rd / sum_r' w_r' T_r'd with T = exp(L), evaluated max-subtracted
     ("some care ... finite precision"; only max and sum are needed):
-        a = L + log w_r;  m_d = max_r a;  e = exp(a - m_d);  P = e / sum_r e,
-    with values below P_MIN = 2^-126 stored as 0 (G20: P is a float32 quantity; below
-    the smallest normal float32 a value has no relative precision left, so P is flushed to zero
-    there; a rotation whose whole row is 0 has s[r] = 0 and is skipped by Compress, G17).
+        a = L + log w_r;  m_d = max_r a;  e = exp(a - m_d);  P = e / sum_r e.
+    Values below `p_min` (default P_MIN = 0: none) are returned as 0: p_min = P_MIN_FLUSH = 2^-126 is the
+    flush-to-zero storage of float32 (G20); a rotation whose whole row is 0 has s[r] = 0 and is skipped
+    by Compress (G17).
     Also s[r] = sum_d P[r,d] and the total log-likelihood LL = sum_d (m_d + log sum_r e).
     `big_l` is taken as given (tests feed the float32-rounded L, DESIGN.md §4 T2).
     Returns (P float64 [R,N], s float64 [R], LL float)."""
@@ -191,7 +197,7 @@ def normalize(big_l, weight):
     e = np.exp(a - m[None, :])
     z = e.sum(axis=0)
     p = e / z[None, :]
-    p[p < P_MIN] = 0.0                                          # G20
+    p[p < (P_MIN if p_min is None else p_min)] = 0.0            # G20 (a no-op at the default)
     return p, p.sum(axis=1), float((m + np.log(z)).sum())
 
 
@@ -254,13 +260,14 @@ def compress(wn, q, quat, mask, n, slice_w=None, chunk=64):
 # One iteration (Algorithm 1), with pattern chunks (config 4, G9)
 # ----------------------------------------------------------------------------------------------
 
-def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=False):
+def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=False, p_min=None):
     """expand -> [per pattern chunk: loglik -> normalize] -> update -> compress.
 
     Stage boundaries carry float32 (W, L, P, W'), as the C-ABI does.  The soft-max is over
     rotations per pattern, so pattern chunks are independent in stages 2-3; s[r] and the update
     numerators add up over chunks and are divided after the last one (G9).
     `weighted` selects eq. (2.12) (om_r = s[r]) instead of eq. (2.10) (om_r = 1).
+    `p_min`: see normalize (default: the plain float32 cast of P).
     Returns dict(model, W, idx, L, P, s, Wn, LL)."""
     counts = np.asarray(counts)
     n = np.asarray(model).shape[0]
@@ -277,7 +284,7 @@ def iterate(model, q, mask, quat, weight, counts, n_pat_chunk=None, weighted=Fal
         d1 = min(n_pat, d0 + chunk)
         big_l, _ = loglik(w, idx, counts[d0:d1], mask)
         l32 = big_l.astype(np.float32)
-        p, _, ll_c = normalize(l32, weight)
+        p, _, ll_c = normalize(l32, weight, p_min)
         p32 = p.astype(np.float32)
         l_all[:, d0:d1] = l32
         p_all[:, d0:d1] = p32
@@ -351,14 +358,14 @@ def _merge_max_sum(m, z, a):
     return m_new, z
 
 
-def normalize_rotation_chunks(big_l, weight, n_rot_chunk):
+def normalize_rotation_chunks(big_l, weight, n_rot_chunk, p_min=None):
     """The normalisation of `normalize` when the rotations arrive in chunks C_c and only one chunk of
     L is held at a time.  "Only maximal rotational probabilities and sums are necessary":
     sweep 1 carries, per pattern d, the running maximum m_d and the running sum z_d of exp(a - m_d)
     over the chunks seen so far,
         m' = max(m, m_c),   z' = z exp(m - m') + z_c exp(m_c - m'),
     with (m_c, z_c) the max and sum of chunk c alone; sweep 2 revisits every chunk with the final
-    (m_d, z_d):  P = exp(a - m_d) / z_d.  Same flush (G20), same s and LL as `normalize`.
+    (m_d, z_d):  P = exp(a - m_d) / z_d.  Same `p_min` (G20), same s and LL as `normalize`.
     Returns (P float64 [R,N], s float64 [R], LL float)."""
     big_l = np.asarray(big_l).astype(np.float64)
     lw = np.log(np.asarray(weight).astype(np.float64))
@@ -372,11 +379,11 @@ def normalize_rotation_chunks(big_l, weight, n_rot_chunk):
     for r0 in range(0, n_rot, n_rot_chunk):                     # sweep 2
         a = big_l[r0:r0 + n_rot_chunk] + lw[r0:r0 + n_rot_chunk, None]
         p[r0:r0 + n_rot_chunk] = np.exp(a - m[None, :]) / z[None, :]
-    p[p < P_MIN] = 0.0                                          # G20
+    p[p < (P_MIN if p_min is None else p_min)] = 0.0            # G20
     return p, p.sum(axis=1), float((m + np.log(z)).sum())
 
 
-def iterate_rotation_chunks(model, q, mask, quat, weight, counts, n_rot_chunk, weighted=False):
+def iterate_rotation_chunks(model, q, mask, quat, weight, counts, n_rot_chunk, weighted=False, p_min=None):
     """One iteration of Algorithm 1 with the rotation list streamed in chunks of `n_rot_chunk`
     (PAPER.md:164-166): nothing of size R x N or R x P is ever held.
       sweep 1, per chunk: expand -> loglik -> merge the chunk's (max, sum) into the running ones
@@ -407,7 +414,7 @@ def iterate_rotation_chunks(model, q, mask, quat, weight, counts, n_rot_chunk, w
         l32 = loglik(w, idx, counts, mask)[0].astype(np.float32)
         a = l32.astype(np.float64) + lw[sl, None]
         p = np.exp(a - m[None, :]) / z[None, :]
-        p[p < P_MIN] = 0.0
+        p[p < (P_MIN if p_min is None else p_min)] = 0.0        # G20
         p32 = p.astype(np.float32)
         wn, s = update(p32, counts, mask)
         s_all[sl] = s

@@ -1,6 +1,6 @@
 """Writes tests/golden/g20_threshold_study.txt: one full oracle iteration of C1 and C2 under three storage conventions
-for the float32 responsibilities (flush below 2^-100 as in round 1, flush below 2^-126 = the reading G20, gradual
-underflow) and both c-steps.  Calls only oracle/ and the seeded input generator.  About 4 minutes on 8 cores.
+for the float32 responsibilities (flush below 2^-100 as in round 1, flush below 2^-126 = libemc's storage, gradual
+underflow = the oracle's default) and both c-steps.  Calls only oracle/ and the seeded input generator.  About 4 minutes on 8 cores.
 
     python tests/golden/make_g20_threshold_study.py
 """

@@ -1,17 +1,17 @@
 """Reading G20: where float32 stops representing a responsibility.
 
-The paper only says "some care ... finite precision".  P is carried in float32, and the
-oracle stores it flush-to-zero: below 2^-126 (the smallest normal float32) a value is 0.  This file measures, on the
-oracle alone, what that choice does to model' against the other float32 convention (gradual underflow: subnormals kept,
-0 below 2^-150), so that the threshold rests on float32's own limits and on numbers, not on any kernel:
+The paper only says "some care ... finite precision".  P is carried in float32.  The ORACLE
+does nothing about its underflow: P becomes float32 by numpy's cast (gradual underflow: subnormals kept, 0 below 2^-150).
+libemc stores P flush-to-zero below 2^-126, the smallest normal float32 (EMC_P_MIN in include/emc.h).  This file measures,
+on the oracle alone (o.P_MIN switched by hand), what separates the two conventions in model', so that the GPU tests can
+gate exactly that and nothing more (tests/gates.py):
 
  * eq. (2.12) (the c-step the paper implements) weights slice r by s[r] = sum_d P[r,d]: a slice made of
    subnormal responsibilities weighs < 2^-126 N against slices of weight O(1).  model' moves by far less than T3's 1e-5.
  * eq. (2.10) (north_star's literal stage 5) gives EVERY slice with s[r] > 0 the weight 1, so it is
    discontinuous in P at 0: which slices take part is decided by the last representable number of whatever arithmetic
    is used.  The slices whose status differs between the two conventions are exactly the rows made of float32
-   subnormals only, and model' differs on the voxels they touch by O(1e-3) -- under ANY threshold.  The reading fixes
-   one; the GPU path implements the same one (EMC_P_MIN in include/emc.h).
+   subnormals only, and model' differs on the voxels they touch by O(1e-3 ... 1) -- under ANY threshold.
 
 tests/golden/g20_threshold_study.txt holds the same numbers for one full C2 iteration (written by
 tests/golden/make_g20_threshold_study.py, oracle only, about 4 minutes)."""
@@ -47,8 +47,8 @@ def test_flush_to_zero_against_gradual_underflow(inputs_cache, name, n_pat):
     inp = inputs_cache(name, n_pat=n_pat) if n_pat else inputs_cache(name)
     tiny = float(np.finfo(np.float32).tiny)
     for weighted in (True, False):
-        ftz = run(inp, tiny, weighted)           # the reading: flush below 2^-126
-        grad = run(inp, 0.0, weighted)           # numpy's float32 cast: subnormals kept, 0 below 2^-150
+        ftz = run(inp, tiny, weighted)           # libemc's storage: flush below 2^-126
+        grad = run(inp, 0.0, weighted)           # the oracle's default: numpy's float32 cast, subnormals kept, 0 below 2^-150
         changed = (ftz["s"] > 0) != (grad["s"] > 0)
         # the rows whose status differs are exactly those that hold float32 subnormals and nothing larger
         only_subnormal = (grad["P"].max(axis=1) < tiny) & (grad["P"].max(axis=1) > 0)

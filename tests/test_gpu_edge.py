@@ -8,6 +8,7 @@ import pytest
 import torch
 
 from emc_inputs import CONFIGS, make_inputs
+import gates
 from oracle import emc_oracle as o
 
 pytestmark = pytest.mark.gpu
@@ -33,6 +34,7 @@ def run_both(model, q, mask, quat, weight, counts, weighted=False, null_weight=F
     n, n_pix, n_rot, n_pat = model.shape[0], q.shape[0], quat.shape[0], counts.shape[0]
     out["L"] = host(emc.emc_workspace_view(out["ws"], n, n_pix, n_rot, n_pat, emc.EMC_VIEW_LOGLIK,
                                            emc.EMC_COMPRESS_WEIGHTED if weighted else 0))
+    out["weighted"], out["geometry"] = weighted, (q, quat, mask, float(np.asarray(counts).max()))
     return ref, out
 
 
@@ -43,11 +45,7 @@ def check(ref, out):
     bound = 1e-6 + ref["P"] * np.expm1(2.0 * m)[None, :]
     assert np.all(np.abs(p - ref["P"]) <= bound), f"max dP {np.abs(p - ref['P']).max():.3e}"
     assert abs(float(host(out["loglik"])[0]) - ref["LL"]) <= 1e-5 * abs(ref["LL"]) + 1e-6
-    m, m_ref = host(out["model"]).reshape(-1), ref["model"].reshape(-1)
-    cov = ref["den"] >= 1e-3 * ref["den"].max()
-    rel = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-6 * np.abs(m_ref).max())
-    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2
-    assert np.all(m[ref["den"] == 0] == 0)
+    gates.model_gate(host(out["model"]), ref, out["weighted"], *out["geometry"], dl_max=float(m.max()), label="edge case")
 
 
 @pytest.fixture(scope="module")

@@ -12,6 +12,7 @@ import numpy as np
 import pytest
 import torch
 
+import gates
 from oracle import emc_oracle as o
 
 pytestmark = pytest.mark.gpu
@@ -119,7 +120,9 @@ def test_normalize_stagewise_1e6(case, ref):
 @pytest.mark.parametrize("flags", [0, emc.EMC_GEMM_1CTA, emc.EMC_DEBUG_SIMT], ids=["tcgen05-pair", "tcgen05-1cta", "simt"])
 def test_update_stagewise(case, ref, flags):
     inp = case.inp
-    p32 = ref["P"]
+    # emc_update takes P as libemc stores it: float32 subnormals count as 0 (EMC_P_MIN, include/emc.h; G20).  The oracle's
+    # update is given the same array, so that the comparison is of eq. (2.11) itself on every row, fragile ones included
+    p32 = gates.flushed(ref["P"])
     wn_ref, s_ref = o.update(p32, inp.counts, inp.mask)
     n_pat = p32.shape[1]
     p = torch.zeros((p32.shape[0], emc.ld_for(n_pat)), dtype=torch.float32, device="cuda")
@@ -153,17 +156,14 @@ def test_compress_stagewise(case, ref, weighted):
     assert np.all(m[den_ref == 0] == 0)
 
 
-def model_gate(m, ref, weighted):
-    """End-to-end gate on model': T3's 1e-5 is held stage-wise (test_compress_stagewise); end to
-    end the float32 rounding of L moves P by up to P (e^(2 dL) - 1) ~ 1e-5 ... 1e-3 relative, and eq. (2.10) turns a
-    slice whose s[r] crosses 0 on or off (tests/test_g20_threshold.py), so the worst voxel gets a loose bound and the
-    median a tight one."""
-    m, m_ref = m.reshape(-1), ref["model"].reshape(-1)
-    cov = ref["den"] >= 1e-3 * ref["den"].max()
-    rel = np.abs(m[cov] - m_ref[cov]) / (np.abs(m_ref[cov]) + 1e-6 * np.abs(m_ref).max())
-    assert rel.max() <= (2e-3 if weighted else 5e-2), f"max rel model error {rel.max():.3e}"
-    assert np.median(rel) <= 1e-4, f"median rel model error {np.median(rel):.3e}"
-    assert np.all(m[ref["den"] == 0] == 0)
+def model_gate(m, ref, weighted, case, quat=None, s_gpu=None, dl_max=0.0, label=""):
+    """End-to-end gate on model' (tests/gates.py): T3's 1e-5 is held stage-wise
+    (test_compress_stagewise); end to end the float32 rounding of L moves P by up to P (e^(2 dL) - 1) ~ 1e-5 ... 1e-3
+    relative.  The oracle keeps P as the plain float32 cast; the slices whose weights hang on float32 subnormals (where
+    libemc's flush-to-zero storage differs, G20) are identified on the oracle's P and gated by their footprint."""
+    inp = case.inp
+    gates.model_gate(m, ref, weighted, inp.q, case.quat if quat is None else quat, inp.mask, float(inp.counts.max()),
+                     s_gpu=s_gpu, dl_max=dl_max, label=label or f"{inp.cfg.name} {'eq2.12' if weighted else 'eq2.10'}")
 
 
 @pytest.mark.parametrize("uniform_null", [False, True], ids=["weights", "weights=NULL"])
@@ -197,7 +197,8 @@ def test_iterate_end_to_end(case, weighted, uniform_null):
     assert np.abs(p.sum(axis=0) - 1).max() <= 1e-5
     ll = float(host(out["loglik"])[0])
     assert abs(ll - r["LL"]) <= 1e-5 * abs(r["LL"])
-    model_gate(host(out["model"]), r, weighted)
+    dl_max = float(np.abs(l_it.astype(np.float64) - r["L"].astype(np.float64)).max())
+    model_gate(host(out["model"]), r, weighted, case, s_gpu=s_it, dl_max=dl_max)
 
 
 def test_iterate_pattern_chunks_against_the_chunked_oracle(inputs_cache):
@@ -216,7 +217,7 @@ def test_iterate_pattern_chunks_against_the_chunked_oracle(inputs_cache):
             emc.emc_check(out["ws"])
             ll = float(host(out["loglik"])[0])
             assert abs(ll - ref["LL"]) <= 1e-5 * abs(ref["LL"])
-            model_gate(host(out["model"]), ref, weighted)
+            model_gate(host(out["model"]), ref, weighted, c)
         # the oracle's own chunked and unchunked runs agree (pinned on the CPU too); the GPU's as well
         assert np.abs(ref["model"] - one["model"]).max() <= 1e-5 * np.abs(one["model"]).max()
     m = inp.model_init
@@ -385,8 +386,10 @@ def test_iterate_rot_chunked_matches_oracle(inputs_cache, name, chunk, weighted,
     scale = np.abs(m_ref).max()
     rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
     rel1 = np.abs(m - m1)[cov] / (np.abs(m1[cov]) + 1e-6 * scale)
-    # end to end: the same gates as test_iterate_end_to_end (P amplifies the float32 rounding of L)
-    assert np.median(rel) <= 1e-4 and rel.max() <= 5e-2, (np.median(rel), rel.max())
+    # end to end: the same gate as test_iterate_end_to_end (P amplifies the float32 rounding of L);
+    # the fragile slices are read off the unchunked oracle's P (the same numbers: test_oracle_pins)
+    full = o.iterate(inp.model_init, inp.q, inp.mask, c.quat, w, inp.counts, weighted=weighted)
+    model_gate(m, dict(ref, P=full["P"], model=ref["model"]), weighted, c, label=f"{name} rotation chunks of {chunk}")
     assert np.median(rel1) <= 1e-5 and rel1.max() <= 2e-2, (np.median(rel1), rel1.max())
     assert np.array_equal(m == 0, m1 == 0)
 
@@ -437,7 +440,10 @@ def test_iterate_sparse_photons_matches_oracle(inputs_cache, name, chunk, weight
     rel = np.abs(m - m_ref)[cov] / (np.abs(m_ref[cov]) + 1e-6 * scale)
     reld = np.abs(m - md)[cov] / (np.abs(md[cov]) + 1e-6 * scale)
     lim = (1e-4, 5e-2) if n_iter == 1 else (1e-3, 0.5)
-    assert np.median(rel) <= lim[0] and rel.max() <= lim[1], (np.median(rel), rel.max())
+    if n_iter == 1:
+        model_gate(m, ref, weighted, c, label=f"{name} photon lists")
+    else:       # the second iteration starts from models that already differ where a fragile slice (G20) took part or not
+        assert np.median(rel) <= lim[0] and rel.max() <= lim[1], (np.median(rel), rel.max())
     assert np.median(reld) <= lim[0] and reld.max() <= lim[1], (np.median(reld), reld.max())
     # a voxel that is exactly 0 on one side (responsibilities below 2^-40 of their chunk's maximum vanish from the dense
     # path's fp16 operand planes) is at most a rounding error of the largest voxel on the other

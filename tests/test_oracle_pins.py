@@ -429,25 +429,45 @@ def test_masked_counts_never_matter():
     assert np.array_equal(a["model"], b["model"]) and np.array_equal(a["P"], b["P"])
 
 
-def test_normalize_is_flush_to_zero_float32():
-    """G20: P is a float32 quantity stored flush-to-zero: what float32 holds as a normal number (>= 2^-126) is kept
-    with full precision, what would be a float32 subnormal is 0; a row made only of such values has s = 0.
-    Pinned against numpy's own float32: the kept set is exactly {p : float32(p) is a normal number}."""
-    assert o.P_MIN == 2.0 ** -126 == float(np.finfo(np.float32).tiny)
+def test_normalize_underflow_conventions():
+    """G20.  By default the oracle does nothing about float32 underflow: normalize returns the soft-max itself (pinned
+    against the exact quotient, no value touched) and P becomes float32 by numpy's own cast at the stage boundary (gradual
+    underflow).  p_min = P_MIN_FLUSH selects flush-to-zero storage, libemc's convention: what float32 holds as a normal
+    number (>= 2^-126) is kept with full precision, what would be a float32 subnormal is 0, a row made only of such values
+    has s = 0.  Pinned against numpy's own float32: the kept set is exactly {p : float32(p) is a normal number}."""
+    assert o.P_MIN == 0.0 and o.P_MIN_FLUSH == 2.0 ** -126 == float(np.finfo(np.float32).tiny)
     # ln 2^-126 = -87.34: e^-87 is a normal float32, e^-88 and e^-100 are subnormal, e^-104 underflows float32 altogether
     big_l = np.array([[0.0, 0.0, 0.0], [-60.0, -88.0, -104.0], [-87.0, -100.0, -86.0]], np.float32)
-    p, s, _ = o.normalize(big_l, np.full(3, 1 / 3, np.float32))
     exact = np.exp(big_l.astype(np.float64)) / np.exp(big_l.astype(np.float64)).sum(axis=0)
-    p32 = exact.astype(np.float32)
-    normal = p32 >= np.finfo(np.float32).tiny
+    p, s, _ = o.normalize(big_l, np.full(3, 1 / 3, np.float32))
+    assert np.all(p > 0) and np.allclose(p, exact, rtol=1e-14) and np.allclose(s, exact.sum(axis=1), rtol=1e-14)
+    p32 = p.astype(np.float32)                                     # the stage boundary: subnormals kept, 0 below 2^-150
+    assert p32[1, 1] > 0 and p32[2, 1] > 0 and p32[1, 2] == 0
+    p, s, _ = o.normalize(big_l, np.full(3, 1 / 3, np.float32), p_min=o.P_MIN_FLUSH)
+    normal = exact.astype(np.float32) >= np.finfo(np.float32).tiny
     assert np.array_equal(p > 0, normal)
     assert np.allclose(p[normal], exact[normal], rtol=1e-14)
     assert p[1, 1] == 0 and p[1, 2] == 0 and p[2, 1] == 0 and p[2, 0] > 0 and p[2, 2] > 0
     assert abs(p[:, 0].sum() - 1) < 1e-12 and s[1] == p[1, 0]
-    # a row entirely below the threshold drops out: s = 0
+    # a row entirely below the threshold drops out under flush-to-zero (s = 0) and stays in under the plain cast
     big_l = np.array([[0.0, 0.0], [-95.0, -99.0]], np.float32)
-    p, s, _ = o.normalize(big_l, np.full(2, 0.5, np.float32))
+    p, s, _ = o.normalize(big_l, np.full(2, 0.5, np.float32), p_min=o.P_MIN_FLUSH)
     assert s[1] == 0 and np.all(p[0] == 1.0)
+    p, s, _ = o.normalize(big_l, np.full(2, 0.5, np.float32))
+    assert s[1] > 0 and np.all(p.astype(np.float32)[1] > 0)
+    # iterate hands p_min through: the two conventions differ exactly on rows made of float32 subnormals
+    rng = np.random.default_rng(3)
+    n = 8
+    model = rng.random((n, n, n)).astype(np.float32) + 0.5
+    q = (rng.random((30, 3)).astype(np.float32) - 0.5) * 4
+    quat = rng.standard_normal((6, 4)).astype(np.float32)
+    quat /= np.linalg.norm(quat, axis=1, keepdims=True)
+    counts = rng.poisson(40.0, size=(5, 30)).astype(np.int32)
+    a = o.iterate(model, q, None, quat, np.full(6, 1 / 6, np.float32), counts)
+    b = o.iterate(model, q, None, quat, np.full(6, 1 / 6, np.float32), counts, p_min=o.P_MIN_FLUSH)
+    tiny = np.finfo(np.float32).tiny
+    assert np.array_equal(b["P"], np.where(a["P"] >= tiny, a["P"], 0))
+    assert np.array_equal(a["L"], b["L"]) and a["LL"] == b["LL"]
 
 
 # ---------------------------------------------------------------------------------------------- rotation chunks (NEXT-2)

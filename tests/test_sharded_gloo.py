@@ -41,7 +41,7 @@ class OracleBackend:
         z = (st[:, 2] * np.exp(key - m[None, :])).sum(axis=0)
         a = self.l32.astype(np.float64) + self.lw[:, None]
         p = np.exp(a - m[None, :]) / z[None, :]
-        p[p < o.P_MIN] = 0.0
+        p[p < o.P_MIN] = 0.0                                       # the oracle's default: nothing flushed (G20)
         wn, s = o.update(p.astype(np.float32), counts.numpy(), mask.numpy())
         n = model.shape[0]
         _, num, den = o.compress(wn, q.numpy(), quat.numpy(), mask.numpy(), n, slice_w=(s > 0).astype(np.float32))
