@@ -58,6 +58,9 @@ def parse():
                     help="> 0: time the paper's Gaussian likelihood with fluence (emc_iterate_gaussian, DESIGN.md section 11) "
                          "instead of the Poisson path; not the BASELINE.json metric, no cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="skip the `configs` sub-records (C1 with the step in a CUDA graph, C2, C4, C5) that the default "
+                         "single-GPU C3 run adds to its line")
     ap.add_argument("--no-comparator", action="store_true", help="skip the cuBLAS fp16 GEMM on the same operands")
     ap.add_argument("--cuda-graph", action="store_true",
                     help="capture the whole step into one CUDA graph and replay it for `value` (the launch-bound C1); "
@@ -339,10 +342,38 @@ def cublas_comparator(emc, torch, d_model0, d_q, d_mask, quat, d_counts, n_rep=4
 
 # ------------------------------------------------------------------------------ our arm
 
+def other_configs(args):
+    """Sub-records of the other BASELINE.json configs for the default line: each is this same script run on that config in
+    a process of its own (before the headline measurement allocates anything), so the numbers of DESIGN.md section 9's
+    table come from the same driver-timed run as `value`.  A config that fails or runs out of time is recorded as such."""
+    import subprocess
+
+    subs = {}
+    for name, extra, steps in (("C1", ["--cuda-graph"], 50), ("C2", [], 20), ("C4", [], 3), ("C5", [], 3)):
+        cmd = [sys.executable, str(ROOT / "bench.py"), "--config", name, "--steps", str(steps), "--warmup", "3",
+               "--no-cpu-baseline", "--no-comparator", "--no-configs"] + extra
+        t0 = time.perf_counter()
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
+            d = json.loads([ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1])
+            subs[name] = dict(workload=d["config"]["workload"], value=d["value"], unit=d["unit"], steps=d["steps"],
+                              ms_per_step=d["ms_per_step"], e2e=d["e2e"]["value"], gpu_launches=d["gpu_launches"],
+                              stage_ms={k: v["ms"] for k, v in d["stages"].items()}, clocks=d["clocks"],
+                              loglik_per_iteration=d["loglik_per_iteration"], cuda_graph=bool(extra),
+                              roofline_frac=d["roofline"]["frac"], wall_s=time.perf_counter() - t0)
+        except Exception as e:                                      # noqa: BLE001  (reported, never fatal for the headline)
+            subs[name] = dict(error=f"{type(e).__name__}: {str(e)[:200]}", wall_s=time.perf_counter() - t0)
+    return subs
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    configs_extra = None
+    if (args.config == "C3" and not args.no_configs and int(os.environ.get("WORLD_SIZE", "1")) == 1 and args.gpus == 1
+            and not (args.sparse or args.rot_chunk or args.cuda_graph or args.gaussian_sigma > 0 or args.photons > 0 or args.n_pat > 0)):
+        configs_extra = other_configs(args)
 
     from emc_inputs import CONFIGS, make_inputs
 
@@ -612,6 +643,8 @@ def main():
             line["comparator"] = cublas_comparator(emc, torch, d_model0, d_q, d_mask, plan[-1][0], d_counts)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(inp)
+        if configs_extra is not None:
+            line["configs"] = configs_extra
         print(json.dumps(line))
     if world > 1:
         dist.barrier()
